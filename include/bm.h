@@ -1,0 +1,162 @@
+/*
+ * bm.h -- C ABI of the B200-native ensemble Langevin integrator for Brownian motors
+ *         (hot path of arXiv 1409.4923, Spiechowicz, Kostur, Machura).
+ *
+ * What one call computes: "multiple realizations of [eq. 24] have to be simulated and then
+ * according to (18) an ensemble average must be performed", for many parameter values in one call
+ * (PAPER.md:397).  Each realization is integrated with the jump-adapted weak-order-2.0 predictor-corrector
+ * scheme (Alg. 1; jump adaptation :301) driven by Gaussian white noise (eq. 9), white
+ * Poissonian noise (eq. 3-8) and dichotomous noise (eq. 13-17); the observable is eq. (30).
+ * DESIGN.md section 3 lists every reading (R1..R12) taken where the paper is silent or garbled.
+ *
+ * Conventions
+ *   - Unless a function says HOST, every data pointer is a DEVICE pointer owned by the caller (e.g. the
+ *     storage of a torch tensor); the library never frees or retains it.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device-pointer
+ *     calls are asynchronous on `stream`, never synchronise and keep no global mutable state.
+ *   - Every call returns a bm_status; nothing throws.  There is no CPU fallback of any kind: without a
+ *     CUDA device the compute calls return BM_ERR_CUDA.
+ *   - Determinism: identical arguments give bit-identical outputs, independent of stream or of earlier
+ *     calls.  Path g = point*n_paths + p sees the same random words whatever the grid shape is.
+ */
+#ifndef BM_H
+#define BM_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define BM_VERSION 100 /* 0.1.0 */
+
+#if defined(__GNUC__)
+#define BM_API __attribute__((visibility("default")))
+#else
+#define BM_API
+#endif
+
+typedef enum {
+  BM_OK = 0,
+  BM_ERR_INVALID_ARG = 1, /* null pointer, n <= 0, dt <= 0, n_discard >= n_steps, bad enum, ... */
+  BM_ERR_UNSUPPORTED = 2, /* combination not compiled (see bm_simulate) */
+  BM_ERR_WORKSPACE = 3,   /* workspace too small or misaligned */
+  BM_ERR_CUDA = 4         /* a CUDA runtime call failed (no device, launch error, ...) */
+} bm_status;
+
+typedef enum { BM_OVERDAMPED = 0, BM_INERTIAL = 1 } bm_model;
+typedef enum { BM_F32 = 0, BM_F64 = 1 } bm_prec;
+/* fp32 only: where sin/cos/log/sqrt are evaluated.  SFU = MUFU approximations, FMA = polynomial
+ * evaluation of the force cosines on the FMA pipe.  AUTO = the variant measured faster. */
+typedef enum { BM_SINCOS_AUTO = 0, BM_SINCOS_SFU = 1, BM_SINCOS_FMA = 2 } bm_sincos;
+/* SINE2: V = A1 sin(2 pi x) + A2 sin(4 pi x), L = 1 (BASELINE.json configs).
+ * PWL:   eq. (2), scaled by A1, L = 2.      QUAD: V = A1 x^2/2 (no folding; OU pin). */
+typedef enum { BM_POT_SINE2 = 0, BM_POT_PWL = 1, BM_POT_QUAD = 2 } bm_potential;
+/* JUMP_ADAPTED: exact kick/flip times, Box-Muller Gaussians (the hot path).
+ * PAPER_LITERAL: Alg. 2/3/4 exactly as printed (three-point increments, grid-quantised countdowns,
+ * constant forces in the corrector line only); over-damped only. */
+typedef enum { BM_SCHEME_JUMP_ADAPTED = 0, BM_SCHEME_PAPER_LITERAL = 1 } bm_scheme;
+/* noise sources that are switched on; a source that is off ignores its parameters */
+enum { BM_NOISE_GAUSS = 1, BM_NOISE_POISSON = 2, BM_NOISE_DICH = 4 };
+
+/* One parameter point: 16 doubles = 128 B. */
+typedef struct {
+  double A1, A2;            /* potential amplitudes (see bm_potential) */
+  double F;                 /* static load (f of the inertial model) */
+  double D;                 /* Gaussian intensity: overdamped sqrt(2D) dW (eq. 9-10); inertial D := gamma*Q */
+  double lambda, zeta;      /* Poisson rate (eq. 4) and mean amplitude (eq. 5); bias -lambda*zeta (eq. 3, 6) */
+  double Fa, Fb;            /* dichotomous values -Fa, +Fb (eq. 13), both > 0 */
+  double mu_a, mu_b;        /* rate of leaving -Fa, rate of leaving +Fb (eq. 14) */
+  double gamma, amp, omega; /* inertial: friction, drive amplitude, drive angular frequency */
+  double x0_fixed;          /* >= 0: x0 = x0_fixed; < 0: x0 ~ U[0,L) */
+  double v0_lo, v0_hi;      /* inertial: v0 ~ U[v0_lo, v0_hi] */
+} bm_params;
+
+/* Per-point result: 8 doubles = 64 B.  Variances are unbiased (divide by n-1). */
+typedef struct {
+  double n;             /* paths averaged */
+  double mean_v, var_v; /* vbar_p = (x_p(t_f) - x_p(t_i))/(t_f - t_i), eq. (30); t_i = n_discard*dt */
+  double mean_xT, var_xT; /* unfolded x_p(t_f) */
+  double mean_jumps;    /* kicks + flips per path */
+  double mean_substeps; /* predictor-corrector sub-steps per path (= n_steps + events inside grid cells) */
+  double rsv;
+} bm_stats;
+
+typedef struct {
+  int32_t model;       /* bm_model */
+  int32_t prec;        /* bm_prec */
+  int32_t sincos;      /* bm_sincos */
+  int32_t potential;   /* bm_potential */
+  int32_t scheme;      /* bm_scheme */
+  int32_t noise;       /* OR of BM_NOISE_* */
+  int32_t block_threads; /* 0 = library default; else multiple of 32 in [32,256].  Part of the determinism contract
+                            (it fixes the reduction tree). */
+  int32_t reserved;
+  int64_t n_discard;   /* grid steps before t_i, 0 <= n_discard < n_steps (PAPER.md:423 uses n_steps/10) */
+  int64_t trace_steps; /* with out_trace: record the first trace_steps grid steps ... */
+  int64_t trace_paths; /* ... of global paths 0..trace_paths-1 (BM_F64 only) */
+} bm_config;
+
+/* per-path record written to out_paths: 6 doubles */
+enum { BM_OUT_XT = 0, BM_OUT_VT = 1, BM_OUT_VBAR = 2, BM_OUT_JUMPS = 3, BM_OUT_SUBSTEPS = 4, BM_OUT_XTI = 5,
+       BM_OUT_STRIDE = 6 };
+
+/* Bytes of device scratch bm_simulate needs (per-block partial sums of the two-level reduction).
+ * Returns 0 on invalid arguments. */
+BM_API size_t bm_workspace_bytes(const bm_config *cfg, int32_t n_points, int64_t n_paths);
+
+/*
+ * Simulate n_points x n_paths realizations for n_steps grid steps of length dt and reduce them.
+ *   params     [n_points]               device, read only
+ *   out_stats  [n_points]               device, written
+ *   out_paths  [n_points*n_paths][6]    device, optional (NULL to skip): BM_OUT_* per path, index g
+ *   out_trace  [trace_paths][trace_steps][2] device, optional: (x unfolded, v) after each grid step
+ *   workspace  device scratch of >= bm_workspace_bytes(...) bytes, 16-byte aligned
+ * Kernels launched on `stream`: the path kernel (a1-a10 of DESIGN.md section 2) and the grid pass of the
+ * reduction (a11).  Errors: BM_ERR_INVALID_ARG as listed above; BM_ERR_UNSUPPORTED for
+ * PAPER_LITERAL with BM_INERTIAL, BM_INERTIAL with a potential other than SINE2, out_trace with BM_F32;
+ * BM_ERR_WORKSPACE; BM_ERR_CUDA.
+ */
+BM_API bm_status bm_simulate(const bm_config *cfg, const bm_params *params, int32_t n_points, int64_t n_paths,
+                      int64_t n_steps, double dt, uint64_t seed, bm_stats *out_stats, double *out_paths,
+                      double *out_trace, void *workspace, size_t workspace_bytes, void *stream);
+
+/*
+ * HOST-pointer convenience entry (the end-to-end path): params, out_stats and out_paths (optional) are HOST
+ * buffers.  Allocates device memory, copies params in, runs bm_simulate on `stream`, copies the results
+ * out, synchronises the stream and frees the device memory.
+ */
+BM_API bm_status bm_simulate_host(const bm_config *cfg, const bm_params *params, int32_t n_points, int64_t n_paths,
+                           int64_t n_steps, double dt, uint64_t seed, bm_stats *out_stats, double *out_paths,
+                           void *stream);
+
+/* Raw Philox4x32-10 words (R1, R2): out[p][j][0..3] = call (seed, g = path0+p, stream_id, idx = idx0+j). */
+BM_API bm_status bm_philox_fill(uint64_t seed, uint64_t path0, int32_t n_paths, uint32_t stream_id, uint32_t idx0,
+                         int32_t n_idx, uint32_t *out, void *stream);
+
+/* Standard normals of the Gaussian stream (R3): out[p][j] = Gaussian number m0+j of path path0+p, produced by
+ * exactly the device code the path kernels use.  prec BM_F64: out is double*; BM_F32: out is float*.
+ * m0 must be a multiple of 4. */
+BM_API bm_status bm_gauss_fill(int32_t prec, int32_t sincos, uint64_t seed, uint64_t path0, int32_t n_paths, uint64_t m0,
+                        int32_t n_m, void *out, void *stream);
+
+/* Registers per thread, static shared memory and resident blocks per SM of the path kernel bm_simulate
+ * would launch for cfg (measurement aid; HOST outputs). */
+BM_API bm_status bm_kernel_info(const bm_config *cfg, int32_t *regs_per_thread, int32_t *block_threads,
+                         int32_t *blocks_per_sm, int32_t *sm_count);
+
+/* Pipe-throughput probes used by bench.py for the "alu" roofline: launches a kernel
+ * of `blocks` x `threads` threads each issuing iters x 64 dependent-chain-free operations of kind `op`
+ * (BM_PROBE_*); `sink` is a device buffer of >= blocks*threads floats.  The caller times it with CUDA events. */
+enum { BM_PROBE_FFMA = 0, BM_PROBE_MUFU_COS = 1, BM_PROBE_MUFU_LG2 = 2, BM_PROBE_MUFU_SQRT = 3, BM_PROBE_IMAD_WIDE = 4,
+       BM_PROBE_LOP3 = 5, BM_PROBE_DFMA = 6, BM_PROBE_I2F = 7, BM_PROBE_FADD = 8, BM_PROBE_MIX = 9,
+       BM_PROBE_COUNT = 10 };
+BM_API bm_status bm_pipe_probe(int32_t op, int32_t iters, int32_t blocks, int32_t threads, float *sink, void *stream);
+
+BM_API const char *bm_status_string(bm_status s);
+BM_API int bm_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,217 @@
+"""Thin ctypes binding of include/bm.h: same names, argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of libbm.so; PyTorch is used for device memory and streams.
+There is no CPU fallback: if libbm.so is missing or cannot be loaded, every call raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import workloads as W
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libbm.so")
+
+BM_OK, BM_ERR_INVALID_ARG, BM_ERR_UNSUPPORTED, BM_ERR_WORKSPACE, BM_ERR_CUDA = range(5)
+BM_OVERDAMPED, BM_INERTIAL = 0, 1
+BM_F32, BM_F64 = 0, 1
+BM_SINCOS_AUTO, BM_SINCOS_SFU, BM_SINCOS_FMA = 0, 1, 2
+BM_POT_SINE2, BM_POT_PWL, BM_POT_QUAD = 0, 1, 2
+BM_SCHEME_JUMP_ADAPTED, BM_SCHEME_PAPER_LITERAL = 0, 1
+BM_NOISE_GAUSS, BM_NOISE_POISSON, BM_NOISE_DICH = 1, 2, 4
+BM_OUT_XT, BM_OUT_VT, BM_OUT_VBAR, BM_OUT_JUMPS, BM_OUT_SUBSTEPS, BM_OUT_XTI, BM_OUT_STRIDE = 0, 1, 2, 3, 4, 5, 6
+(BM_PROBE_FFMA, BM_PROBE_MUFU_COS, BM_PROBE_MUFU_LG2, BM_PROBE_MUFU_SQRT, BM_PROBE_IMAD_WIDE, BM_PROBE_LOP3,
+ BM_PROBE_DFMA, BM_PROBE_I2F, BM_PROBE_FADD, BM_PROBE_MIX, BM_PROBE_COUNT) = range(11)
+
+EXPORTS = ("bm_workspace_bytes", "bm_simulate", "bm_simulate_host", "bm_philox_fill", "bm_gauss_fill",
+           "bm_kernel_info", "bm_pipe_probe", "bm_status_string", "bm_version")
+STATS_FIELDS = ("n", "mean_v", "var_v", "mean_xT", "var_xT", "mean_jumps", "mean_substeps", "rsv")
+
+
+class BmConfig(C.Structure):
+    _fields_ = [("model", C.c_int32), ("prec", C.c_int32), ("sincos", C.c_int32), ("potential", C.c_int32),
+                ("scheme", C.c_int32), ("noise", C.c_int32), ("block_threads", C.c_int32), ("reserved", C.c_int32),
+                ("n_discard", C.c_int64), ("trace_steps", C.c_int64), ("trace_paths", C.c_int64)]
+
+
+class BmError(RuntimeError):
+    def __init__(self, status, where):
+        self.status = status
+        super().__init__(f"{where}: {status_string(status)}")
+
+
+_lib = None
+
+
+def lib():
+    """Load libbm.so (fails loudly when it has not been built: there is no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_1409_4923_b200.build` "
+                               "(no CPU fallback exists)")
+        L = C.CDLL(LIB_PATH)
+        vp, i32, i64, u64, u32, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_uint64, C.c_uint32, C.c_double
+        cfgp = C.POINTER(BmConfig)
+        L.bm_workspace_bytes.argtypes = [cfgp, i32, i64]
+        L.bm_workspace_bytes.restype = C.c_size_t
+        L.bm_simulate.argtypes = [cfgp, vp, i32, i64, i64, dbl, u64, vp, vp, vp, vp, C.c_size_t, vp]
+        L.bm_simulate.restype = C.c_int
+        L.bm_simulate_host.argtypes = [cfgp, vp, i32, i64, i64, dbl, u64, vp, vp, vp]
+        L.bm_simulate_host.restype = C.c_int
+        L.bm_philox_fill.argtypes = [u64, u64, i32, u32, u32, i32, vp, vp]
+        L.bm_philox_fill.restype = C.c_int
+        L.bm_gauss_fill.argtypes = [i32, i32, u64, u64, i32, u64, i32, vp, vp]
+        L.bm_gauss_fill.restype = C.c_int
+        ip = C.POINTER(C.c_int32)
+        L.bm_kernel_info.argtypes = [cfgp, ip, ip, ip, ip]
+        L.bm_kernel_info.restype = C.c_int
+        L.bm_pipe_probe.argtypes = [i32, i32, i32, i32, vp, vp]
+        L.bm_pipe_probe.restype = C.c_int
+        L.bm_status_string.argtypes = [C.c_int]
+        L.bm_status_string.restype = C.c_char_p
+        L.bm_version.restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def status_string(s):
+    return lib().bm_status_string(int(s)).decode()
+
+
+def bm_version():
+    return lib().bm_version()
+
+
+def noise_mask(params):
+    """Noise sources a parameter table switches on (host-side helper; the C ABI takes the mask explicitly)."""
+    p = np.asarray(params)
+    m = 0
+    if np.any(p[:, W.COL["D"]] > 0):
+        m |= BM_NOISE_GAUSS
+    if np.any(p[:, W.COL["lambda"]] > 0):
+        m |= BM_NOISE_POISSON
+    if np.any(p[:, W.COL["mu_a"]] > 0):
+        m |= BM_NOISE_DICH
+    return m
+
+
+def make_config(model=BM_OVERDAMPED, prec=BM_F32, sincos=BM_SINCOS_AUTO, potential=BM_POT_SINE2,
+                scheme=BM_SCHEME_JUMP_ADAPTED, noise=BM_NOISE_GAUSS, block_threads=0, n_discard=0, trace_steps=0,
+                trace_paths=0):
+    return BmConfig(model, prec, sincos, potential, scheme, noise, block_threads, 0, n_discard, trace_steps,
+                    trace_paths)
+
+
+def _stream_ptr(stream):
+    import torch
+    if stream is None:
+        if not torch.cuda.is_available():
+            return None          # the library itself reports BM_ERR_CUDA; nothing is computed on the host
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream)
+
+
+def bm_workspace_bytes(cfg, n_points, n_paths):
+    return int(lib().bm_workspace_bytes(C.byref(cfg), n_points, n_paths))
+
+
+def bm_simulate(cfg, params, n_points, n_paths, n_steps, dt, seed, out_stats, out_paths=None, out_trace=None,
+                workspace=None, stream=None):
+    """Device-pointer call.  params/out_stats/out_paths/out_trace/workspace are CUDA torch tensors (float64 /
+    uint8 workspace).  Asynchronous on `stream` (default: torch's current stream)."""
+    import torch
+    assert params.is_cuda and params.dtype == torch.float64 and params.is_contiguous() and params.numel() == 16 * n_points
+    assert out_stats.is_cuda and out_stats.dtype == torch.float64 and out_stats.is_contiguous() and out_stats.numel() == 8 * n_points
+    need = bm_workspace_bytes(cfg, n_points, n_paths)
+    if workspace is None:
+        workspace = torch.empty(max(need, 16), dtype=torch.uint8, device=params.device)
+    op = C.c_void_p(out_paths.data_ptr()) if out_paths is not None else None
+    ot = C.c_void_p(out_trace.data_ptr()) if out_trace is not None else None
+    if out_paths is not None:
+        assert out_paths.is_cuda and out_paths.dtype == torch.float64 and out_paths.numel() == n_points * n_paths * BM_OUT_STRIDE
+    if out_trace is not None:
+        assert out_trace.is_cuda and out_trace.dtype == torch.float64 and out_trace.numel() == cfg.trace_paths * cfg.trace_steps * 2
+    rc = lib().bm_simulate(C.byref(cfg), C.c_void_p(params.data_ptr()), n_points, n_paths, n_steps, float(dt),
+                           int(seed), C.c_void_p(out_stats.data_ptr()), op, ot, C.c_void_p(workspace.data_ptr()),
+                           workspace.numel(), _stream_ptr(stream))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_simulate")
+    return workspace
+
+
+def bm_simulate_host(cfg, params, n_points, n_paths, n_steps, dt, seed, out_stats, out_paths=None, stream=None):
+    """HOST-pointer call: params/out_stats/out_paths are numpy float64 arrays (or pinned CPU torch tensors)."""
+    def ptr(a):
+        if a is None:
+            return None
+        if isinstance(a, np.ndarray):
+            assert a.dtype == np.float64 and a.flags.c_contiguous
+            return C.c_void_p(a.ctypes.data)
+        assert (not a.is_cuda) and a.is_contiguous()
+        return C.c_void_p(a.data_ptr())
+    rc = lib().bm_simulate_host(C.byref(cfg), ptr(params), n_points, n_paths, n_steps, float(dt), int(seed),
+                                ptr(out_stats), ptr(out_paths), _stream_ptr(stream))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_simulate_host")
+
+
+def bm_philox_fill(seed, path0, n_paths, stream_id, idx0, n_idx, out, stream=None):
+    import torch
+    assert out.is_cuda and out.dtype in (torch.int32, torch.uint32) and out.numel() == n_paths * n_idx * 4
+    rc = lib().bm_philox_fill(int(seed), int(path0), n_paths, stream_id, idx0, n_idx, C.c_void_p(out.data_ptr()),
+                              _stream_ptr(stream))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_philox_fill")
+
+
+def bm_gauss_fill(prec, sincos, seed, path0, n_paths, m0, n_m, out, stream=None):
+    import torch
+    assert out.is_cuda and out.numel() == n_paths * n_m
+    assert out.dtype == (torch.float64 if prec == BM_F64 else torch.float32)
+    rc = lib().bm_gauss_fill(prec, sincos, int(seed), int(path0), n_paths, int(m0), n_m, C.c_void_p(out.data_ptr()),
+                             _stream_ptr(stream))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_gauss_fill")
+
+
+def bm_kernel_info(cfg):
+    r, b, o, s = C.c_int32(), C.c_int32(), C.c_int32(), C.c_int32()
+    rc = lib().bm_kernel_info(C.byref(cfg), C.byref(r), C.byref(b), C.byref(o), C.byref(s))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_kernel_info")
+    return {"regs_per_thread": r.value, "block_threads": b.value, "blocks_per_sm": o.value, "sm_count": s.value}
+
+
+def bm_pipe_probe(op, iters, blocks, threads, sink, stream=None):
+    rc = lib().bm_pipe_probe(op, iters, blocks, threads, C.c_void_p(sink.data_ptr()), _stream_ptr(stream))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_pipe_probe")
+
+
+# ---- conveniences used by tests and bench.py (marshalling only) -------------------------------------------
+
+def config_for(w, prec, sincos=BM_SINCOS_AUTO, block_threads=0, trace_steps=0, trace_paths=0):
+    """bm_config of a workloads.Workload."""
+    return make_config(model=w.model, prec=prec, sincos=sincos, potential=w.potential, scheme=w.scheme,
+                       noise=noise_mask(w.params), block_threads=block_threads, n_discard=w.n_discard,
+                       trace_steps=trace_steps, trace_paths=trace_paths)
+
+
+def run_workload(w, prec, want_paths=False, sincos=BM_SINCOS_AUTO, block_threads=0, trace_steps=0, trace_paths=0,
+                 device="cuda:0"):
+    """Run a Workload through bm_simulate; returns (stats[n_points,8], paths or None, trace or None) as numpy."""
+    import torch
+    cfg = config_for(w, prec, sincos, block_threads, trace_steps, trace_paths)
+    dev = torch.device(device)
+    params = torch.from_numpy(np.ascontiguousarray(w.params)).to(dev)
+    stats = torch.zeros((w.n_points, 8), dtype=torch.float64, device=dev)
+    paths = torch.zeros((w.n_points * w.n_paths, BM_OUT_STRIDE), dtype=torch.float64, device=dev) if want_paths else None
+    trace = (torch.zeros((trace_paths, trace_steps, 2), dtype=torch.float64, device=dev)
+             if trace_steps and trace_paths else None)
+    with torch.cuda.device(dev):
+        bm_simulate(cfg, params, w.n_points, w.n_paths, w.n_steps, w.dt, w.seed, stats, paths, trace)
+        torch.cuda.synchronize()
+    return (stats.cpu().numpy(), paths.cpu().numpy() if paths is not None else None,
+            trace.cpu().numpy() if trace is not None else None)

@@ -1,0 +1,212 @@
+// api.cu -- the C ABI of include/bm.h: argument validation, kernel selection, launches.  No compute here.
+#include <cstdio>
+#include <cstring>
+
+#include "dispatch.cuh"
+
+using namespace bm;
+
+namespace {
+
+constexpr int DEFAULT_BLOCK_F32 = 128;
+constexpr int DEFAULT_BLOCK_F64 = 128;
+
+PhiloxKeys make_keys(uint64_t seed) {
+  PhiloxKeys K;
+  uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+  for (int r = 0; r < 10; ++r) {
+    K.k0[r] = k0;
+    K.k1[r] = k1;
+    k0 += PHILOX_W0;
+    k1 += PHILOX_W1;
+  }
+  return K;
+}
+
+bool valid_cfg(const bm_config *c) {
+  if (!c) return false;
+  if (c->model != BM_OVERDAMPED && c->model != BM_INERTIAL) return false;
+  if (c->prec != BM_F32 && c->prec != BM_F64) return false;
+  if (c->sincos < BM_SINCOS_AUTO || c->sincos > BM_SINCOS_FMA) return false;
+  if (c->potential < BM_POT_SINE2 || c->potential > BM_POT_QUAD) return false;
+  if (c->scheme != BM_SCHEME_JUMP_ADAPTED && c->scheme != BM_SCHEME_PAPER_LITERAL) return false;
+  if (c->noise < 0 || c->noise > 7) return false;
+  if (c->block_threads != 0 && (c->block_threads < 32 || c->block_threads > 256 || (c->block_threads & 31))) return false;
+  if (c->n_discard < 0 || c->trace_steps < 0 || c->trace_paths < 0) return false;
+  return true;
+}
+
+int block_threads_of(const bm_config *c) {
+  if (c->block_threads) return c->block_threads;
+  return c->prec == BM_F64 ? DEFAULT_BLOCK_F64 : DEFAULT_BLOCK_F32;
+}
+
+int resolve_sincos(const bm_config *c) {
+  // AUTO: the SFU variant measured faster on B200 for every config
+  return c->sincos == BM_SINCOS_FMA ? BM_SINCOS_FMA : BM_SINCOS_SFU;
+}
+
+bm_status pick_kernel(const bm_config *c, KernelFn *fn) {
+  *fn = nullptr;
+  if (c->scheme == BM_SCHEME_PAPER_LITERAL) return BM_ERR_UNSUPPORTED;  // NEXT row f1, not built yet
+  if (c->model == BM_INERTIAL && c->potential != BM_POT_SINE2) return BM_ERR_UNSUPPORTED;
+  if (c->prec == BM_F64) {
+    *fn = c->model == BM_OVERDAMPED ? pick_f64_overdamped(c->potential, c->noise)
+                                    : pick_f64_inertial(c->potential, c->noise);
+  } else {
+    const bool sfu = resolve_sincos(c) == BM_SINCOS_SFU;
+    if (c->model == BM_OVERDAMPED)
+      *fn = sfu ? pick_f32_overdamped_sfu(c->potential, c->noise) : pick_f32_overdamped_fma(c->potential, c->noise);
+    else
+      *fn = sfu ? pick_f32_inertial_sfu(c->potential, c->noise) : pick_f32_inertial_fma(c->potential, c->noise);
+  }
+  return *fn ? BM_OK : BM_ERR_UNSUPPORTED;
+}
+
+long long blocks_per_point_of(const bm_config *c, int64_t n_paths) {
+  const int bt = block_threads_of(c);
+  return (n_paths + bt - 1) / bt;
+}
+
+}  // namespace
+
+extern "C" {
+
+BM_API int bm_version(void) { return BM_VERSION; }
+
+BM_API const char *bm_status_string(bm_status s) {
+  switch (s) {
+    case BM_OK: return "BM_OK";
+    case BM_ERR_INVALID_ARG: return "BM_ERR_INVALID_ARG";
+    case BM_ERR_UNSUPPORTED: return "BM_ERR_UNSUPPORTED";
+    case BM_ERR_WORKSPACE: return "BM_ERR_WORKSPACE";
+    case BM_ERR_CUDA: return "BM_ERR_CUDA";
+    default: return "BM_ERR_UNKNOWN";
+  }
+}
+
+BM_API size_t bm_workspace_bytes(const bm_config *cfg, int32_t n_points, int64_t n_paths) {
+  if (!valid_cfg(cfg) || n_points <= 0 || n_paths <= 0) return 0;
+  const long long bpp = blocks_per_point_of(cfg, n_paths);
+  const long long grid = bpp * (long long)n_points;
+  if (grid > 0x7FFFFFFFLL) return 0;
+  return (size_t)grid * PARTIAL_STRIDE * sizeof(double);
+}
+
+BM_API bm_status bm_simulate(const bm_config *cfg, const bm_params *params, int32_t n_points, int64_t n_paths,
+                      int64_t n_steps, double dt, uint64_t seed, bm_stats *out_stats, double *out_paths,
+                      double *out_trace, void *workspace, size_t workspace_bytes, void *stream) {
+  if (!valid_cfg(cfg) || !params || !out_stats || n_points <= 0 || n_paths <= 0 || n_steps <= 0) return BM_ERR_INVALID_ARG;
+  if (!(dt > 0.0) || !(dt < 1e300)) return BM_ERR_INVALID_ARG;
+  if (cfg->n_discard >= n_steps) return BM_ERR_INVALID_ARG;
+  if (cfg->prec == BM_F32 && n_steps > 0x7FFFFFF0LL) return BM_ERR_INVALID_ARG;
+  if (out_trace && (cfg->trace_steps <= 0 || cfg->trace_paths <= 0)) return BM_ERR_INVALID_ARG;
+  if (out_trace && cfg->prec != BM_F64) return BM_ERR_UNSUPPORTED;
+  KernelFn fn;
+  const bm_status ps = pick_kernel(cfg, &fn);
+  if (ps != BM_OK) return ps;
+  const size_t need = bm_workspace_bytes(cfg, n_points, n_paths);
+  if (need == 0) return BM_ERR_INVALID_ARG;
+  if (!workspace || workspace_bytes < need || ((uintptr_t)workspace & 15)) return BM_ERR_WORKSPACE;
+
+  SimArgs a;
+  memset(&a, 0, sizeof(a));
+  a.params = params;
+  a.partials = reinterpret_cast<double *>(workspace);
+  a.out_paths = out_paths;
+  a.out_trace = out_trace;
+  a.n_paths = n_paths;
+  a.n_steps = n_steps;
+  a.n_discard = cfg->n_discard;
+  a.trace_steps = out_trace ? cfg->trace_steps : 0;
+  a.trace_paths = out_trace ? cfg->trace_paths : 0;
+  a.dt = dt;
+  a.n_points = n_points;
+  a.blocks_per_point = (int)blocks_per_point_of(cfg, n_paths);
+  a.keys = make_keys(seed);
+
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  const unsigned grid = (unsigned)((long long)a.blocks_per_point * n_points);
+  fn<<<grid, block_threads_of(cfg), 0, st>>>(a);  // a1: (point x path) -> grid
+  if (cudaGetLastError() != cudaSuccess) return BM_ERR_CUDA;
+  if (launch_grid_reduce(a.partials, n_points, a.blocks_per_point, out_stats, st) != cudaSuccess) return BM_ERR_CUDA;
+  return BM_OK;
+}
+
+BM_API bm_status bm_simulate_host(const bm_config *cfg, const bm_params *params, int32_t n_points, int64_t n_paths,
+                           int64_t n_steps, double dt, uint64_t seed, bm_stats *out_stats, double *out_paths,
+                           void *stream) {
+  if (!valid_cfg(cfg) || !params || !out_stats || n_points <= 0 || n_paths <= 0) return BM_ERR_INVALID_ARG;
+  const size_t ws = bm_workspace_bytes(cfg, n_points, n_paths);
+  if (ws == 0) return BM_ERR_INVALID_ARG;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  const size_t pb = (size_t)n_points * sizeof(bm_params), sb = (size_t)n_points * sizeof(bm_stats);
+  const size_t ob = out_paths ? (size_t)n_points * (size_t)n_paths * BM_OUT_STRIDE * sizeof(double) : 0;
+  void *d_params = nullptr, *d_stats = nullptr, *d_ws = nullptr, *d_paths = nullptr;
+  bm_status rc = BM_ERR_CUDA;
+  do {
+    if (cudaMalloc(&d_params, pb) != cudaSuccess) break;
+    if (cudaMalloc(&d_stats, sb) != cudaSuccess) break;
+    if (cudaMalloc(&d_ws, ws) != cudaSuccess) break;
+    if (ob && cudaMalloc(&d_paths, ob) != cudaSuccess) break;
+    if (cudaMemcpyAsync(d_params, params, pb, cudaMemcpyHostToDevice, st) != cudaSuccess) break;
+    rc = bm_simulate(cfg, (const bm_params *)d_params, n_points, n_paths, n_steps, dt, seed, (bm_stats *)d_stats,
+                     (double *)d_paths, nullptr, d_ws, ws, stream);
+    if (rc != BM_OK) break;
+    rc = BM_ERR_CUDA;
+    if (cudaMemcpyAsync(out_stats, d_stats, sb, cudaMemcpyDeviceToHost, st) != cudaSuccess) break;
+    if (ob && cudaMemcpyAsync(out_paths, d_paths, ob, cudaMemcpyDeviceToHost, st) != cudaSuccess) break;
+    if (cudaStreamSynchronize(st) != cudaSuccess) break;
+    rc = BM_OK;
+  } while (0);
+  if (rc == BM_ERR_CUDA) cudaGetLastError();
+  cudaFree(d_params); cudaFree(d_stats); cudaFree(d_ws); cudaFree(d_paths);
+  return rc;
+}
+
+BM_API bm_status bm_philox_fill(uint64_t seed, uint64_t path0, int32_t n_paths, uint32_t stream_id, uint32_t idx0,
+                         int32_t n_idx, uint32_t *out, void *stream) {
+  if (!out || n_paths <= 0 || n_idx <= 0 || ((uintptr_t)out & 15)) return BM_ERR_INVALID_ARG;
+  if ((long long)n_paths * n_idx > (1LL << 36)) return BM_ERR_INVALID_ARG;
+  const PhiloxKeys K = make_keys(seed);
+  return launch_philox_fill(K, path0, n_paths, stream_id, idx0, n_idx, out, reinterpret_cast<cudaStream_t>(stream)) ==
+                 cudaSuccess ? BM_OK : BM_ERR_CUDA;
+}
+
+BM_API bm_status bm_gauss_fill(int32_t prec, int32_t sincos, uint64_t seed, uint64_t path0, int32_t n_paths, uint64_t m0,
+                        int32_t n_m, void *out, void *stream) {
+  if (!out || n_paths <= 0 || n_m <= 0 || (m0 & 3)) return BM_ERR_INVALID_ARG;
+  if (prec != BM_F32 && prec != BM_F64) return BM_ERR_INVALID_ARG;
+  const PhiloxKeys K = make_keys(seed);
+  return launch_gauss_fill(prec, sincos, K, path0, n_paths, m0, n_m, out, reinterpret_cast<cudaStream_t>(stream)) ==
+                 cudaSuccess ? BM_OK : BM_ERR_CUDA;
+}
+
+BM_API bm_status bm_kernel_info(const bm_config *cfg, int32_t *regs_per_thread, int32_t *block_threads,
+                         int32_t *blocks_per_sm, int32_t *sm_count) {
+  if (!valid_cfg(cfg)) return BM_ERR_INVALID_ARG;
+  KernelFn fn;
+  const bm_status ps = pick_kernel(cfg, &fn);
+  if (ps != BM_OK) return ps;
+  cudaFuncAttributes attr;
+  if (cudaFuncGetAttributes(&attr, (const void *)fn) != cudaSuccess) { cudaGetLastError(); return BM_ERR_CUDA; }
+  const int bt = block_threads_of(cfg);
+  int nb = 0, dev = 0, sms = 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, (const void *)fn, bt, 0) != cudaSuccess) { cudaGetLastError(); return BM_ERR_CUDA; }
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+    cudaGetLastError();
+    return BM_ERR_CUDA;
+  }
+  if (regs_per_thread) *regs_per_thread = attr.numRegs;
+  if (block_threads) *block_threads = bt;
+  if (blocks_per_sm) *blocks_per_sm = nb;
+  if (sm_count) *sm_count = sms;
+  return BM_OK;
+}
+
+BM_API bm_status bm_pipe_probe(int32_t op, int32_t iters, int32_t blocks, int32_t threads, float *sink, void *stream) {
+  if (op < 0 || op >= BM_PROBE_COUNT || iters <= 0 || blocks <= 0 || threads <= 0 || threads > 1024 || !sink) return BM_ERR_INVALID_ARG;
+  return launch_probe(op, iters, blocks, threads, sink, reinterpret_cast<cudaStream_t>(stream)) == cudaSuccess ? BM_OK : BM_ERR_CUDA;
+}
+
+}  // extern "C"

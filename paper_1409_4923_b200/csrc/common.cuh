@@ -1,0 +1,143 @@
+// common.cuh -- pieces shared by every kernel of the CUDA path: launch arguments, Philox4x32-10 (a3),
+// the (n, mean, M2) merge of the deterministic ensemble reduction (a11).  sm_100a only.
+// Nothing here is shared with oracle/ (which has its own Philox, Box-Muller and stepper).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/bm.h"
+
+namespace bm {
+
+constexpr int STREAM_INIT = 0, STREAM_GAUSS = 1, STREAM_POISSON = 2, STREAM_DICH = 3;
+
+// Round keys of Philox4x32-10 (R1): k0 + i*W0, k1 + i*W1.  They depend on the seed only, so the host
+// computes them once and they reach the kernels through the parameter constant bank (no registers).
+struct PhiloxKeys {
+  uint32_t k0[10];
+  uint32_t k1[10];
+};
+
+struct SimArgs {
+  const bm_params *params;
+  double *partials;   // [grid][PARTIAL_STRIDE]
+  double *out_paths;  // optional [n_points*n_paths][6]
+  double *out_trace;  // optional [trace_paths][trace_steps][2]
+  long long n_paths;  // per point
+  long long n_steps;
+  long long n_discard;
+  long long trace_steps;
+  long long trace_paths;
+  double dt;
+  int n_points;
+  int blocks_per_point;
+  PhiloxKeys keys;
+};
+
+constexpr uint32_t PHILOX_M0 = 0xD2511F53u, PHILOX_M1 = 0xCD9E8D57u;
+constexpr uint32_t PHILOX_W0 = 0x9E3779B9u, PHILOX_W1 = 0xBB67AE85u;
+
+// PAPER.md:40 uses cuRAND with per-thread state in global memory (Alg. 5 steps 2, 6); here the generator is
+// stateless: (seed, path, stream, index) -> four words, recomputed in registers (reading R1, R2).
+// Counter = (idx, stream, g lo, g hi); one round: (hi0,lo0) = M0*c0, (hi1,lo1) = M1*c2,
+// c <- (hi1^c1^k0, lo1, hi0^c3^k1, lo0).
+__device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                               const PhiloxKeys &K) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const unsigned long long p0 = (unsigned long long)PHILOX_M0 * c0;  // IMAD.WIDE.U32
+    const unsigned long long p1 = (unsigned long long)PHILOX_M1 * c2;
+    const uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+    const uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+    c0 = hi1 ^ c1 ^ K.k0[r];  // LOP3
+    c1 = lo1;
+    c2 = hi0 ^ c3 ^ K.k1[r];
+    c3 = lo0;
+  }
+  return make_uint4(c0, c1, c2, c3);
+}
+
+__device__ __forceinline__ uint4 philox_call(const PhiloxKeys &K, unsigned long long g, uint32_t stream,
+                                             uint32_t idx) {
+  return philox4x32_10(idx, stream, (uint32_t)g, (uint32_t)(g >> 32), K);
+}
+
+// ---- deterministic ensemble reduction (a11) -----------------------------------------------------------
+// A leaf/partial carries n, mean and M2 (sum of squared deviations) of vbar and of x(T), plus plain sums of
+// the event and sub-step counts.  Two partials merge with Chan's pairwise update, which is exact up to
+// rounding whatever the split; the merge ORDER is fixed by (path index, block size) only, so results are
+// bit-reproducible from run to run (PAPER.md:412 names the parallel reduction as the optimisation not taken).
+constexpr int PARTIAL_STRIDE = 8;  // doubles
+struct Partial {
+  double n, mv, qv, mx, qx, sj, ss;
+};
+
+__device__ __forceinline__ Partial partial_zero() { return Partial{0, 0, 0, 0, 0, 0, 0}; }
+
+__device__ __forceinline__ Partial merge(const Partial &a, const Partial &b) {
+  Partial r;
+  r.n = a.n + b.n;
+  if (r.n == 0.0) return partial_zero();
+  const double fb = b.n / r.n;            // weight of b
+  const double w = a.n * fb;              // na*nb/n
+  const double dv = b.mv - a.mv, dx = b.mx - a.mx;
+  r.mv = a.mv + dv * fb;
+  r.mx = a.mx + dx * fb;
+  r.qv = a.qv + b.qv + dv * dv * w;
+  r.qx = a.qx + b.qx + dx * dx * w;
+  r.sj = a.sj + b.sj;
+  r.ss = a.ss + b.ss;
+  return r;
+}
+
+__device__ __forceinline__ Partial shfl_down(const Partial &p, int delta) {
+  Partial r;
+  r.n = __shfl_down_sync(0xffffffffu, p.n, delta);
+  r.mv = __shfl_down_sync(0xffffffffu, p.mv, delta);
+  r.qv = __shfl_down_sync(0xffffffffu, p.qv, delta);
+  r.mx = __shfl_down_sync(0xffffffffu, p.mx, delta);
+  r.qx = __shfl_down_sync(0xffffffffu, p.qx, delta);
+  r.sj = __shfl_down_sync(0xffffffffu, p.sj, delta);
+  r.ss = __shfl_down_sync(0xffffffffu, p.ss, delta);
+  return r;
+}
+
+// lane 0 ends with the merge of lanes 0..31 in the fixed order ((0,1),(2,3)),... (tree by lane index)
+__device__ __forceinline__ Partial warp_reduce(Partial p) {
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const Partial o = shfl_down(p, d);
+    p = merge(p, o);  // lanes whose partner is out of range merge garbage, but their value is never used
+  }
+  return p;
+}
+
+// Whole block -> one partial, written by thread 0 to dst[PARTIAL_STRIDE].  smem: 32 * 7 doubles.
+__device__ __forceinline__ void block_reduce_store(Partial p, double *dst) {
+  __shared__ double sm[32][7];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = (blockDim.x + 31) >> 5;
+  p = warp_reduce(p);
+  if (lane == 0) {
+    sm[warp][0] = p.n; sm[warp][1] = p.mv; sm[warp][2] = p.qv; sm[warp][3] = p.mx; sm[warp][4] = p.qx;
+    sm[warp][5] = p.sj; sm[warp][6] = p.ss;
+  }
+  __syncthreads();
+  if (warp == 0) {
+    Partial q = partial_zero();
+    if (lane < nwarps) q = Partial{sm[lane][0], sm[lane][1], sm[lane][2], sm[lane][3], sm[lane][4], sm[lane][5], sm[lane][6]};
+    q = warp_reduce(q);
+    if (lane == 0) {
+      dst[0] = q.n; dst[1] = q.mv; dst[2] = q.qv; dst[3] = q.mx; dst[4] = q.qx; dst[5] = q.sj; dst[6] = q.ss;
+      dst[7] = 0.0;
+    }
+  }
+}
+
+__device__ __forceinline__ Partial leaf(double vbar, double xT, double jumps, double substeps) {
+  return Partial{1.0, vbar, 0.0, xT, 0.0, jumps, substeps};
+}
+
+// launchers implemented per precision (sim_f64.cu / sim_f32_*.cu); return cudaError_t of the launch
+struct KernelInfo { int regs; int smem; int blocks_per_sm; };
+
+}  // namespace bm

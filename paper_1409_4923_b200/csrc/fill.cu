@@ -1,0 +1,102 @@
+// fill.cu -- small kernels around the path kernels: raw Philox words (a3), Gaussian-stream normals (a4),
+// the grid pass of the ensemble reduction (a11).
+#include "dispatch.cuh"
+#include "sim_f32.cuh"
+#include "sim_f64.cuh"
+
+namespace bm {
+
+__global__ void philox_fill_kernel(const __grid_constant__ PhiloxKeys K, unsigned long long path0, int n_paths,
+                                   uint32_t stream_id, uint32_t idx0, int n_idx, uint32_t *out) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= (long long)n_paths * n_idx) return;
+  const int p = (int)(i / n_idx), j = (int)(i - (long long)p * n_idx);
+  const uint4 w = philox_call(K, path0 + (unsigned long long)p, stream_id, idx0 + (uint32_t)j);
+  reinterpret_cast<uint4 *>(out)[i] = w;
+}
+
+cudaError_t launch_philox_fill(const PhiloxKeys &K, unsigned long long path0, int n_paths, uint32_t stream_id,
+                               uint32_t idx0, int n_idx, uint32_t *out, cudaStream_t st) {
+  const long long total = (long long)n_paths * n_idx;
+  const int threads = 256;
+  const long long blocks = (total + threads - 1) / threads;
+  philox_fill_kernel<<<(unsigned)blocks, threads, 0, st>>>(K, path0, n_paths, stream_id, idx0, n_idx, out);
+  return cudaGetLastError();
+}
+
+// one thread = one Gaussian block (4 normals) of one path
+template <int PREC>
+__global__ void gauss_fill_kernel(const __grid_constant__ PhiloxKeys K, unsigned long long path0, int n_paths,
+                                  unsigned long long m0, int n_blocks, int n_m, void *out) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= (long long)n_paths * n_blocks) return;
+  const int p = (int)(i / n_blocks), b = (int)(i - (long long)p * n_blocks);
+  const uint4 w = philox_call(K, path0 + (unsigned long long)p, STREAM_GAUSS, (uint32_t)((m0 >> 2) + b));
+  if (PREC == BM_F64) {
+    double q[4];
+    box_muller_f64(w.x, w.y, q[0], q[1]);
+    box_muller_f64(w.z, w.w, q[2], q[3]);
+    double *o = reinterpret_cast<double *>(out) + (long long)p * n_m;
+    for (int j = 0; j < 4; ++j)
+      if (4 * b + j < n_m) o[4 * b + j] = q[j];
+  } else {
+    float q[4];
+    box_muller_f32(w.x, w.y, q[0], q[1]);
+    box_muller_f32(w.z, w.w, q[2], q[3]);
+    float *o = reinterpret_cast<float *>(out) + (long long)p * n_m;
+    for (int j = 0; j < 4; ++j)
+      if (4 * b + j < n_m) o[4 * b + j] = q[j];
+  }
+}
+
+cudaError_t launch_gauss_fill(int prec, int /*sincos*/, const PhiloxKeys &K, unsigned long long path0, int n_paths,
+                              unsigned long long m0, int n_m, void *out, cudaStream_t st) {
+  const int n_blocks = (n_m + 3) / 4;
+  const long long total = (long long)n_paths * n_blocks;
+  const int threads = 256;
+  const unsigned blocks = (unsigned)((total + threads - 1) / threads);
+  if (prec == BM_F64)
+    gauss_fill_kernel<BM_F64><<<blocks, threads, 0, st>>>(K, path0, n_paths, m0, n_blocks, n_m, out);
+  else
+    gauss_fill_kernel<BM_F32><<<blocks, threads, 0, st>>>(K, path0, n_paths, m0, n_blocks, n_m, out);
+  return cudaGetLastError();
+}
+
+// Grid pass (a11): one warp per parameter point merges that point's per-block partials.  Lane l takes partials
+// l, l+32, ... in order, then the warp tree merges the 32 lane results: a fixed order for a given
+// (n_paths, block size), hence bit-reproducible.
+__global__ void grid_reduce_kernel(const double *__restrict__ partials, int n_points, int blocks_per_point,
+                                   bm_stats *__restrict__ out) {
+  const int warp = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
+  const int lane = threadIdx.x & 31;
+  if (warp >= n_points) return;
+  const double *src = partials + (long long)warp * blocks_per_point * PARTIAL_STRIDE;
+  Partial acc = partial_zero();
+  for (int b = lane; b < blocks_per_point; b += 32) {
+    const double *q = src + (long long)b * PARTIAL_STRIDE;
+    acc = merge(acc, Partial{q[0], q[1], q[2], q[3], q[4], q[5], q[6]});
+  }
+  acc = warp_reduce(acc);
+  if (lane == 0) {
+    bm_stats s;
+    s.n = acc.n;
+    s.mean_v = acc.mv;
+    s.var_v = acc.n > 1.0 ? acc.qv / (acc.n - 1.0) : 0.0;
+    s.mean_xT = acc.mx;
+    s.var_xT = acc.n > 1.0 ? acc.qx / (acc.n - 1.0) : 0.0;
+    s.mean_jumps = acc.n > 0.0 ? acc.sj / acc.n : 0.0;
+    s.mean_substeps = acc.n > 0.0 ? acc.ss / acc.n : 0.0;
+    s.rsv = 0.0;
+    out[warp] = s;
+  }
+}
+
+cudaError_t launch_grid_reduce(const double *partials, int n_points, int blocks_per_point, bm_stats *out,
+                               cudaStream_t st) {
+  const int threads = 128;  // 4 points per block
+  const unsigned blocks = (unsigned)((n_points + 3) / 4);
+  grid_reduce_kernel<<<blocks, threads, 0, st>>>(partials, n_points, blocks_per_point, out);
+  return cudaGetLastError();
+}
+
+}  // namespace bm

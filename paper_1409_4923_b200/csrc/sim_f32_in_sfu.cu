@@ -1,0 +1,28 @@
+// fp32 inertial path kernels, BM_SINCOS_SFU variant: all noise combinations.
+#include "sim_f32.cuh"
+#include "dispatch.cuh"
+
+namespace bm {
+
+template <int POT>
+static KernelFn pick_noise_in_sfu(int noise) {
+  switch (noise & 7) {
+    case 0: return bm_paths_f32<BM_INERTIAL, POT, 0, BM_SINCOS_SFU>;
+    case 1: return bm_paths_f32<BM_INERTIAL, POT, 1, BM_SINCOS_SFU>;
+    case 2: return bm_paths_f32<BM_INERTIAL, POT, 2, BM_SINCOS_SFU>;
+    case 3: return bm_paths_f32<BM_INERTIAL, POT, 3, BM_SINCOS_SFU>;
+    case 4: return bm_paths_f32<BM_INERTIAL, POT, 4, BM_SINCOS_SFU>;
+    case 5: return bm_paths_f32<BM_INERTIAL, POT, 5, BM_SINCOS_SFU>;
+    case 6: return bm_paths_f32<BM_INERTIAL, POT, 6, BM_SINCOS_SFU>;
+    default: return bm_paths_f32<BM_INERTIAL, POT, 7, BM_SINCOS_SFU>;
+  }
+}
+
+KernelFn pick_f32_inertial_sfu(int potential, int noise) {
+  switch (potential) {
+    case BM_POT_SINE2: return pick_noise_in_sfu<BM_POT_SINE2>(noise);
+    default: return nullptr;
+  }
+}
+
+}  // namespace bm

