@@ -1,0 +1,358 @@
+#!/usr/bin/env python
+"""bench.py -- path-steps/s of the hot path (bm_simulate) on B200, with the roofline and the oracle beside it.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload C1] [--prec f32]
+
+A "step" is ONE pass of the whole hot path over one batch of synthetic input: one bm_simulate call = path kernel
+(a1-a10 of DESIGN.md section 2) + grid pass of the reduction (a11) for the full workload.  Default workload is
+BASELINE.json configs[1] = C1 (65536 paths x 1e5 grid steps, overdamped ratchet + Poissonian + Gaussian noise),
+the configuration the metric is quoted on; the headline value is fp32, the same workload in fp64 is reported in
+`fp64`.  Inputs are synthetic (paper_1409_4923_b200/workloads.py, seeded); nothing is read from disk.
+
+Timing: every step is bracketed by CUDA events on the stream the kernels are launched on; W >= 3 warm-up steps;
+an L2 flush (256 MiB device write) runs between steps, outside the event pairs.  N > 1 = independent replicas
+("replicas only", rank r uses seed + r); barrier + synchronize on both sides, max over ranks.
+--impl reference times the fp64 CPU oracle (oracle/) on this box's host cores on a bounded sample.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "path-steps/s"
+UNIT = "path-steps/s"
+# Algorithmic SFU-class operations per overdamped sub-step in fp32: 3 force cosines + one half
+# of a Box-Muller pair (lg2, sqrt, sin, cos for two Gaussians) = 5; the inertial step adds the drive cosine = 6.
+# A kick adds 2 lg2 (waiting time, amplitude), a flip 1; sub-steps and events are COUNTED by the kernel.
+XU_OPS_PER_SUBSTEP = {0: 5.0, 1: 6.0}
+XU_LANES_PER_SM = 16          # MUFU lanes per SM per clock (4 per SM sub-partition); confirmed by bm_pipe_probe
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C1", choices=["C0", "C1", "C2", "C3", "C4"])
+    ap.add_argument("--prec", default="f32", choices=["f32", "f64"])
+    ap.add_argument("--sincos", default="auto", choices=["auto", "sfu", "fma"])
+    ap.add_argument("--block-threads", type=int, default=0)
+    ap.add_argument("--scale-steps", type=float, default=1.0, help="shrink n_steps (profiling runs only; flagged)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-fp64", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
+    return ap.parse_args()
+
+
+def workload_of(args):
+    from paper_1409_4923_b200 import workloads as W
+    w = W.CONFIGS[args.workload]()
+    if args.scale_steps != 1.0:
+        w = w.scaled(n_steps=max(8, int(w.n_steps * args.scale_steps)))
+    return w
+
+
+def workload_config(w, args, extra=None):
+    c = {"workload": f"{w.name}: BASELINE.json configs[{w.name[1]}]" if w.name[1:].isdigit() else w.name,
+         "n_points": int(w.n_points), "n_paths_per_point": int(w.n_paths), "n_steps": int(w.n_steps),
+         "dt": w.dt, "n_discard": int(w.n_discard), "seed": int(w.seed),
+         "model": "inertial" if w.model == 1 else "overdamped",
+         "l2": "inputs are 128 B/point of parameters (compute-bound path); 256 MiB L2 flush between steps, "
+               "outside the event pairs"}
+    if args.scale_steps != 1.0:
+        c["REDUCED"] = f"n_steps scaled by {args.scale_steps} (profiling run, not a bench value)"
+    if extra:
+        c.update(extra)
+    return c
+
+
+# ---- clocks sampled DURING the timed region ------------------------------------------------------------------
+
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index, self.rows, self.proc, self.thr = index, [], None, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.thr = threading.Thread(target=self._read, daemon=True)
+        self.thr.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        inside = [r for (t, r) in self.rows if t0 <= t <= t1 + 0.1] or [r for (_, r) in self.rows]
+        for r in inside:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---- the oracle, timed as it stands (cpu_baseline leg and --impl reference) -----------------------------------
+
+def oracle_time_sample(w, n_sample_paths):
+    """Oracle on the first n_sample_paths global paths of w at full length; returns seconds."""
+    from oracle import bm_oracle as orc
+    ids = np.arange(n_sample_paths, dtype=np.int64)
+    t0 = time.perf_counter()
+    orc.simulate(w.params, w.n_paths, w.n_steps, w.dt, w.seed, model=w.model, potential=w.potential,
+                 scheme=w.scheme, n_discard=w.n_discard, ids=ids)
+    return time.perf_counter() - t0
+
+
+def oracle_sample_size(w, target_seconds):
+    """Calibrate on 2 paths per core, then size the sample for ~target_seconds of wall time."""
+    from oracle import bm_oracle as orc
+    orc.lib()
+    cores = os.cpu_count() or 1
+    total = w.n_points * w.n_paths
+    n_cal = min(total, 2 * cores)
+    t = oracle_time_sample(w, n_cal)
+    per_path = max(t / n_cal, 1e-9)
+    n = int(target_seconds / per_path)
+    n = max(cores, (n // cores) * cores)
+    return min(n, total), orc.threads_used() or cores
+
+
+def cpu_baseline(w, target_seconds):
+    n, cores = oracle_sample_size(w, target_seconds)
+    t = oracle_time_sample(w, n)
+    from oracle import bm_oracle as orc
+    return {"value": n * w.n_steps / t, "unit": UNIT, "cores": int(orc.threads_used() or cores), "kind": "oracle",
+            "sample": f"first {n} of {w.n_points * w.n_paths} paths of {w.name} at full length "
+                      f"({w.n_steps} grid steps), fp64, gcc -O2 + OpenMP, {t:.1f} s"}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    w = workload_of(args)
+    per_step = max(1.0, min(args.cpu_seconds, 150.0 / max(1, args.steps + args.warmup)))
+    n, cores = oracle_sample_size(w, per_step)
+    for _ in range(args.warmup):
+        oracle_time_sample(w, n)
+    ts = [oracle_time_sample(w, n) for _ in range(args.steps)]
+    from oracle import bm_oracle as orc
+    cores = int(orc.threads_used() or cores)
+    t = sum(ts) / len(ts)
+    value = n * w.n_steps / t
+    sample = f"each step = first {n} of {w.n_points * w.n_paths} paths of {w.name} at full length ({w.n_steps} grid steps)"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(w, args, {"sample": sample}),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ---- our arm ---------------------------------------------------------------------------------------------------
+
+def sincos_of(B, name):
+    return {"auto": B.BM_SINCOS_AUTO, "sfu": B.BM_SINCOS_SFU, "fma": B.BM_SINCOS_FMA}[name]
+
+
+class Runner:
+    """Device buffers of one workload + the event-timed bm_simulate call (marshalling only)."""
+
+    def __init__(self, B, torch, w, prec, sincos, block_threads, seed, dev, stream):
+        self.B, self.torch, self.w, self.seed, self.stream, self.dev = B, torch, w, seed, stream, dev
+        self.cfg = B.config_for(w, prec, sincos, block_threads)
+        self.params = torch.from_numpy(np.ascontiguousarray(w.params)).to(dev)
+        self.stats = torch.zeros((w.n_points, 8), dtype=torch.float64, device=dev)
+        self.ws = torch.empty(max(16, B.bm_workspace_bytes(self.cfg, w.n_points, w.n_paths)), dtype=torch.uint8,
+                              device=dev)
+        # e2e: pinned host buffers, copied every step inside the timed region by bm_simulate_host
+        self.h_params = torch.from_numpy(np.ascontiguousarray(w.params)).pin_memory()
+        self.h_stats = torch.zeros((w.n_points, 8), dtype=torch.float64).pin_memory()
+
+    def device_step(self):
+        """One step with inputs resident in HBM; returns milliseconds (CUDA events on the launching stream)."""
+        t = self.torch
+        e0, e1 = t.cuda.Event(enable_timing=True), t.cuda.Event(enable_timing=True)
+        with t.cuda.stream(self.stream):
+            e0.record(self.stream)
+            self.B.bm_simulate(self.cfg, self.params, self.w.n_points, self.w.n_paths, self.w.n_steps, self.w.dt,
+                               self.seed, self.stats, workspace=self.ws, stream=self.stream)
+            e1.record(self.stream)
+        e1.synchronize()
+        return e0.elapsed_time(e1)
+
+    def host_step(self):
+        """One step through the HOST-pointer entry: H2D of params, kernels, D2H of stats inside the timed region."""
+        t = self.torch
+        e0, e1 = t.cuda.Event(enable_timing=True), t.cuda.Event(enable_timing=True)
+        t0 = time.perf_counter()
+        e0.record(self.stream)
+        self.B.bm_simulate_host(self.cfg, self.h_params, self.w.n_points, self.w.n_paths, self.w.n_steps, self.w.dt,
+                                self.seed, self.h_stats, stream=self.stream)
+        e1.record(self.stream)
+        e1.synchronize()
+        return max(e0.elapsed_time(e1), 1e3 * (time.perf_counter() - t0))
+
+
+def run_ours(args):
+    import torch
+    from paper_1409_4923_b200 import binding as B
+    B.lib()                                             # raises when libbm.so is missing: there is no fallback
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product has no CPU path)")
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        torch.cuda.set_device(local_rank)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    dev = torch.device("cuda", local_rank)
+    torch.cuda.set_device(dev)
+    stream = torch.cuda.Stream(device=dev)
+    w = workload_of(args)
+    prec = B.BM_F32 if args.prec == "f32" else B.BM_F64
+    sc = sincos_of(B, args.sincos)
+    seed = w.seed + rank                                # replicas only: independent ensembles, no collective
+    run = Runner(B, torch, w, prec, sc, args.block_threads, seed, dev, stream)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    info = B.bm_kernel_info(run.cfg)
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    for _ in range(max(args.warmup, 0)):
+        run.device_step()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    time.sleep(0.25)
+    barrier()
+    t_wall0 = time.time()
+    ms = []
+    for _ in range(args.steps):
+        flush.zero_()                                   # L2 flush, outside the event pair
+        torch.cuda.synchronize(dev)
+        ms.append(run.device_step())
+    barrier()
+    t_wall1 = time.time()
+    clocks = sampler.stop(t_wall0, t_wall1)
+    stats = run.stats.cpu().numpy().copy()
+    total_ms = float(sum(ms))
+    if dist is not None:
+        tt = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)       # timing plumbing only (max over ranks)
+        total_ms = float(tt.item())
+    ms_per_step = total_ms / args.steps
+    value = world * w.path_steps / (ms_per_step * 1e-3)
+
+    # e2e: same metric through the HOST-pointer C-ABI call (copies inside the timed region)
+    run.host_step()
+    barrier()
+    e2e_ms = [run.host_step() for _ in range(max(2, min(args.steps, 5)))]
+    e2e_total = float(np.mean(e2e_ms))
+    if dist is not None:
+        tt = torch.tensor([e2e_total], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        e2e_total = float(tt.item())
+    e2e = {"value": world * w.path_steps / (e2e_total * 1e-3), "unit": UNIT,
+           "h2d_bytes_per_step": int(run.h_params.numel() * 8), "d2h_bytes_per_step": int(run.h_stats.numel() * 8),
+           "ms_per_step": e2e_total, "call": "bm_simulate_host (cudaMalloc + H2D + kernels + D2H + sync per call)"}
+    if world == 1 and not np.array_equal(run.h_stats.numpy(), stats):
+        raise SystemExit("bench.py: host-pointer call and device-pointer call disagree (determinism contract broken)")
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    # roofline of the dominant kernel (the path kernel; the grid pass is < 0.1 % of the step): "alu" bound, XU pipe
+    substeps = float(stats[:, 6].mean())                # counted by the kernel
+    jumps = float(stats[:, 5].mean())
+    xu_per_path = XU_OPS_PER_SUBSTEP[w.model] * substeps + 2.0 * jumps
+    xu_ops = xu_per_path * w.n_points * w.n_paths       # algorithmic MUFU-class ops per launch (fp32 accounting)
+    sm_mhz = clocks.get("sm_max_mhz") or 1965.0
+    peak = XU_LANES_PER_SM * info["sm_count"] * sm_mhz * 1e6 / 1e9
+    achieved = xu_ops / (ms_per_step * 1e-3) / 1e9
+    roof = {"bound": "alu", "pipe": "xu (MUFU) for fp32; fp64 runs the same algorithm on the FP64 pipe",
+            "achieved": achieved, "peak": peak, "unit": "Gop/s", "frac": achieved / peak, "traffic": None,
+            "peak_source": f"derived: {XU_LANES_PER_SM} MUFU lanes/SM/clk x {info['sm_count']} SMs x {sm_mhz:.0f} MHz "
+                           "(max SM clock; lane count confirmed by bm_pipe_probe, DESIGN.md section 6)",
+            "ops_per_path_step": xu_per_path / w.n_steps, "kernel": "bm_paths_f32" if prec == B.BM_F32 else "bm_paths_f64",
+            "kernel_ms": ms_per_step, "regs_per_thread": info["regs_per_thread"],
+            "block_threads": info["block_threads"], "blocks_per_sm": info["blocks_per_sm"]}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": args.prec, "data": "synthetic",
+            "config": workload_config(w, args, {"parallelism": "replicas only" if world > 1 else "single GPU",
+                                                "sincos": args.sincos, "substeps_per_step": substeps / w.n_steps}),
+            "clocks": clocks, "e2e": e2e, "gpu_launches": 2 * args.steps, "roofline": roof,
+            "result": {"mean_v": float(stats[0, 1]), "var_v": float(stats[0, 2]), "mean_jumps": jumps}}
+
+    if world == 1 and not args.no_fp64 and args.prec == "f32":
+        r64 = Runner(B, torch, w, B.BM_F64, sc, args.block_threads, seed, dev, stream)
+        r64.device_step()
+        m64 = [r64.device_step() for _ in range(2)]
+        line["fp64"] = {"value": w.path_steps / (min(m64) * 1e-3), "unit": UNIT, "ms_per_step": float(min(m64)),
+                        "mean_v": float(r64.stats.cpu().numpy()[0, 1])}
+    if world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(w, args.cpu_seconds)
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
