@@ -13,6 +13,11 @@ KernelFn pick_f32_overdamped_sfu(int potential, int noise);
 KernelFn pick_f32_overdamped_fma(int potential, int noise);
 KernelFn pick_f32_inertial_sfu(int potential, int noise);
 KernelFn pick_f32_inertial_fma(int potential, int noise);
+// warp-specialised variants (Gaussian producer warps; launched with 2 x block_threads threads and
+// ws_ring_bytes(block_threads) of dynamic shared memory); nullptr when the combination has none
+KernelFn pick_f32_overdamped_ws(int sincos, int potential, int noise);
+KernelFn pick_f32_inertial_ws(int sincos, int potential, int noise);
+size_t ws_ring_bytes(int path_threads);
 
 // fills (fill.cu)
 cudaError_t launch_philox_fill(const PhiloxKeys &K, unsigned long long path0, int n_paths, uint32_t stream_id,

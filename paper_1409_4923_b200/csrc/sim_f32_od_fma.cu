@@ -7,14 +7,14 @@ namespace bm {
 template <int POT>
 static KernelFn pick_noise_od_fma(int noise) {
   switch (noise & 7) {
-    case 0: return bm_paths_f32<BM_OVERDAMPED, POT, 0, BM_SINCOS_FMA>;
-    case 1: return bm_paths_f32<BM_OVERDAMPED, POT, 1, BM_SINCOS_FMA>;
-    case 2: return bm_paths_f32<BM_OVERDAMPED, POT, 2, BM_SINCOS_FMA>;
-    case 3: return bm_paths_f32<BM_OVERDAMPED, POT, 3, BM_SINCOS_FMA>;
-    case 4: return bm_paths_f32<BM_OVERDAMPED, POT, 4, BM_SINCOS_FMA>;
-    case 5: return bm_paths_f32<BM_OVERDAMPED, POT, 5, BM_SINCOS_FMA>;
-    case 6: return bm_paths_f32<BM_OVERDAMPED, POT, 6, BM_SINCOS_FMA>;
-    default: return bm_paths_f32<BM_OVERDAMPED, POT, 7, BM_SINCOS_FMA>;
+    case 0: return bm_paths_f32<BM_OVERDAMPED, POT, 0, BM_SINCOS_FMA, false>;
+    case 1: return bm_paths_f32<BM_OVERDAMPED, POT, 1, BM_SINCOS_FMA, false>;
+    case 2: return bm_paths_f32<BM_OVERDAMPED, POT, 2, BM_SINCOS_FMA, false>;
+    case 3: return bm_paths_f32<BM_OVERDAMPED, POT, 3, BM_SINCOS_FMA, false>;
+    case 4: return bm_paths_f32<BM_OVERDAMPED, POT, 4, BM_SINCOS_FMA, false>;
+    case 5: return bm_paths_f32<BM_OVERDAMPED, POT, 5, BM_SINCOS_FMA, false>;
+    case 6: return bm_paths_f32<BM_OVERDAMPED, POT, 6, BM_SINCOS_FMA, false>;
+    default: return bm_paths_f32<BM_OVERDAMPED, POT, 7, BM_SINCOS_FMA, false>;
   }
 }
 

@@ -7,14 +7,14 @@ namespace bm {
 template <int POT>
 static KernelFn pick_noise_od_sfu(int noise) {
   switch (noise & 7) {
-    case 0: return bm_paths_f32<BM_OVERDAMPED, POT, 0, BM_SINCOS_SFU>;
-    case 1: return bm_paths_f32<BM_OVERDAMPED, POT, 1, BM_SINCOS_SFU>;
-    case 2: return bm_paths_f32<BM_OVERDAMPED, POT, 2, BM_SINCOS_SFU>;
-    case 3: return bm_paths_f32<BM_OVERDAMPED, POT, 3, BM_SINCOS_SFU>;
-    case 4: return bm_paths_f32<BM_OVERDAMPED, POT, 4, BM_SINCOS_SFU>;
-    case 5: return bm_paths_f32<BM_OVERDAMPED, POT, 5, BM_SINCOS_SFU>;
-    case 6: return bm_paths_f32<BM_OVERDAMPED, POT, 6, BM_SINCOS_SFU>;
-    default: return bm_paths_f32<BM_OVERDAMPED, POT, 7, BM_SINCOS_SFU>;
+    case 0: return bm_paths_f32<BM_OVERDAMPED, POT, 0, BM_SINCOS_SFU, false>;
+    case 1: return bm_paths_f32<BM_OVERDAMPED, POT, 1, BM_SINCOS_SFU, false>;
+    case 2: return bm_paths_f32<BM_OVERDAMPED, POT, 2, BM_SINCOS_SFU, false>;
+    case 3: return bm_paths_f32<BM_OVERDAMPED, POT, 3, BM_SINCOS_SFU, false>;
+    case 4: return bm_paths_f32<BM_OVERDAMPED, POT, 4, BM_SINCOS_SFU, false>;
+    case 5: return bm_paths_f32<BM_OVERDAMPED, POT, 5, BM_SINCOS_SFU, false>;
+    case 6: return bm_paths_f32<BM_OVERDAMPED, POT, 6, BM_SINCOS_SFU, false>;
+    default: return bm_paths_f32<BM_OVERDAMPED, POT, 7, BM_SINCOS_SFU, false>;
   }
 }
 

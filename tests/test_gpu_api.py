@@ -151,8 +151,13 @@ def test_host_pointer_entry_matches_device_entry(B):
 
 def test_kernel_info_and_probe(B):
     import torch
-    info = B.bm_kernel_info(B.config_for(W.c1(), B.BM_F32))
+    w = W.c1()
+    info = B.bm_kernel_info(B.config_for(w, B.BM_F32), w.n_points, w.n_paths)
     assert 16 <= info["regs_per_thread"] <= 255 and info["blocks_per_sm"] >= 1 and info["sm_count"] >= 1
+    assert info["launch_threads"] in (128, 256)
+    off = B.bm_kernel_info(B.config_for(w, B.BM_F32, warp_spec=B.BM_WS_OFF), w.n_points, w.n_paths)
+    on = B.bm_kernel_info(B.config_for(w, B.BM_F32, warp_spec=B.BM_WS_ON), w.n_points, w.n_paths)
+    assert not off["warp_spec"] and on["warp_spec"] and on["launch_threads"] == 2 * off["launch_threads"]
     sink = torch.zeros(148 * 256, dtype=torch.float32, device="cuda")
     for op in range(B.BM_PROBE_COUNT):
         B.bm_pipe_probe(op, 4, 148, 256, sink)
