@@ -28,7 +28,7 @@
 extern "C" {
 #endif
 
-#define BM_VERSION 100 /* 0.1.0 */
+#define BM_VERSION 101 /* 0.1.1 */
 
 #if defined(__GNUC__)
 #define BM_API __attribute__((visibility("default")))
@@ -56,11 +56,12 @@ typedef enum { BM_POT_SINE2 = 0, BM_POT_PWL = 1, BM_POT_QUAD = 2 } bm_potential;
  * PAPER_LITERAL: Alg. 2/3/4 exactly as printed (three-point increments, grid-quantised countdowns,
  * constant forces in the corrector line only); over-damped only. */
 typedef enum { BM_SCHEME_JUMP_ADAPTED = 0, BM_SCHEME_PAPER_LITERAL = 1 } bm_scheme;
-/* fp32 only.  ON: every path warp gets a producer warp in the same block that draws its Philox/Box-Muller normals
- * into a shared-memory ring (blocks of 2 x block_threads threads); OFF: each path thread draws its own.  The two give
- * bit-identical results.  AUTO = ON when the launch has few path warps per SM scheduler.
- * Ignored (OFF) without Gaussian noise, for BM_F64 and for potentials other than SINE2. */
-typedef enum { BM_WS_AUTO = 0, BM_WS_OFF = 1, BM_WS_ON = 2 } bm_warp_spec;
+/* fp32 only: how Philox words of the Gaussian stream become Box-Muller pairs (R3, R13).
+ * W32: one word per uniform (radius from w0, angle from w1, ...): four normals per call -- the oracle's assignment,
+ *      so a jump-free fp32 path follows the fp64 oracle's path (common random numbers).
+ * W16: radius from the top 23 bits and angle from the low 16 bits of ONE word: eight normals per call, half the
+ *      integer work.  AUTO = W16 (the variant measured faster).  Ignored for BM_F64. */
+typedef enum { BM_GAUSS_AUTO = 0, BM_GAUSS_W32 = 1, BM_GAUSS_W16 = 2 } bm_gauss;
 /* noise sources that are switched on; a source that is off ignores its parameters */
 enum { BM_NOISE_GAUSS = 1, BM_NOISE_POISSON = 2, BM_NOISE_DICH = 4 };
 
@@ -96,7 +97,7 @@ typedef struct {
   int32_t noise;       /* OR of BM_NOISE_* */
   int32_t block_threads; /* 0 = library default; else multiple of 32 in [32,256].  Part of the determinism contract
                             (it fixes the reduction tree). */
-  int32_t warp_spec;   /* bm_warp_spec: BM_F32 kernels with Gaussian noise may draw the normals in partner warps */
+  int32_t gauss;       /* bm_gauss (BM_F32 only) */
   int64_t n_discard;   /* grid steps before t_i, 0 <= n_discard < n_steps (PAPER.md:423 uses n_steps/10) */
   int64_t trace_steps; /* with out_trace: record the first trace_steps grid steps ... */
   int64_t trace_paths; /* ... of global paths 0..trace_paths-1 (BM_F64 only) */
@@ -140,16 +141,16 @@ BM_API bm_status bm_philox_fill(uint64_t seed, uint64_t path0, int32_t n_paths, 
                          int32_t n_idx, uint32_t *out, void *stream);
 
 /* Standard normals of the Gaussian stream (R3): out[p][j] = Gaussian number m0+j of path path0+p, produced by
- * exactly the device code the path kernels use.  prec BM_F64: out is double*; BM_F32: out is float*.
- * m0 must be a multiple of 4. */
-BM_API bm_status bm_gauss_fill(int32_t prec, int32_t sincos, uint64_t seed, uint64_t path0, int32_t n_paths, uint64_t m0,
+ * exactly the device code the path kernels use.  prec BM_F64: out is double*; BM_F32: out is float* and `gauss`
+ * (bm_gauss; AUTO = W16) selects the assignment.  m0 must be a multiple of 8. */
+BM_API bm_status bm_gauss_fill(int32_t prec, int32_t gauss, uint64_t seed, uint64_t path0, int32_t n_paths, uint64_t m0,
                         int32_t n_m, void *out, void *stream);
 
-/* Registers per thread, threads per block (2 x block_threads when warp specialised), resident blocks per SM, SM
- * count and whether the warp-specialised variant is selected, for the path kernel bm_simulate would launch for
- * (cfg, n_points, n_paths) (measurement aid; HOST outputs, each may be NULL). */
+/* Registers per thread, threads per block, resident blocks per SM, SM count and the Gaussian assignment selected
+ * (bm_gauss, never AUTO; 0 for BM_F64), for the path kernel bm_simulate would launch for (cfg, n_points, n_paths)
+ * (measurement aid; HOST outputs, each may be NULL). */
 BM_API bm_status bm_kernel_info(const bm_config *cfg, int32_t n_points, int64_t n_paths, int32_t *regs_per_thread,
-                         int32_t *launch_threads, int32_t *blocks_per_sm, int32_t *sm_count, int32_t *warp_spec);
+                         int32_t *launch_threads, int32_t *blocks_per_sm, int32_t *sm_count, int32_t *gauss);
 
 /* Pipe-throughput probes used by bench.py for the "alu" roofline: launches a kernel
  * of `blocks` x `threads` threads each issuing iters x 64 dependent-chain-free operations of kind `op`

@@ -20,7 +20,7 @@ BM_SINCOS_AUTO, BM_SINCOS_SFU, BM_SINCOS_FMA = 0, 1, 2
 BM_POT_SINE2, BM_POT_PWL, BM_POT_QUAD = 0, 1, 2
 BM_SCHEME_JUMP_ADAPTED, BM_SCHEME_PAPER_LITERAL = 0, 1
 BM_NOISE_GAUSS, BM_NOISE_POISSON, BM_NOISE_DICH = 1, 2, 4
-BM_WS_AUTO, BM_WS_OFF, BM_WS_ON = 0, 1, 2
+BM_GAUSS_AUTO, BM_GAUSS_W32, BM_GAUSS_W16 = 0, 1, 2
 BM_OUT_XT, BM_OUT_VT, BM_OUT_VBAR, BM_OUT_JUMPS, BM_OUT_SUBSTEPS, BM_OUT_XTI, BM_OUT_STRIDE = 0, 1, 2, 3, 4, 5, 6
 (BM_PROBE_FFMA, BM_PROBE_MUFU_COS, BM_PROBE_MUFU_LG2, BM_PROBE_MUFU_SQRT, BM_PROBE_IMAD_WIDE, BM_PROBE_LOP3,
  BM_PROBE_DFMA, BM_PROBE_I2F, BM_PROBE_FADD, BM_PROBE_MIX, BM_PROBE_COUNT) = range(11)
@@ -32,7 +32,7 @@ STATS_FIELDS = ("n", "mean_v", "var_v", "mean_xT", "var_xT", "mean_jumps", "mean
 
 class BmConfig(C.Structure):
     _fields_ = [("model", C.c_int32), ("prec", C.c_int32), ("sincos", C.c_int32), ("potential", C.c_int32),
-                ("scheme", C.c_int32), ("noise", C.c_int32), ("block_threads", C.c_int32), ("warp_spec", C.c_int32),
+                ("scheme", C.c_int32), ("noise", C.c_int32), ("block_threads", C.c_int32), ("gauss", C.c_int32),
                 ("n_discard", C.c_int64), ("trace_steps", C.c_int64), ("trace_paths", C.c_int64)]
 
 
@@ -100,8 +100,8 @@ def noise_mask(params):
 
 def make_config(model=BM_OVERDAMPED, prec=BM_F32, sincos=BM_SINCOS_AUTO, potential=BM_POT_SINE2,
                 scheme=BM_SCHEME_JUMP_ADAPTED, noise=BM_NOISE_GAUSS, block_threads=0, n_discard=0, trace_steps=0,
-                trace_paths=0, warp_spec=BM_WS_AUTO):
-    return BmConfig(model, prec, sincos, potential, scheme, noise, block_threads, warp_spec, n_discard, trace_steps,
+                trace_paths=0, gauss=BM_GAUSS_AUTO):
+    return BmConfig(model, prec, sincos, potential, scheme, noise, block_threads, gauss, n_discard, trace_steps,
                     trace_paths)
 
 
@@ -167,11 +167,11 @@ def bm_philox_fill(seed, path0, n_paths, stream_id, idx0, n_idx, out, stream=Non
         raise BmError(rc, "bm_philox_fill")
 
 
-def bm_gauss_fill(prec, sincos, seed, path0, n_paths, m0, n_m, out, stream=None):
+def bm_gauss_fill(prec, gauss, seed, path0, n_paths, m0, n_m, out, stream=None):
     import torch
     assert out.is_cuda and out.numel() == n_paths * n_m
     assert out.dtype == (torch.float64 if prec == BM_F64 else torch.float32)
-    rc = lib().bm_gauss_fill(prec, sincos, int(seed), int(path0), n_paths, int(m0), n_m, C.c_void_p(out.data_ptr()),
+    rc = lib().bm_gauss_fill(prec, gauss, int(seed), int(path0), n_paths, int(m0), n_m, C.c_void_p(out.data_ptr()),
                              _stream_ptr(stream))
     if rc != BM_OK:
         raise BmError(rc, "bm_gauss_fill")
@@ -183,7 +183,7 @@ def bm_kernel_info(cfg, n_points=1, n_paths=1 << 30):
     if rc != BM_OK:
         raise BmError(rc, "bm_kernel_info")
     return {"regs_per_thread": r.value, "launch_threads": b.value, "blocks_per_sm": o.value, "sm_count": s.value,
-            "warp_spec": bool(w.value)}
+            "gauss": int(w.value)}
 
 
 def bm_pipe_probe(op, iters, blocks, threads, sink, stream=None):
@@ -194,18 +194,18 @@ def bm_pipe_probe(op, iters, blocks, threads, sink, stream=None):
 
 # ---- conveniences used by tests and bench.py (marshalling only) -------------------------------------------
 
-def config_for(w, prec, sincos=BM_SINCOS_AUTO, block_threads=0, trace_steps=0, trace_paths=0, warp_spec=BM_WS_AUTO):
+def config_for(w, prec, sincos=BM_SINCOS_AUTO, block_threads=0, trace_steps=0, trace_paths=0, gauss=BM_GAUSS_AUTO):
     """bm_config of a workloads.Workload."""
     return make_config(model=w.model, prec=prec, sincos=sincos, potential=w.potential, scheme=w.scheme,
                        noise=noise_mask(w.params), block_threads=block_threads, n_discard=w.n_discard,
-                       trace_steps=trace_steps, trace_paths=trace_paths, warp_spec=warp_spec)
+                       trace_steps=trace_steps, trace_paths=trace_paths, gauss=gauss)
 
 
 def run_workload(w, prec, want_paths=False, sincos=BM_SINCOS_AUTO, block_threads=0, trace_steps=0, trace_paths=0,
-                 device="cuda:0", warp_spec=BM_WS_AUTO):
+                 device="cuda:0", gauss=BM_GAUSS_AUTO):
     """Run a Workload through bm_simulate; returns (stats[n_points,8], paths or None, trace or None) as numpy."""
     import torch
-    cfg = config_for(w, prec, sincos, block_threads, trace_steps, trace_paths, warp_spec)
+    cfg = config_for(w, prec, sincos, block_threads, trace_steps, trace_paths, gauss)
     dev = torch.device(device)
     params = torch.from_numpy(np.ascontiguousarray(w.params)).to(dev)
     stats = torch.zeros((w.n_points, 8), dtype=torch.float64, device=dev)

@@ -32,7 +32,7 @@ bool valid_cfg(const bm_config *c) {
   if (c->scheme != BM_SCHEME_JUMP_ADAPTED && c->scheme != BM_SCHEME_PAPER_LITERAL) return false;
   if (c->noise < 0 || c->noise > 7) return false;
   if (c->block_threads != 0 && (c->block_threads < 32 || c->block_threads > 256 || (c->block_threads & 31))) return false;
-  if (c->warp_spec < BM_WS_AUTO || c->warp_spec > BM_WS_ON) return false;
+  if (c->gauss < BM_GAUSS_AUTO || c->gauss > BM_GAUSS_W16) return false;
   if (c->n_discard < 0 || c->trace_steps < 0 || c->trace_paths < 0) return false;
   return true;
 }
@@ -47,62 +47,37 @@ int resolve_sincos(const bm_config *c) {
   return c->sincos == BM_SINCOS_FMA ? BM_SINCOS_FMA : BM_SINCOS_SFU;
 }
 
-// Path warps the launch puts on one SM scheduler if spread evenly (148 SMs x 4 schedulers is the B200; the
-// heuristic only needs the order of magnitude, so the device is not queried).
-double path_warps_per_scheduler(const bm_config *c, int64_t total_paths) {
-  const int bt = block_threads_of(c);
-  const double warps = (double)((total_paths + bt - 1) / bt) * (bt / 32);
-  return warps / (148.0 * 4.0);
+int resolve_gauss(const bm_config *c) {
+  // AUTO: eight normals per Philox call measured faster on B200 for every config
+  return c->gauss == BM_GAUSS_W32 ? BM_GAUSS_W32 : BM_GAUSS_W16;
 }
-
-// AUTO: the producer-warp variant measured SLOWER on C1 (19.0 ms vs 17.1 ms), so AUTO never
-// picks it; BM_WS_ON keeps it reachable as the measured alternative.
-constexpr double WS_AUTO_MAX_WARPS_PER_SCHEDULER = 0.0;
 
 struct Launch {
   KernelFn fn = nullptr;
-  int threads = 0;      // threads per block of the launch (2 x block_threads when warp specialised)
-  size_t smem = 0;      // dynamic shared memory
-  bool ws = false;
+  int threads = 0;  // threads per block
+  int gauss = 0;    // bm_gauss selected (fp32), 0 for fp64
 };
 
-bm_status pick_kernel(const bm_config *c, int64_t total_paths, Launch *L) {
+bm_status pick_kernel(const bm_config *c, Launch *L) {
   *L = Launch();
   if (c->scheme == BM_SCHEME_PAPER_LITERAL) return BM_ERR_UNSUPPORTED;  // NEXT row f1, not built yet
   if (c->model == BM_INERTIAL && c->potential != BM_POT_SINE2) return BM_ERR_UNSUPPORTED;
-  const int bt = block_threads_of(c);
-  L->threads = bt;
+  L->threads = block_threads_of(c);
   if (c->prec == BM_F64) {
     L->fn = c->model == BM_OVERDAMPED ? pick_f64_overdamped(c->potential, c->noise)
                                       : pick_f64_inertial(c->potential, c->noise);
   } else {
-    const int sc = resolve_sincos(c);
-    const bool sfu = sc == BM_SINCOS_SFU;
-    bool want_ws = c->warp_spec == BM_WS_ON ||
-                   (c->warp_spec == BM_WS_AUTO && path_warps_per_scheduler(c, total_paths) <= WS_AUTO_MAX_WARPS_PER_SCHEDULER);
-    if (want_ws) {
-      KernelFn f = c->model == BM_OVERDAMPED ? pick_f32_overdamped_ws(sc, c->potential, c->noise)
-                                             : pick_f32_inertial_ws(sc, c->potential, c->noise);
-      if (f) {
-        L->fn = f;
-        L->threads = 2 * bt;
-        L->smem = ws_ring_bytes(bt);
-        L->ws = true;
-      }
-    }
-    if (!L->fn) {
-      if (c->model == BM_OVERDAMPED)
-        L->fn = sfu ? pick_f32_overdamped_sfu(c->potential, c->noise) : pick_f32_overdamped_fma(c->potential, c->noise);
-      else
-        L->fn = sfu ? pick_f32_inertial_sfu(c->potential, c->noise) : pick_f32_inertial_fma(c->potential, c->noise);
-    }
+    const bool sfu = resolve_sincos(c) == BM_SINCOS_SFU;
+    const bool w16 = resolve_gauss(c) == BM_GAUSS_W16;
+    L->gauss = w16 ? BM_GAUSS_W16 : BM_GAUSS_W32;
+    if (c->model == BM_OVERDAMPED)
+      L->fn = sfu ? (w16 ? pick_f32_od_sfu_w16 : pick_f32_od_sfu_w32)(c->potential, c->noise)
+                  : (w16 ? pick_f32_od_fma_w16 : pick_f32_od_fma_w32)(c->potential, c->noise);
+    else
+      L->fn = sfu ? (w16 ? pick_f32_in_sfu_w16 : pick_f32_in_sfu_w32)(c->potential, c->noise)
+                  : (w16 ? pick_f32_in_fma_w16 : pick_f32_in_fma_w32)(c->potential, c->noise);
   }
   if (!L->fn) return BM_ERR_UNSUPPORTED;
-  if (L->smem > 48 * 1024 &&
-      cudaFuncSetAttribute((const void *)L->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L->smem) != cudaSuccess) {
-    cudaGetLastError();
-    return BM_ERR_CUDA;
-  }
   return BM_OK;
 }
 
@@ -146,7 +121,7 @@ BM_API bm_status bm_simulate(const bm_config *cfg, const bm_params *params, int3
   if (out_trace && (cfg->trace_steps <= 0 || cfg->trace_paths <= 0)) return BM_ERR_INVALID_ARG;
   if (out_trace && cfg->prec != BM_F64) return BM_ERR_UNSUPPORTED;
   Launch L;
-  const bm_status ps = pick_kernel(cfg, (int64_t)n_points * n_paths, &L);
+  const bm_status ps = pick_kernel(cfg, &L);
   if (ps != BM_OK) return ps;
   const size_t need = bm_workspace_bytes(cfg, n_points, n_paths);
   if (need == 0) return BM_ERR_INVALID_ARG;
@@ -170,7 +145,7 @@ BM_API bm_status bm_simulate(const bm_config *cfg, const bm_params *params, int3
 
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   const unsigned grid = (unsigned)((long long)a.blocks_per_point * n_points);
-  L.fn<<<grid, L.threads, L.smem, st>>>(a);  // a1: (point x path) -> grid
+  L.fn<<<grid, L.threads, 0, st>>>(a);  // a1: (point x path) -> grid
   if (cudaGetLastError() != cudaSuccess) return BM_ERR_CUDA;
   if (launch_grid_reduce(a.partials, n_points, a.blocks_per_point, out_stats, st) != cudaSuccess) return BM_ERR_CUDA;
   return BM_OK;
@@ -216,25 +191,26 @@ BM_API bm_status bm_philox_fill(uint64_t seed, uint64_t path0, int32_t n_paths, 
                  cudaSuccess ? BM_OK : BM_ERR_CUDA;
 }
 
-BM_API bm_status bm_gauss_fill(int32_t prec, int32_t sincos, uint64_t seed, uint64_t path0, int32_t n_paths, uint64_t m0,
+BM_API bm_status bm_gauss_fill(int32_t prec, int32_t gauss, uint64_t seed, uint64_t path0, int32_t n_paths, uint64_t m0,
                         int32_t n_m, void *out, void *stream) {
-  if (!out || n_paths <= 0 || n_m <= 0 || (m0 & 3)) return BM_ERR_INVALID_ARG;
+  if (!out || n_paths <= 0 || n_m <= 0 || (m0 & 7)) return BM_ERR_INVALID_ARG;
+  if (gauss < BM_GAUSS_AUTO || gauss > BM_GAUSS_W16) return BM_ERR_INVALID_ARG;
   if (prec != BM_F32 && prec != BM_F64) return BM_ERR_INVALID_ARG;
   const PhiloxKeys K = make_keys(seed);
-  return launch_gauss_fill(prec, sincos, K, path0, n_paths, m0, n_m, out, reinterpret_cast<cudaStream_t>(stream)) ==
+  return launch_gauss_fill(prec, gauss, K, path0, n_paths, m0, n_m, out, reinterpret_cast<cudaStream_t>(stream)) ==
                  cudaSuccess ? BM_OK : BM_ERR_CUDA;
 }
 
 BM_API bm_status bm_kernel_info(const bm_config *cfg, int32_t n_points, int64_t n_paths, int32_t *regs_per_thread,
-                         int32_t *launch_threads, int32_t *blocks_per_sm, int32_t *sm_count, int32_t *warp_spec) {
+                         int32_t *launch_threads, int32_t *blocks_per_sm, int32_t *sm_count, int32_t *gauss) {
   if (!valid_cfg(cfg) || n_points <= 0 || n_paths <= 0) return BM_ERR_INVALID_ARG;
   Launch L;
-  const bm_status ps = pick_kernel(cfg, (int64_t)n_points * n_paths, &L);
+  const bm_status ps = pick_kernel(cfg, &L);
   if (ps != BM_OK) return ps;
   cudaFuncAttributes attr;
   if (cudaFuncGetAttributes(&attr, (const void *)L.fn) != cudaSuccess) { cudaGetLastError(); return BM_ERR_CUDA; }
   int nb = 0, dev = 0, sms = 0;
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, (const void *)L.fn, L.threads, L.smem) != cudaSuccess) { cudaGetLastError(); return BM_ERR_CUDA; }
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, (const void *)L.fn, L.threads, 0) != cudaSuccess) { cudaGetLastError(); return BM_ERR_CUDA; }
   if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
     cudaGetLastError();
     return BM_ERR_CUDA;
@@ -243,7 +219,7 @@ BM_API bm_status bm_kernel_info(const bm_config *cfg, int32_t n_points, int64_t 
   if (launch_threads) *launch_threads = L.threads;
   if (blocks_per_sm) *blocks_per_sm = nb;
   if (sm_count) *sm_count = sms;
-  if (warp_spec) *warp_spec = L.ws ? 1 : 0;
+  if (gauss) *gauss = L.gauss;
   return BM_OK;
 }
 

@@ -24,15 +24,18 @@ cudaError_t launch_philox_fill(const PhiloxKeys &K, unsigned long long path0, in
   return cudaGetLastError();
 }
 
-// one thread = one Gaussian block (4 normals) of one path
-template <int PREC>
+// one thread = one Gaussian call of one path: NB = 4 normals (fp64, fp32 W32) or 8 (fp32 W16)
+template <int PREC, int GW>
 __global__ void gauss_fill_kernel(const __grid_constant__ PhiloxKeys K, unsigned long long path0, int n_paths,
                                   unsigned long long m0, int n_blocks, int n_m, void *out) {
+  constexpr int NB = (PREC == BM_F32 && GW == BM_GAUSS_W16) ? 8 : 4;
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= (long long)n_paths * n_blocks) return;
   const int p = (int)(i / n_blocks), b = (int)(i - (long long)p * n_blocks);
-  const uint4 w = philox_call(K, path0 + (unsigned long long)p, STREAM_GAUSS, (uint32_t)((m0 >> 2) + b));
+  const unsigned long long g = path0 + (unsigned long long)p;
+  const uint32_t call = (uint32_t)(m0 / NB + b);
   if (PREC == BM_F64) {
+    const uint4 w = philox_call(K, g, STREAM_GAUSS, call);
     double q[4];
     box_muller_f64(w.x, w.y, q[0], q[1]);
     box_muller_f64(w.z, w.w, q[2], q[3]);
@@ -40,25 +43,27 @@ __global__ void gauss_fill_kernel(const __grid_constant__ PhiloxKeys K, unsigned
     for (int j = 0; j < 4; ++j)
       if (4 * b + j < n_m) o[4 * b + j] = q[j];
   } else {
-    float q[4];
-    box_muller_f32(w.x, w.y, q[0], q[1]);
-    box_muller_f32(w.z, w.w, q[2], q[3]);
+    float q[NB];
+    gauss_block_standard_f32<GW>(K, g, call, q);
     float *o = reinterpret_cast<float *>(out) + (long long)p * n_m;
-    for (int j = 0; j < 4; ++j)
-      if (4 * b + j < n_m) o[4 * b + j] = q[j];
+    for (int j = 0; j < NB; ++j)
+      if (NB * b + j < n_m) o[NB * b + j] = q[j];
   }
 }
 
-cudaError_t launch_gauss_fill(int prec, int /*sincos*/, const PhiloxKeys &K, unsigned long long path0, int n_paths,
+cudaError_t launch_gauss_fill(int prec, int gauss, const PhiloxKeys &K, unsigned long long path0, int n_paths,
                               unsigned long long m0, int n_m, void *out, cudaStream_t st) {
-  const int n_blocks = (n_m + 3) / 4;
+  const int nb = (prec == BM_F32 && gauss != BM_GAUSS_W32) ? 8 : 4;
+  const int n_blocks = (n_m + nb - 1) / nb;
   const long long total = (long long)n_paths * n_blocks;
   const int threads = 256;
   const unsigned blocks = (unsigned)((total + threads - 1) / threads);
   if (prec == BM_F64)
-    gauss_fill_kernel<BM_F64><<<blocks, threads, 0, st>>>(K, path0, n_paths, m0, n_blocks, n_m, out);
+    gauss_fill_kernel<BM_F64, BM_GAUSS_W32><<<blocks, threads, 0, st>>>(K, path0, n_paths, m0, n_blocks, n_m, out);
+  else if (gauss == BM_GAUSS_W32)
+    gauss_fill_kernel<BM_F32, BM_GAUSS_W32><<<blocks, threads, 0, st>>>(K, path0, n_paths, m0, n_blocks, n_m, out);
   else
-    gauss_fill_kernel<BM_F32><<<blocks, threads, 0, st>>>(K, path0, n_paths, m0, n_blocks, n_m, out);
+    gauss_fill_kernel<BM_F32, BM_GAUSS_W16><<<blocks, threads, 0, st>>>(K, path0, n_paths, m0, n_blocks, n_m, out);
   return cudaGetLastError();
 }
 

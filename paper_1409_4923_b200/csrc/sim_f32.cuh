@@ -1,23 +1,30 @@
-// sim_f32.cuh -- fp32 path kernel (the throughput kernel), v2.  One thread = one realization; position, clocks,
+// sim_f32.cuh -- fp32 path kernel (the throughput kernel), v3.  One thread = one realization; position, clocks,
 // Gaussian cache and observable snapshot stay in registers for the whole run.
 //
 // Same method as the fp64 kernel (R1-R9), arranged for fp32 accuracy and for the SM's pipes
-// (profiles/r1_c1_f32_v1.md is the measurement this layout answers):
+// (profiles/r1_c1_f32_v2.md is the measurement this layout answers):
 //  * the position is carried as theta = 2 pi x / L (radians of the potential's phase), folded to [-pi, pi) with an
 //    int32 wrap counter by a round-to-nearest "magic add" (no F2I/FRND, which share the 16-lane XU
 //    pipe with MUFU).  In these units a force cosine is FMUL.RZ + MUFU.COS with no scaling multiply in front;
 //  * Alg. 1 is evaluated with the step length folded into the constants:
 //    x1 = (xs + h K0) + c (h K1 + h K2 c), so every stage is 2 FFMA behind its cosine;
-//  * time is (cell index n, offset tau in the cell); a jump clock is (cell index, offset in that cell), so nothing
-//    small is ever subtracted from something large;
-//  * a warp takes the FAST path (full grid step, all constants hoisted) when no lane has a jump or an observable
-//    boundary in its current cell (one vote), else every lane takes the GENERAL sub-step (a5-a8);
+//  * ALL lanes of a warp are always in the SAME grid cell n (the cell counter is warp-uniform).  A cell without a
+//    kick or flip in any lane is one FAST step with loop-invariant constants; NB such cells (one Philox call of
+//    normals) form one basic block when no lane has an event within them (one vote per block);
+//  * a lane with events inside the current cell integrates up to each event on its own (a divergent loop:
+//    sub-step of length h, a8, redraw of the clock), then every lane finishes the cell together with its own
+//    remaining length (a5).  The Gaussian of a grid cell comes from the Gaussian stream indexed by the CELL, the
+//    Gaussian of a sub-step that ends at an event from the spare word of that event's own Philox call (R13), so
+//    the normal cache never gets out of phase between lanes;
+//  * a jump clock is (cell index, offset in that cell), so nothing small is ever subtracted from something large;
 //  * the Box-Muller radius carries the noise amplitude (sqrt(-2 ln u) * sqrt(2 D dt) in one MUFU.SQRT);
-//  * uniforms come from the top 23 bits of a Philox word through a mantissa splice (no I2F);
+//  * uniforms come from Philox words through a mantissa splice (no I2F).  BM_GAUSS_W32: one word per uniform,
+//    four normals per call (the oracle's assignment R3, so a jump-free fp32 path follows the oracle's path);
+//    BM_GAUSS_W16: radius from the top 23 bits and angle from the low 16 bits of ONE word, eight normals per
+//    call -- half the integer work (IMAD.WIDE is a quarter-rate instruction on sm_100, DESIGN.md s.6);
 //  * transcendental functions: MUFU.{COS,SIN,LG2,SQRT} (SFU variant) or, for the force cosine,
 //    an even polynomial on the FMA pipe (FMA variant) -- a measured choice (DESIGN.md s.6).
-// fp32 results are judged statistically against the fp64 oracle (3 combined standard errors); because both
-// use the same Philox words for the same purpose they are in fact strongly correlated path by path.
+// fp32 results are judged statistically against the fp64 oracle (3 combined standard errors).
 #pragma once
 #include "common.cuh"
 
@@ -74,14 +81,6 @@ __device__ __forceinline__ void box_muller_f32(uint32_t wa, uint32_t wb, float &
   const float ang = turns12_f32(wb) * TWO_PI_F;
   g0 = r * cos_approx(ang);
   g1 = r * sin_approx(ang);
-}
-// The same pair left in factors, with the amplitude inside the root: r = sqrt(cn * lg2 u), cn = -2 ln2 * s^2,
-// so that s*g0 = r*c and s*g1 = r*s cost one FFMA each at the point of use.
-__device__ __forceinline__ void box_muller_factors_f32(uint32_t wa, uint32_t wb, float cn, float &r, float &c, float &s) {
-  r = sqrt_approx(cn * lg2_approx(u01_open0_f32(wa)));
-  const float ang = turns12_f32(wb) * TWO_PI_F;
-  c = cos_approx(ang);
-  s = sin_approx(ang);
 }
 
 // theta units: theta = SCALE * x; the potential has period PERIOD_TH in theta and PERIOD_X in x
@@ -164,64 +163,61 @@ __device__ __forceinline__ void schedule_f32(int n, float tau, float dt, float i
   off = f;
 }
 
+// ---- Gaussian cache (a3 + a4) ---------------------------------------------------------------------------------
+// A Box-Muller pair left in factors, with the amplitude inside the root: r = sqrt(cn * lg2 u), cn = -2 ln2 * s^2,
+// so that s*g0 = r*c and s*g1 = r*s cost one FFMA each at the point of use.
+struct Pair { float r, c, s; };
 
-// ---- warp specialisation: Gaussian producer warps feed the stepping (consumer) warps through shared memory -----
-// The three cosines of Alg. 1 are one serial chain (~90 cycles per step for a lone warp, measured) and C1 gives a
-// scheduler only 3-4 path warps, so a kernel that also draws its normals in the path warp is latency bound
-// (profiles/r1_c1_f32_v2.md).  Philox + Box-Muller have no serial dependence at all (counter-based, R1-R2), so they
-// move to a partner warp of the same block: consumer warp w steps 32 paths, producer warp w + W draws the normals
-// of exactly those paths (lane l <-> lane l) STAGE by STAGE into a ring; the hardware scheduler then fills the
-// consumer's latency bubbles with producer instructions.
-constexpr int RING_STAGES = 3;  // stages in flight per warp pair
-constexpr int RING_BLOCKS = 4;  // Gaussian blocks (4 normals each) per stage = 16 sub-steps
-struct GaussSlot {              // one Gaussian block of one warp: (ra, ca, sa, rb), (cb, sb) per lane; 768 B
-  float4 a[32];
-  float2 b[32];
-};
-struct PairRing {
-  GaussSlot slot[RING_STAGES][RING_BLOCKS];
-  unsigned long long full[RING_STAGES], empty[RING_STAGES];  // mbarriers, one arrival each (lane 0 of the warp)
-  int done;  // consumer -> producer: no more stages needed
-  int pad[3];
-};
-
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(void *bar, int count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+// R3 assignment: radius from word wa, angle from word wb (top 23 bits of each)
+__device__ __forceinline__ Pair pair_w32(uint32_t wa, uint32_t wb, float cn) {
+  Pair p;
+  p.r = sqrt_approx(cn * lg2_approx(u01_open0_f32(wa)));
+  const float ang = turns12_f32(wb) * TWO_PI_F;
+  p.c = cos_approx(ang);
+  p.s = sin_approx(ang);
+  return p;
 }
-__device__ __forceinline__ void mbar_arrive(void *bar) {  // release at CTA scope
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ bool mbar_try_wait(void *bar, uint32_t parity) {  // acquire at CTA scope
-  uint32_t ok;
-  asm volatile(
-      "{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
-      : "=r"(ok)
-      : "r"(smem_u32(bar)), "r"(parity)
-      : "memory");
-  return ok != 0;
-}
-// the same with a suspend-time hint (ns): the waiting warp leaves the issue slots to the others
-__device__ __forceinline__ bool mbar_try_wait_hint(void *bar, uint32_t parity, uint32_t ns) {
-  uint32_t ok;
-  asm volatile(
-      "{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\nselp.u32 %0, 1, 0, p;\n}"
-      : "=r"(ok)
-      : "r"(smem_u32(bar)), "r"(parity), "r"(ns)
-      : "memory");
-  return ok != 0;
+// compact assignment: radius from the top 23 bits of w (u on a 2^-23 grid), angle 2 pi k / 65536 from its low 16 bits
+// (k spliced into the low mantissa bits: t = 1 + k 2^-23, angle = (t - 1) * 2^7 * 2 pi in one FFMA, one rounding)
+__device__ __forceinline__ Pair pair_w16(uint32_t w, float cn) {
+  Pair p;
+  p.r = sqrt_approx(cn * lg2_approx(u01_open0_f32(w)));
+  const float t = __uint_as_float((w & 0xFFFFu) | 0x3F800000u);
+  const float ang = fmaf(t, 128.0f * TWO_PI_F, -128.0f * TWO_PI_F);
+  p.c = cos_approx(ang);
+  p.s = sin_approx(ang);
+  return p;
 }
 
-// Gaussian cache: one Philox call = two Box-Muller pairs = the normals of four consecutive sub-steps (R2, R3),
-// kept as (radius, cos, sin) factors with the full-step amplitude inside the radius.
-struct Gauss4 { float ra, ca, sa, rb, cb, sb; };
+// normals of NB = 4 (W32) or 8 (W16) consecutive grid cells: Gaussian-stream call b
+template <int GW> struct GaussBlock { Pair p[GW == BM_GAUSS_W16 ? 4 : 2]; };
 
-__device__ __forceinline__ Gauss4 draw_gauss_f32(const PhiloxKeys &K, unsigned long long g, uint32_t b, float cn) {
-  Gauss4 q;
+template <int GW>
+__device__ __forceinline__ GaussBlock<GW> draw_block_f32(const PhiloxKeys &K, unsigned long long g, uint32_t b, float cn) {
+  GaussBlock<GW> q;
   const uint4 w = philox_call(K, g, STREAM_GAUSS, b);
-  box_muller_factors_f32(w.x, w.y, cn, q.ra, q.ca, q.sa);
-  box_muller_factors_f32(w.z, w.w, cn, q.rb, q.cb, q.sb);
+  if (GW == BM_GAUSS_W16) {
+    q.p[0] = pair_w16(w.x, cn);
+    q.p[1] = pair_w16(w.y, cn);
+    q.p[2] = pair_w16(w.z, cn);
+    q.p[3] = pair_w16(w.w, cn);
+  } else {
+    q.p[0] = pair_w32(w.x, w.y, cn);
+    q.p[1] = pair_w32(w.z, w.w, cn);
+  }
   return q;
+}
+
+// Standard normals of call b in cell order (bm_gauss_fill)
+template <int GW>
+__device__ __forceinline__ void gauss_block_standard_f32(const PhiloxKeys &K, unsigned long long g, uint32_t b, float *out) {
+  const GaussBlock<GW> q = draw_block_f32<GW>(K, g, b, -2.0f * LN2_F);
+  constexpr int NP = GW == BM_GAUSS_W16 ? 4 : 2;
+#pragma unroll
+  for (int i = 0; i < NP; ++i) {
+    out[2 * i] = q.p[i].r * q.p[i].c;
+    out[2 * i + 1] = q.p[i].r * q.p[i].s;
+  }
 }
 
 // Per-point constants, fp32, theta units (theta = SCALE x)
@@ -238,304 +234,245 @@ struct PointF32 {
   float w_turns;     // omega/(2 pi): drive turns per unit time
 };
 
-// WS = warp specialised (blockDim.x = 2 x path threads; needs dynamic shared memory of one PairRing per path warp)
-template <int MODEL, int POT, int NOISE, int SINCOS, bool WS>
-__global__ void __launch_bounds__(512) bm_paths_f32(const __grid_constant__ SimArgs a) {
+template <int MODEL, int POT, int NOISE, int SINCOS, int GW>
+__global__ void __launch_bounds__(256) bm_paths_f32(const __grid_constant__ SimArgs a) {
   constexpr bool HAS_G = NOISE & BM_NOISE_GAUSS, HAS_P = NOISE & BM_NOISE_POISSON, HAS_D = NOISE & BM_NOISE_DICH;
   constexpr bool INERTIAL = MODEL == BM_INERTIAL;
-  constexpr bool RING = WS && HAS_G;  // without Gaussian noise there is nothing to produce
+  constexpr int NB = GW == BM_GAUSS_W16 ? 8 : 4;  // grid cells per Gaussian call
   constexpr float S = Units<POT>::SCALE;
   constexpr unsigned FULL = 0xffffffffu;
-  extern __shared__ __align__(16) unsigned char ring_mem[];
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int path_threads = RING ? (int)(blockDim.x >> 1) : (int)blockDim.x;
-  const int path_warps = path_threads >> 5;
-  const bool producer = RING && warp >= path_warps;
-  const int pair = producer ? warp - path_warps : warp;
-  PairRing *ring = RING ? reinterpret_cast<PairRing *>(ring_mem) + pair : nullptr;
+  constexpr int NEVER = 0x7FFFFFFF;
 
   const int point = blockIdx.x / a.blocks_per_point;
   const int chunk = blockIdx.x - point * a.blocks_per_point;
-  const long long p = (long long)chunk * path_threads + pair * 32 + lane;
+  const long long p = (long long)chunk * blockDim.x + threadIdx.x;
   const bool valid = p < a.n_paths;  // lanes past a ragged end run along (the warp votes) and contribute nothing
   const unsigned long long g =
       (unsigned long long)point * (unsigned long long)a.n_paths + (unsigned long long)(valid ? p : 0);
 
-  if (RING) {
-    if (!producer && lane == 0) {
-      for (int s = 0; s < RING_STAGES; ++s) { mbar_init(&ring->full[s], 1); mbar_init(&ring->empty[s], 1); }
-      ring->done = 0;
-    }
-    __syncthreads();
-  }
-
   const PhiloxKeys &K = a.keys;
   const bm_params bp = a.params[point];
   const double Dd = HAS_G ? bp.D : 0.0;
-  const float cn = (float)(-2.0 * M_LN2 * (double)S * (double)S * 2.0 * Dd * a.dt);
-  Partial mine = partial_zero();
-
-  if (producer) {
-    // ---- a3 + a4 for the partner warp: stage after stage until the consumer says stop -----------------------
-    uint32_t b = 0, stage = 0, phase = 0;
-    for (;;) {
-      bool stop = false;
-      while (!mbar_try_wait_hint(&ring->empty[stage], phase ^ 1u, 2000u)) {
-        if (*reinterpret_cast<volatile int *>(&ring->done)) { stop = true; break; }
-        __nanosleep(256);
-      }
-      if (stop || *reinterpret_cast<volatile int *>(&ring->done)) break;
-#pragma unroll
-      for (int i = 0; i < RING_BLOCKS; i += 2) {  // two independent Philox calls in flight
-        const Gauss4 q0 = draw_gauss_f32(K, g, b + i, cn);
-        const Gauss4 q1 = draw_gauss_f32(K, g, b + i + 1, cn);
-        GaussSlot &s0 = ring->slot[stage][i], &s1 = ring->slot[stage][i + 1];
-        s0.a[lane] = make_float4(q0.ra, q0.ca, q0.sa, q0.rb);
-        s0.b[lane] = make_float2(q0.cb, q0.sb);
-        s1.a[lane] = make_float4(q1.ra, q1.ca, q1.sa, q1.rb);
-        s1.b[lane] = make_float2(q1.cb, q1.sb);
-      }
-      b += RING_BLOCKS;
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&ring->full[stage]);
-      if (++stage == RING_STAGES) { stage = 0; phase ^= 1u; }
-    }
+  const float dt = (float)a.dt;
+  const float inv_dt = (float)(1.0 / a.dt);
+  const double lam = HAS_P ? bp.lambda : 0.0, zet = HAS_P ? bp.zeta : 0.0;
+  PointF32 P;
+  if (POT == BM_POT_SINE2) {
+    // -V' = -2 pi A1 c - 4 pi A2 (2 c^2 - 1)
+    P.kk1 = (float)((double)S * (-2.0 * M_PI * bp.A1));
+    P.kk2 = (float)((double)S * (-8.0 * M_PI * bp.A2));
+    P.base = (float)((double)S * (bp.F - lam * zet + 4.0 * M_PI * bp.A2));
   } else {
-    const float dt = (float)a.dt;
-    const float inv_dt = (float)(1.0 / a.dt);
-    const double lam = HAS_P ? bp.lambda : 0.0, zet = HAS_P ? bp.zeta : 0.0;
-    PointF32 P;
-    if (POT == BM_POT_SINE2) {
-      // -V' = -2 pi A1 c - 4 pi A2 (2 c^2 - 1)
-      P.kk1 = (float)((double)S * (-2.0 * M_PI * bp.A1));
-      P.kk2 = (float)((double)S * (-8.0 * M_PI * bp.A2));
-      P.base = (float)((double)S * (bp.F - lam * zet + 4.0 * M_PI * bp.A2));
+    P.kk1 = (float)bp.A1;
+    P.kk2 = 0.f;
+    P.base = (float)(bp.F - lam * zet);
+  }
+  P.Ga = (float)((double)S * (-bp.Fa));
+  P.Gb = (float)((double)S * bp.Fb);
+  P.cn = (float)(-2.0 * M_LN2 * (double)S * (double)S * 2.0 * Dd * a.dt);
+  P.inv_lam_dt = (lam > 0.0) ? (float)(1.0 / (lam * a.dt)) : 0.f;
+  P.zeta = (float)((double)S * zet);
+  P.inv_mua_dt = (HAS_D && bp.mu_a > 0.0) ? (float)(1.0 / (bp.mu_a * a.dt)) : 0.f;
+  P.inv_mub_dt = (HAS_D && bp.mu_b > 0.0) ? (float)(1.0 / (bp.mu_b * a.dt)) : 0.f;
+  P.gamma = (float)bp.gamma;
+  P.amp = (float)((double)S * bp.amp);
+  P.w_turns = (float)(bp.omega / (2.0 * M_PI));
+
+  // R4: initial condition
+  const uint4 wi = philox_call(K, g, STREAM_INIT, 0);
+  float x;  // theta; between sub-steps within about one period of [-P/2, P/2) (folded where it is used as a base)
+  int wraps = 0;
+  {
+    const double L0 = (POT == BM_POT_QUAD) ? 1.0 : Units<POT>::PERIOD_X;
+    const double x0 = (bp.x0_fixed >= 0.0) ? bp.x0_fixed : L0 * ((double)wi.x * (1.0 / 4294967296.0));
+    if (POT == BM_POT_QUAD) {
+      x = (float)x0;
+    } else {  // fold in fp64 once
+      const double k = rint(x0 / L0);
+      x = (float)((double)S * (x0 - k * L0));
+      wraps = (int)k;
+      fold_f32<POT>(x, wraps);
+    }
+  }
+  float v = 0.f;  // theta units per unit time
+  if (INERTIAL)
+    v = (float)((double)S * (bp.v0_lo + (bp.v0_hi - bp.v0_lo) * (((double)wi.y + 0.5) * (1.0 / 4294967296.0))));
+  int d = 0;
+  if (HAS_D) d = ((((double)wi.z + 0.5) * (1.0 / 4294967296.0)) < bp.mu_a / (bp.mu_a + bp.mu_b)) ? 1 : 0;
+
+  const int n_steps = (int)a.n_steps, n_discard = (int)a.n_discard;
+  // jump clocks: (cell index, offset inside that cell); NEVER = switched off at this point
+  int nP = NEVER, nD = NEVER;
+  float fP = 0.f, fD = 0.f, z = 0.f;
+  uint32_t kP = 0, kD = 0;
+  if (HAS_P && lam > 0.0) {
+    const uint4 w = philox_call(K, g, STREAM_POISSON, 0);
+    schedule_f32(0, 0.f, dt, inv_dt, neg_log_u_f32(w.x) * P.inv_lam_dt, nP, fP);
+    z = P.zeta * neg_log_u_f32(w.y);
+  }
+  if (HAS_D) {
+    const uint4 w = philox_call(K, g, STREAM_DICH, 0);
+    schedule_f32(0, 0.f, dt, inv_dt, neg_log_u_f32(w.x) * (d ? P.inv_mub_dt : P.inv_mua_dt), nD, fD);
+  }
+
+  // drive phase in 2^-64 turns per cell (inertial): exact integer accumulation, no float time.  n is the same in
+  // every lane, so ph and the drive at the cell boundaries are warp-uniform values.
+  unsigned long long ph = 0, dph = 0;
+  float drive0 = 0.f;  // SCALE * amp * cos(omega n dt)
+  if (INERTIAL) {
+    double turns_per_cell = bp.omega * a.dt / (2.0 * M_PI);
+    turns_per_cell -= floor(turns_per_cell);
+    dph = (unsigned long long)(turns_per_cell * 18446744073709551616.0);
+    drive0 = P.amp;  // cos(0)
+  }
+
+  int jumps = 0;  // events applied = sub-steps that ended inside a cell
+  float snap_x = x;
+  int snap_w = wraps;
+  float cst = P.base + (HAS_D ? (d ? P.Gb : P.Ga) : 0.f);
+  const float hh_full = 0.5f * dt;
+  // full-step constants of Alg. 1 (loop invariant; k0f, k0h follow cst across a flip)
+  const float k1f = dt * P.kk1, k2f = dt * P.kk2, k1h = hh_full * P.kk1, k2h = hh_full * P.kk2;
+  float k0f = dt * cst, k0h = hh_full * cst;
+
+  // ---- FAST: a full grid step without events in this lane (h = dt) --------------------------------------------
+  auto fast_cell = [&](float gr, float gc, bool do_fold) {
+    float xf = x;
+    if (do_fold || POT != BM_POT_SINE2) fold_f32<POT>(xf, wraps);
+    if (!INERTIAL) {
+      const float xs = HAS_G ? fmaf(gr, gc, xf) : xf;
+      x = pc_overdamped_f32<POT, SINCOS>(POT == BM_POT_SINE2 ? x : xf, xs, k0f, k1f, k2f, k0h, k1h, k2h);
     } else {
-      P.kk1 = (float)bp.A1;
-      P.kk2 = 0.f;
-      P.base = (float)(bp.F - lam * zet);
+      ph += dph;
+      const float drive1 = P.amp * cos_turns<SINCOS>(__uint_as_float((uint32_t)(ph >> 41) | 0x3F800000u));
+      const float vs = HAS_G ? fmaf(gr, gc, v) : v;
+      pc_inertial_f32<SINCOS>(x, v, xf, vs, dt, hh_full, P.gamma, P.kk1, P.kk2, cst + drive0, cst + drive1);
+      drive0 = drive1;
     }
-    P.Ga = (float)((double)S * (-bp.Fa));
-    P.Gb = (float)((double)S * bp.Fb);
-    P.cn = cn;
-    P.inv_lam_dt = (lam > 0.0) ? (float)(1.0 / (lam * a.dt)) : 0.f;
-    P.zeta = (float)((double)S * zet);
-    P.inv_mua_dt = (HAS_D && bp.mu_a > 0.0) ? (float)(1.0 / (bp.mu_a * a.dt)) : 0.f;
-    P.inv_mub_dt = (HAS_D && bp.mu_b > 0.0) ? (float)(1.0 / (bp.mu_b * a.dt)) : 0.f;
-    P.gamma = (float)bp.gamma;
-    P.amp = (float)((double)S * bp.amp);
-    P.w_turns = (float)(bp.omega / (2.0 * M_PI));
+  };
 
-    // R4: initial condition
-    const uint4 wi = philox_call(K, g, STREAM_INIT, 0);
-    float x;  // theta; between sub-steps within about one period of [-P/2, P/2) (folded where it is used as a base)
-    int wraps = 0;
-    {
-      const double L0 = (POT == BM_POT_QUAD) ? 1.0 : Units<POT>::PERIOD_X;
-      const double x0 = (bp.x0_fixed >= 0.0) ? bp.x0_fixed : L0 * ((double)wi.x * (1.0 / 4294967296.0));
-      if (POT == BM_POT_QUAD) {
-        x = (float)x0;
-      } else {  // fold in fp64 once
-        const double k = rint(x0 / L0);
-        x = (float)((double)S * (x0 - k * L0));
-        wraps = (int)k;
-        fold_f32<POT>(x, wraps);
-      }
+  // ---- a5-a8: a sub-step of length h from the lane's current state; dr0/dr1 = drive at its two ends -----------
+  auto sub_step = [&](float h, float noise, float dr0, float dr1) {
+    const float hh = 0.5f * h;
+    fold_f32<POT>(x, wraps);
+    if (!INERTIAL) {
+      x = pc_overdamped_f32<POT, SINCOS>(x, x + noise, h * cst, h * P.kk1, h * P.kk2, hh * cst, hh * P.kk1, hh * P.kk2);
+    } else {
+      const float xf = x;
+      pc_inertial_f32<SINCOS>(x, v, xf, v + noise, h, hh, P.gamma, P.kk1, P.kk2, cst + dr0, cst + dr1);
     }
-    float v = 0.f;  // theta units per unit time
-    if (INERTIAL)
-      v = (float)((double)S * (bp.v0_lo + (bp.v0_hi - bp.v0_lo) * (((double)wi.y + 0.5) * (1.0 / 4294967296.0))));
-    int d = 0;
-    if (HAS_D) d = ((((double)wi.z + 0.5) * (1.0 / 4294967296.0)) < bp.mu_a / (bp.mu_a + bp.mu_b)) ? 1 : 0;
+  };
 
-    const int n_steps = (int)a.n_steps, n_discard = (int)a.n_discard;
-    // jump clocks: (cell index, offset inside that cell); INT_MAX = never
-    int nP = 0x7FFFFFFF, nD = 0x7FFFFFFF;
-    float fP = 0.f, fD = 0.f, z = 0.f;
-    uint32_t kP = 0, kD = 0;
-    if (HAS_P && lam > 0.0) {
-      const uint4 w = philox_call(K, g, STREAM_POISSON, 0);
-      schedule_f32(0, 0.f, dt, inv_dt, neg_log_u_f32(w.x) * P.inv_lam_dt, nP, fP);
-      z = P.zeta * neg_log_u_f32(w.y);
-    }
-    if (HAS_D) {
-      const uint4 w = philox_call(K, g, STREAM_DICH, 0);
-      schedule_f32(0, 0.f, dt, inv_dt, neg_log_u_f32(w.x) * (d ? P.inv_mub_dt : P.inv_mua_dt), nD, fD);
-    }
-
-    // drive phase in 2^-64 turns per cell (inertial): exact integer accumulation, no float time
-    unsigned long long ph = 0, dph = 0;
-    float drive0 = 0.f;  // SCALE * amp * cos(omega t) at the current time
-    if (INERTIAL) {
-      double turns_per_cell = bp.omega * a.dt / (2.0 * M_PI);
-      turns_per_cell -= floor(turns_per_cell);
-      dph = (unsigned long long)(turns_per_cell * 18446744073709551616.0);
-      drive0 = P.amp;  // cos(0)
-    }
-
-    int n = valid ? 0 : n_steps;  // current cell; n == n_steps: finished
-    // the cell whose completion needs attention: last discarded cell (snapshot after it), then the last cell
-    int nB = (n_discard > 0) ? n_discard - 1 : n_steps - 1;
-    int nNext = valid ? min(nB, min(nP, nD)) : n_steps;
-    float tau = 0.f;
-    int jumps = 0, extra = 0;  // extra = sub-steps that ended inside a cell
-    float snap_x = x;
-    int snap_w = wraps;
-    float cst = P.base + (HAS_D ? (d ? P.Gb : P.Ga) : 0.f);
-    const float hh_full = 0.5f * dt;
-
-    // ---- FAST: a full grid step without events (h = dt: every step-scaled constant is loop invariant) ------
-    auto fast_step = [&](float gr, float gc, bool do_fold) {
-      float xf = x;
-      if (do_fold) fold_f32<POT>(xf, wraps);
-      if (!INERTIAL) {
-        const float xs = HAS_G ? fmaf(gr, gc, xf) : xf;
-        x = pc_overdamped_f32<POT, SINCOS>(x, xs, dt * cst, dt * P.kk1, dt * P.kk2, hh_full * cst, hh_full * P.kk1,
-                                           hh_full * P.kk2);
-      } else {
-        ph += dph;
-        const float drive1 = P.amp * cos_turns<SINCOS>(__uint_as_float((uint32_t)(ph >> 41) | 0x3F800000u));
-        const float vs = HAS_G ? fmaf(gr, gc, v) : v;
-        pc_inertial_f32<SINCOS>(x, v, xf, vs, dt, hh_full, P.gamma, P.kk1, P.kk2, cst + drive0, cst + drive1);
-        drive0 = drive1;
-      }
-      n++;
-    };
-
-    // ---- GENERAL: a5 sub-step to the earliest of {grid point, kick, flip} in this cell, then a8, a10.  Written
-    // with selects; the only branches are the (rare, divergent) kick and flip bodies.  A finished lane takes a
-    // zero-length sub-step, which changes nothing.
-    auto general_step = [&](float gr, float gc) {
-      const bool live = n < n_steps;
+  // ---- SLOW: a cell in which at least one lane of the warp has a kick or a flip --------------------------------
+  auto slow_cell = [&](int n, float gr, float gc) {
+    float tau = 0.f;         // the lane's offset inside cell n
+    float dr_tau = drive0;   // drive at that time
+    const float phf = INERTIAL ? __uint_as_float((uint32_t)(ph >> 41) | 0x3F800000u) : 0.f;  // 1 + frac(omega n dt / 2 pi)
+    // event lanes only (divergent): integrate to the event, apply it (a8), redraw its clock
+    while ((HAS_P && nP == n) || (HAS_D && nD == n)) {
       const bool inP = HAS_P && nP == n, inD = HAS_D && nD == n;
-      float end = dt;
-      if (inP) end = fminf(end, fP);
-      if (inD) end = fminf(end, fD);
-      if (!live) end = tau;
-      const bool at_grid = live && (end == dt);
-      const float h = end - tau, hh = 0.5f * h;
+      const bool isP = inP && (!inD || fP <= fD);  // a tie applies the kick first (R5)
+      const float te = isP ? fP : fD;
+      const float h = fmaxf(te - tau, 0.f);
+      // the event's own Philox call: .x next waiting time, .y next amplitude, .z Gaussian of this sub-step (R13)
+      const uint4 w = philox_call(K, g, isP ? STREAM_POISSON : STREAM_DICH, (isP ? kP : kD) + 1u);
       float noise = 0.f;
       if (HAS_G) {
-        const float rs = (h == dt) ? 1.0f : sqrt_approx(h * inv_dt);  // Var ~ h (A9)
-        noise = gr * gc * rs;
+        const float r = sqrt_approx(P.cn * lg2_approx(u01_open0_f32(w.z)) * (h * inv_dt));  // Var ~ h (A9)
+        const float t = __uint_as_float((w.z & 0xFFFFu) | 0x3F800000u);
+        noise = r * cos_approx(fmaf(t, 128.0f * TWO_PI_F, -128.0f * TWO_PI_F));
       }
-      fold_f32<POT>(x, wraps);
-      if (!INERTIAL) {
-        x = pc_overdamped_f32<POT, SINCOS>(x, x + noise, h * cst, h * P.kk1, h * P.kk2, hh * cst, hh * P.kk1, hh * P.kk2);
-      } else {
-        const unsigned long long ph1 = ph + dph;
-        const float t1 = at_grid ? __uint_as_float((uint32_t)(ph1 >> 41) | 0x3F800000u)
-                                 : fmaf(end, P.w_turns, __uint_as_float((uint32_t)(ph >> 41) | 0x3F800000u));
-        const float drive1 = P.amp * cos_turns<SINCOS>(t1);
-        const float xf = x;
-        pc_inertial_f32<SINCOS>(x, v, xf, v + noise, h, hh, P.gamma, P.kk1, P.kk2, cst + drive0, cst + drive1);
-        drive0 = drive1;
+      float dr1 = 0.f;
+      if (INERTIAL) dr1 = P.amp * cos_turns<SINCOS>(fmaf(te, P.w_turns, phf));
+      sub_step(h, noise, dr_tau, dr1);
+      dr_tau = dr1;
+      tau = te;
+      jumps++;
+      if (HAS_P && isP) {  // a8: kick
+        if (!INERTIAL) x += z; else v += z;
+        kP++;
+        schedule_f32(n, tau, dt, inv_dt, neg_log_u_f32(w.x) * P.inv_lam_dt, nP, fP);
+        z = P.zeta * neg_log_u_f32(w.y);
       }
-      tau = end;
-      if (HAS_P) {
-        if (inP && live && end == fP) {  // a8: kick
-          if (!INERTIAL) x += z; else v += z;
-          jumps++;
-          kP++;
-          const uint4 w = philox_call(K, g, STREAM_POISSON, kP);
-          schedule_f32(n, tau, dt, inv_dt, neg_log_u_f32(w.x) * P.inv_lam_dt, nP, fP);
-          z = P.zeta * neg_log_u_f32(w.y);
-        }
+      if (HAS_D && !isP) {  // a8: flip
+        d ^= 1;
+        kD++;
+        cst = P.base + (d ? P.Gb : P.Ga);
+        k0f = dt * cst;
+        k0h = hh_full * cst;
+        schedule_f32(n, tau, dt, inv_dt, neg_log_u_f32(w.x) * (d ? P.inv_mub_dt : P.inv_mua_dt), nD, fD);
       }
-      if (HAS_D) {
-        if (inD && live && end == fD) {  // a8: flip
-          d ^= 1;
-          jumps++;
-          kD++;
-          cst = P.base + (d ? P.Gb : P.Ga);
-          const uint4 w = philox_call(K, g, STREAM_DICH, kD);
-          schedule_f32(n, tau, dt, inv_dt, neg_log_u_f32(w.x) * (d ? P.inv_mub_dt : P.inv_mua_dt), nD, fD);
-        }
-      }
-      fold_f32<POT>(x, wraps);  // a kick may span several periods
-      n += at_grid ? 1 : 0;
-      tau = at_grid ? 0.f : tau;
-      extra += (live && !at_grid) ? 1 : 0;
-      if (INERTIAL) ph += at_grid ? dph : 0ull;
-      if (at_grid && n == n_discard) {  // a10: t_i
-        snap_x = x;
-        snap_w = wraps;
-      }
-      nB = (n < n_discard) ? n_discard - 1 : n_steps - 1;
-      // a lane inside a cell (tau > 0) stays on the GENERAL path until that cell is complete
-      nNext = (n >= n_steps) ? n_steps : ((at_grid || !live) ? min(nB, min(nP, nD)) : n);
-    };
+    }
+    // every lane: the rest of the cell (the whole cell for a lane without events)
+    const float h = dt - tau;
+    float noise = 0.f;
+    if (HAS_G) noise = gr * gc * ((tau == 0.f) ? 1.0f : sqrt_approx(h * inv_dt));
+    float drive1 = 0.f;
+    if (INERTIAL) {
+      ph += dph;
+      drive1 = P.amp * cos_turns<SINCOS>(__uint_as_float((uint32_t)(ph >> 41) | 0x3F800000u));
+    }
+    sub_step(h, noise, dr_tau, drive1);
+    drive0 = drive1;
+  };
 
-    // Every lane of a warp takes one sub-step per slot, so the Gaussian index m = 4 blk + j is warp-uniform.
-    // One vote per block of four slots, taken a block ahead: if no lane meets a jump, a boundary or its end within
-    // four cells the warp runs four FAST steps as one basic block; otherwise each slot votes FAST or GENERAL.
-    uint32_t blk = 0, stage = 0, phase = 0;
-    Gauss4 qn{0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-    if (HAS_G && !RING) qn = draw_gauss_f32(K, g, 0, P.cn);
-    bool fastable = !__any_sync(FULL, nNext - n < 4);
-    for (;;) {
-      if (RING) {
-        while (!mbar_try_wait(&ring->full[stage], phase)) {}
-      }
-#pragma unroll 1
-      for (int bb = 0; bb < RING_BLOCKS; ++bb) {
-        Gauss4 q = qn;
-        if (RING) {
-          const float4 qa = ring->slot[stage][bb].a[lane];
-          const float2 qb = ring->slot[stage][bb].b[lane];
-          q = Gauss4{qa.x, qa.y, qa.z, qa.w, qb.x, qb.y};
-        }
-        blk++;
-        if (fastable) {
-          fast_step(q.ra, q.ca, true);
-          fastable = !__any_sync(FULL, nNext - n < 7);  // n is 3 short of the block's end here
-          if (HAS_G && !RING) qn = draw_gauss_f32(K, g, blk, P.cn);
-          fast_step(q.ra, q.sa, false);
-          fast_step(q.rb, q.cb, false);
-          fast_step(q.rb, q.sb, false);
-        } else {
-          if (HAS_G && !RING) qn = draw_gauss_f32(K, g, blk, P.cn);
+  // ---- time loop: blocks of NB cells = one Gaussian call -------------------------------------------------------
+  GaussBlock<GW> qn;
 #pragma unroll
-          for (int j = 0; j < 4; ++j) {
-            const float gr = (j < 2) ? q.ra : q.rb;
-            const float gc = (j == 0) ? q.ca : (j == 1) ? q.sa : (j == 2) ? q.cb : q.sb;
-            if (!__any_sync(FULL, n == nNext)) fast_step(gr, gc, true);
-            else general_step(gr, gc);
+  for (int i = 0; i < NB / 2; ++i) qn.p[i] = Pair{0.f, 0.f, 0.f};
+  if (HAS_G) qn = draw_block_f32<GW>(K, g, 0, P.cn);
+  uint32_t blk = 0;
+  for (int n = 0; n < n_steps; n += NB) {
+    const GaussBlock<GW> q = qn;
+    blk++;
+    const int nEv = min(nP, nD);
+    const bool boundary = (n + NB > n_steps) || (n < n_discard && n_discard < n + NB);
+    const bool clean = !boundary && !__any_sync(FULL, nEv < n + NB);
+    if (n == n_discard) {  // a10: t_i on a block boundary
+      fold_f32<POT>(x, wraps);
+      snap_x = x;
+      snap_w = wraps;
+    }
+    if (clean) {
+      if (HAS_G) qn = draw_block_f32<GW>(K, g, blk, P.cn);
+#pragma unroll
+      for (int j = 0; j < NB; ++j) fast_cell(q.p[j >> 1].r, (j & 1) ? q.p[j >> 1].s : q.p[j >> 1].c, j == 0);
+    } else {
+      if (HAS_G) qn = draw_block_f32<GW>(K, g, blk, P.cn);
+#pragma unroll
+      for (int j = 0; j < NB; ++j) {
+        const int nc = n + j;
+        if (nc < n_steps) {
+          if (j > 0 && nc == n_discard) {  // a10: t_i inside a block
+            fold_f32<POT>(x, wraps);
+            snap_x = x;
+            snap_w = wraps;
           }
-          fastable = !__any_sync(FULL, nNext - n < 4);
+          const float gr = q.p[j >> 1].r, gc = (j & 1) ? q.p[j >> 1].s : q.p[j >> 1].c;
+          const bool ev = (HAS_P && nP == nc) || (HAS_D && nD == nc);
+          if ((HAS_P || HAS_D) && __any_sync(FULL, ev)) slow_cell(nc, gr, gc);
+          else fast_cell(gr, gc, true);
         }
       }
-      if (RING) {
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&ring->empty[stage]);
-        if (++stage == RING_STAGES) { stage = 0; phase ^= 1u; }
-      }
-      if (!__any_sync(FULL, n < n_steps)) break;
     }
-    if (RING) {
-      __syncwarp();
-      if (lane == 0) {
-        *reinterpret_cast<volatile int *>(&ring->done) = 1;
-        __threadfence_block();
-      }
-    }
+  }
 
-    if (valid) {
-      // a10: eq. (30), assembled once per path in fp64
-      fold_f32<POT>(x, wraps);
-      const double Ld = Units<POT>::PERIOD_X, iS = 1.0 / (double)S;
-      const double span = (double)(a.n_steps - a.n_discard) * a.dt;
-      const double xT = (double)wraps * Ld + (double)x * iS;
-      const double xTi = (double)snap_w * Ld + (double)snap_x * iS;
-      const double vbar = ((double)(wraps - snap_w) * Ld + ((double)x - (double)snap_x) * iS) / span;
-      const double msub = (double)a.n_steps + (double)extra;
-      if (a.out_paths) {
-        double *o = a.out_paths + g * BM_OUT_STRIDE;
-        o[BM_OUT_XT] = xT; o[BM_OUT_VT] = (double)v * iS; o[BM_OUT_VBAR] = vbar; o[BM_OUT_JUMPS] = (double)jumps;
-        o[BM_OUT_SUBSTEPS] = msub; o[BM_OUT_XTI] = xTi;
-      }
-      mine = leaf(vbar, xT, (double)jumps, msub);
+  Partial mine = partial_zero();
+  if (valid) {
+    // a10: eq. (30), assembled once per path in fp64
+    fold_f32<POT>(x, wraps);
+    const double Ld = Units<POT>::PERIOD_X, iS = 1.0 / (double)S;
+    const double span = (double)(a.n_steps - a.n_discard) * a.dt;
+    const double xT = (double)wraps * Ld + (double)x * iS;
+    const double xTi = (double)snap_w * Ld + (double)snap_x * iS;
+    const double vbar = ((double)(wraps - snap_w) * Ld + ((double)x - (double)snap_x) * iS) / span;
+    const double msub = (double)a.n_steps + (double)jumps;
+    if (a.out_paths) {
+      double *o = a.out_paths + g * BM_OUT_STRIDE;
+      o[BM_OUT_XT] = xT; o[BM_OUT_VT] = (double)v * iS; o[BM_OUT_VBAR] = vbar; o[BM_OUT_JUMPS] = (double)jumps;
+      o[BM_OUT_SUBSTEPS] = msub; o[BM_OUT_XTI] = xTi;
     }
+    mine = leaf(vbar, xT, (double)jumps, msub);
   }
   block_reduce_store(mine, a.partials + (long long)blockIdx.x * PARTIAL_STRIDE);
 }

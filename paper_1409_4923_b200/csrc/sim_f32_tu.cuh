@@ -1,0 +1,34 @@
+// sim_f32_tu.cuh -- body of the fp32 translation units: each sim_f32_<model>_<sincos>_<gauss>.cu instantiates the
+// path kernel for one (model, sincos, gauss) triple and every (potential, noise) combination, so nvcc compiles the
+// families in parallel.  The including file defines BM_TU_PICKER, BM_TU_MODEL, BM_TU_SINCOS, BM_TU_GAUSS.
+#include "sim_f32.cuh"
+#include "dispatch.cuh"
+
+namespace bm {
+
+template <int POT>
+static KernelFn pick_noise_tu(int noise) {
+  switch (noise & 7) {
+    case 0: return bm_paths_f32<BM_TU_MODEL, POT, 0, BM_TU_SINCOS, BM_TU_GAUSS>;
+    case 1: return bm_paths_f32<BM_TU_MODEL, POT, 1, BM_TU_SINCOS, BM_TU_GAUSS>;
+    case 2: return bm_paths_f32<BM_TU_MODEL, POT, 2, BM_TU_SINCOS, BM_TU_GAUSS>;
+    case 3: return bm_paths_f32<BM_TU_MODEL, POT, 3, BM_TU_SINCOS, BM_TU_GAUSS>;
+    case 4: return bm_paths_f32<BM_TU_MODEL, POT, 4, BM_TU_SINCOS, BM_TU_GAUSS>;
+    case 5: return bm_paths_f32<BM_TU_MODEL, POT, 5, BM_TU_SINCOS, BM_TU_GAUSS>;
+    case 6: return bm_paths_f32<BM_TU_MODEL, POT, 6, BM_TU_SINCOS, BM_TU_GAUSS>;
+    default: return bm_paths_f32<BM_TU_MODEL, POT, 7, BM_TU_SINCOS, BM_TU_GAUSS>;
+  }
+}
+
+KernelFn BM_TU_PICKER(int potential, int noise) {
+  switch (potential) {
+    case BM_POT_SINE2: return pick_noise_tu<BM_POT_SINE2>(noise);
+#if BM_TU_MODEL == 0 /* BM_OVERDAMPED: the other potentials exist for the over-damped model only */
+    case BM_POT_PWL: return pick_noise_tu<BM_POT_PWL>(noise);
+    case BM_POT_QUAD: return pick_noise_tu<BM_POT_QUAD>(noise);
+#endif
+    default: return nullptr;
+  }
+}
+
+}  // namespace bm

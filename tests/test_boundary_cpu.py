@@ -42,7 +42,7 @@ def test_struct_layouts_match_header(B):
 
 
 def test_version_and_status_strings(B):
-    assert B.bm_version() == 100
+    assert B.bm_version() == 101
     assert B.status_string(B.BM_OK) == "BM_OK" and B.status_string(B.BM_ERR_CUDA) == "BM_ERR_CUDA"
     assert B.status_string(99) == "BM_ERR_UNKNOWN"
 
@@ -66,7 +66,7 @@ def test_invalid_arguments_are_rejected_before_any_cuda_call(B):
     assert L.bm_simulate(C.byref(cfg), p.ctypes.data, 1, 32, 10, -1.0, 1, st.ctypes.data, None, None, None, 0, None) == B.BM_ERR_INVALID_ARG
     assert L.bm_simulate(C.byref(cfg), p.ctypes.data, 1, 32, 10, 1e-3, 1, st.ctypes.data, None, None, None, 0, None) == B.BM_ERR_WORKSPACE
     assert L.bm_philox_fill(1, 0, 0, 1, 0, 4, None, None) == B.BM_ERR_INVALID_ARG
-    assert L.bm_gauss_fill(B.BM_F64, 0, 1, 0, 4, 2, 4, p.ctypes.data, None) == B.BM_ERR_INVALID_ARG   # m0 % 4 != 0
+    assert L.bm_gauss_fill(B.BM_F64, 0, 1, 0, 4, 2, 4, p.ctypes.data, None) == B.BM_ERR_INVALID_ARG   # m0 % 8 != 0
 
 
 def test_no_cpu_fallback_without_a_device(B):

@@ -115,9 +115,15 @@ def test_n_discard_zero_and_sweep_with_disabled_points(B, orc):
     assert np.abs(paths[:, B.BM_OUT_XT] - ref[:, orc.OUT_XT]).max() < 1e-9
     assert np.array_equal(paths[:, B.BM_OUT_JUMPS], ref[:, orc.OUT_JUMPS])
     assert stats[0, 5] == 0 and stats[2, 5] == 0 and stats[1, 5] > 0
-    s32, p32, _ = B.run_workload(w, B.BM_F32, want_paths=True)
+    # fp32 with the oracle's word assignment (W32): a path follows the oracle's until its first kick (R13 gives
+    # the sub-step that ends at a kick its own normal), so the jump-free points agree path by path and the kicked
+    # point agrees for the paths without a kick; the kick counts are those of the same Poisson words
+    s32, p32, _ = B.run_workload(w, B.BM_F32, want_paths=True, gauss=B.BM_GAUSS_W32)
     assert s32[0, 5] == 0 and s32[2, 5] == 0 and s32[1, 5] > 0
-    assert np.abs(p32[:, B.BM_OUT_XT] - ref[:, orc.OUT_XT]).max() < 5e-3
+    quiet = ref[:, orc.OUT_JUMPS] == 0
+    assert quiet.sum() > 2 * w.n_paths
+    assert np.abs(p32[quiet, B.BM_OUT_XT] - ref[quiet, orc.OUT_XT]).max() < 5e-3
+    assert np.abs(p32[:, B.BM_OUT_JUMPS] - ref[:, orc.OUT_JUMPS]).max() <= 1
 
 
 def test_noise_source_off_ignores_parameters(B):
@@ -155,9 +161,10 @@ def test_kernel_info_and_probe(B):
     info = B.bm_kernel_info(B.config_for(w, B.BM_F32), w.n_points, w.n_paths)
     assert 16 <= info["regs_per_thread"] <= 255 and info["blocks_per_sm"] >= 1 and info["sm_count"] >= 1
     assert info["launch_threads"] in (128, 256)
-    off = B.bm_kernel_info(B.config_for(w, B.BM_F32, warp_spec=B.BM_WS_OFF), w.n_points, w.n_paths)
-    on = B.bm_kernel_info(B.config_for(w, B.BM_F32, warp_spec=B.BM_WS_ON), w.n_points, w.n_paths)
-    assert not off["warp_spec"] and on["warp_spec"] and on["launch_threads"] == 2 * off["launch_threads"]
+    assert info["gauss"] == B.BM_GAUSS_W16                     # AUTO resolves to the variant measured faster
+    w32 = B.bm_kernel_info(B.config_for(w, B.BM_F32, gauss=B.BM_GAUSS_W32), w.n_points, w.n_paths)
+    assert w32["gauss"] == B.BM_GAUSS_W32 and w32["launch_threads"] == info["launch_threads"]
+    assert B.bm_kernel_info(B.config_for(w, B.BM_F64), w.n_points, w.n_paths)["gauss"] == 0
     sink = torch.zeros(148 * 256, dtype=torch.float32, device="cuda")
     for op in range(B.BM_PROBE_COUNT):
         B.bm_pipe_probe(op, 4, 148, 256, sink)

@@ -86,11 +86,11 @@ def test_gauss_f64_matches_oracle(B, orc):
     assert np.abs(got - exp).max() < 5e-15 * (1 + np.abs(exp).max())
 
 
-def test_gauss_f32_tracks_oracle_and_has_unit_moments(B, orc):
+def test_gauss_f32_w32_tracks_oracle_and_has_unit_moments(B, orc):
     import torch
     n_paths, n_m = 64, 4096
     out = torch.zeros((n_paths, n_m), dtype=torch.float32, device="cuda")
-    B.bm_gauss_fill(B.BM_F32, B.BM_SINCOS_SFU, W.SEED, 0, n_paths, 0, n_m, out)
+    B.bm_gauss_fill(B.BM_F32, B.BM_GAUSS_W32, W.SEED, 0, n_paths, 0, n_m, out)
     got = out.cpu().numpy().astype(np.float64)
     exp = np.array([[orc.gauss(W.SEED, p, j) for j in range(256)] for p in range(n_paths)])
     d = np.abs(got[:, :256] - exp)
@@ -100,6 +100,41 @@ def test_gauss_f32_tracks_oracle_and_has_unit_moments(B, orc):
     assert abs(got.mean()) < 4 / math.sqrt(n)
     assert abs(got.var() - 1) < 4 * math.sqrt(2 / n)
     assert abs((got ** 4).mean() - 3) < 4 * math.sqrt(96 / n)
+
+
+def test_gauss_f32_w16_is_standard_normal(B, orc):
+    """W16 (R13): eight normals per Philox call, radius from the top 23 bits and angle from the low 16 bits of one
+    word.  Checked against what the mathematics fixes: moments up to order 6, independence of the two members of a
+    pair and of neighbouring normals, Kolmogorov distance to Phi; and against the oracle's Philox words directly
+    (the pair of word w is sqrt(-2 ln u) (cos, sin)(2 pi k/65536) with u, k read off w)."""
+    import torch
+    from scipy import stats as st
+    n_paths, n_m = 256, 8192
+    out = torch.zeros((n_paths, n_m), dtype=torch.float32, device="cuda")
+    B.bm_gauss_fill(B.BM_F32, B.BM_GAUSS_AUTO, W.SEED, 7, n_paths, 16, n_m, out)
+    got = out.cpu().numpy().astype(np.float64)
+    n = got.size
+    assert abs(got.mean()) < 4 / math.sqrt(n)
+    assert abs(got.var() - 1) < 4 * math.sqrt(2 / n)
+    assert abs((got ** 3).mean()) < 4 * math.sqrt(15 / n)
+    assert abs((got ** 4).mean() - 3) < 4 * math.sqrt(96 / n)
+    assert abs((got ** 6).mean() - 15) < 4 * math.sqrt((10395 - 225) / n)
+    a, b = got[:, 0::2].ravel(), got[:, 1::2].ravel()          # the two members of each pair
+    assert abs((a * b).mean()) < 4 / math.sqrt(a.size)
+    assert abs((a * a * b * b).mean() - 1) < 4 * math.sqrt(8 / a.size)
+    assert abs((got[:, 1:-1:2] * got[:, 2::2]).mean()) < 4 / math.sqrt(a.size)   # across pairs
+    assert st.kstest(got.ravel()[::7], "norm").statistic < 1.63 / math.sqrt(n / 7)  # 1 % critical value
+    # word by word: normals 8 b + 2 i, 8 b + 2 i + 1 of path g come from word i of Gaussian-stream call b
+    for p in (0, 100):
+        for b in (2, 500):
+            w = orc.philox_call(W.SEED, 7 + p, 1, b)
+            for i in range(4):
+                u = ((int(w[i]) >> 9) + 1) * 2.0 ** -23
+                ang = 2 * math.pi * (int(w[i]) & 0xFFFF) / 65536.0
+                r = math.sqrt(-2 * math.log(u))
+                j = 8 * (b - 2) + 2 * i
+                assert abs(got[p, j] - r * math.cos(ang)) < 2e-5 * (1 + r)
+                assert abs(got[p, j + 1] - r * math.sin(ang)) < 2e-5 * (1 + r)
 
 
 # ---- fp64 per-path parity, overdamped ---------------------------------------------------------------------
@@ -191,13 +226,23 @@ FP32_CASES = [
 ]
 
 
-@pytest.mark.parametrize("sincos", ["SFU", "FMA"])
+_ORACLE_CACHE = {}
+
+
+def cached_oracle_run(orc, name, w):
+    if name not in _ORACLE_CACHE:
+        _ORACLE_CACHE[name] = oracle_run(orc, w)[0]
+    return _ORACLE_CACHE[name]
+
+
+@pytest.mark.parametrize("sincos", ["SFU", "FMA", "SFU-W32"])
 @pytest.mark.parametrize("name,make,_", FP32_CASES, ids=[c[0] for c in FP32_CASES])
 def test_fp32_within_3_combined_se(B, orc, name, make, _, sincos):
     w = make()
-    sc = B.BM_SINCOS_SFU if sincos == "SFU" else B.BM_SINCOS_FMA
-    stats, paths, _ = B.run_workload(w, B.BM_F32, want_paths=True, sincos=sc)
-    ref, _ = oracle_run(orc, w)
+    sc = B.BM_SINCOS_FMA if sincos == "FMA" else B.BM_SINCOS_SFU
+    gs = B.BM_GAUSS_W32 if sincos.endswith("W32") else B.BM_GAUSS_AUTO
+    stats, paths, _ = B.run_workload(w, B.BM_F32, want_paths=True, sincos=sc, gauss=gs)
+    ref = cached_oracle_run(orc, name, w)
     for pt in range(w.n_points):
         sl = slice(pt * w.n_paths, (pt + 1) * w.n_paths)
         assert_3se(paths[sl], ref[sl], B.BM_OUT_VBAR, f"{name}/{sincos} point {pt} <v>")
@@ -212,7 +257,7 @@ def test_fp32_within_3_combined_se(B, orc, name, make, _, sincos):
 def test_fp32_paths_are_common_random_number_close(B, orc):
     """Same words for the same purpose: fp32 paths follow the fp64 oracle's path by path on a short horizon."""
     w = W.c0().scaled(n_paths=512, n_steps=400)
-    _, paths, _ = B.run_workload(w, B.BM_F32, want_paths=True)
+    _, paths, _ = B.run_workload(w, B.BM_F32, want_paths=True, gauss=B.BM_GAUSS_W32)
     ref, _ = oracle_run(orc, w)
     d = np.abs(paths[:, B.BM_OUT_XT] - ref[:, orc.OUT_XT])
     assert np.median(d) < 1e-4 and np.quantile(d, 0.99) < 1e-2
@@ -244,5 +289,8 @@ def test_quad_ou_fp64_matches_closed_form_and_oracle(B, orc):
     var_n = 2 * D * h * S * S * (1 - R ** (2 * n)) / (1 - R * R)
     assert abs(stats[0, 3] - x0 * R ** n) < 4 * math.sqrt(var_n / 4096)
     assert abs(stats[0, 4] - var_n) < 4 * var_n * math.sqrt(2 / 4095)
-    _, p32, _ = B.run_workload(w, B.BM_F32, want_paths=True)
+    _, p32, _ = B.run_workload(w, B.BM_F32, want_paths=True, gauss=B.BM_GAUSS_W32)
     assert np.abs(p32[:, B.BM_OUT_XT] - ref[:, orc.OUT_XT]).max() < 1e-4
+    _, p16, _ = B.run_workload(w, B.BM_F32, want_paths=True)          # W16: other normals, same law
+    assert abs(p16[:, B.BM_OUT_XT].mean() - x0 * R ** n) < 4 * math.sqrt(var_n / 4096)
+    assert abs(p16[:, B.BM_OUT_XT].var(ddof=1) - var_n) < 4 * var_n * math.sqrt(2 / 4095)
