@@ -47,7 +47,7 @@ def parse():
     ap.add_argument("--prec", default="f32", choices=["f32", "f64"])
     ap.add_argument("--sincos", default="auto", choices=["auto", "sfu", "fma"])
     ap.add_argument("--block-threads", type=int, default=0)
-    ap.add_argument("--gauss", default="auto", choices=["auto", "w32", "w16"],
+    ap.add_argument("--gauss", default="auto", choices=["auto", "w32", "w16", "w16p"],
                     help="fp32: Philox words per Box-Muller pair (bm_gauss)")
     ap.add_argument("--scale-steps", type=float, default=1.0, help="shrink n_steps (profiling runs only; flagged)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -259,7 +259,7 @@ def run_ours(args):
     sc = sincos_of(B, args.sincos)
     seed = w.seed + rank                                # replicas only: independent ensembles, no collective
     run = Runner(B, torch, w, prec, sc, args.block_threads, seed, dev, stream,
-                 {"auto": B.BM_GAUSS_AUTO, "w32": B.BM_GAUSS_W32, "w16": B.BM_GAUSS_W16}[args.gauss])
+                 {"auto": B.BM_GAUSS_AUTO, "w32": B.BM_GAUSS_W32, "w16": B.BM_GAUSS_W16, "w16p": B.BM_GAUSS_W16P}[args.gauss])
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
     info = B.bm_kernel_info(run.cfg, w.n_points, w.n_paths)
 
@@ -327,7 +327,7 @@ def run_ours(args):
                            "(max SM clock; lane count confirmed by bm_pipe_probe, DESIGN.md section 6)",
             "ops_per_path_step": xu_per_path / w.n_steps, "kernel": "bm_paths_f32" if prec == B.BM_F32 else "bm_paths_f64",
             "kernel_ms": ms_per_step, "regs_per_thread": info["regs_per_thread"],
-            "launch_threads": info["launch_threads"], "gauss": {1: "w32", 2: "w16"}.get(info["gauss"], "n/a"),
+            "launch_threads": info["launch_threads"], "gauss": {1: "w32", 2: "w16", 3: "w16p"}.get(info["gauss"], "n/a"),
             "blocks_per_sm": info["blocks_per_sm"]}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",

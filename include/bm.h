@@ -60,8 +60,11 @@ typedef enum { BM_SCHEME_JUMP_ADAPTED = 0, BM_SCHEME_PAPER_LITERAL = 1 } bm_sche
  * W32: one word per uniform (radius from w0, angle from w1, ...): four normals per call -- the oracle's assignment,
  *      so a jump-free fp32 path follows the fp64 oracle's path (common random numbers).
  * W16: radius from the top 23 bits and angle from the low 16 bits of ONE word: eight normals per call, half the
- *      integer work.  AUTO = W16 (the variant measured faster).  Ignored for BM_F64. */
-typedef enum { BM_GAUSS_AUTO = 0, BM_GAUSS_W32 = 1, BM_GAUSS_W16 = 2 } bm_gauss;
+ *      integer work; the angle's sine and cosine on the SFU (MUFU.SIN, MUFU.COS).
+ * W16P: the W16 assignment with the angle's sine and cosine evaluated by polynomials on the FMA pipe (two MUFU per
+ *      Box-Muller pair instead of four).  AUTO = W16 (the variant measured fastest).
+ * Ignored for BM_F64. */
+typedef enum { BM_GAUSS_AUTO = 0, BM_GAUSS_W32 = 1, BM_GAUSS_W16 = 2, BM_GAUSS_W16P = 3 } bm_gauss;
 /* noise sources that are switched on; a source that is off ignores its parameters */
 enum { BM_NOISE_GAUSS = 1, BM_NOISE_POISSON = 2, BM_NOISE_DICH = 4 };
 
@@ -95,8 +98,9 @@ typedef struct {
   int32_t potential;   /* bm_potential */
   int32_t scheme;      /* bm_scheme */
   int32_t noise;       /* OR of BM_NOISE_* */
-  int32_t block_threads; /* 0 = library default; else multiple of 32 in [32,256].  Part of the determinism contract
-                            (it fixes the reduction tree). */
+  int32_t block_threads; /* 0 = library default (a function of prec, n_points and n_paths only, see bm_kernel_info);
+                            else multiple of 32 in [32,256].  Part of the determinism contract (it fixes the
+                            reduction tree). */
   int32_t gauss;       /* bm_gauss (BM_F32 only) */
   int64_t n_discard;   /* grid steps before t_i, 0 <= n_discard < n_steps (PAPER.md:423 uses n_steps/10) */
   int64_t trace_steps; /* with out_trace: record the first trace_steps grid steps ... */

@@ -20,7 +20,7 @@ BM_SINCOS_AUTO, BM_SINCOS_SFU, BM_SINCOS_FMA = 0, 1, 2
 BM_POT_SINE2, BM_POT_PWL, BM_POT_QUAD = 0, 1, 2
 BM_SCHEME_JUMP_ADAPTED, BM_SCHEME_PAPER_LITERAL = 0, 1
 BM_NOISE_GAUSS, BM_NOISE_POISSON, BM_NOISE_DICH = 1, 2, 4
-BM_GAUSS_AUTO, BM_GAUSS_W32, BM_GAUSS_W16 = 0, 1, 2
+BM_GAUSS_AUTO, BM_GAUSS_W32, BM_GAUSS_W16, BM_GAUSS_W16P = 0, 1, 2, 3
 BM_OUT_XT, BM_OUT_VT, BM_OUT_VBAR, BM_OUT_JUMPS, BM_OUT_SUBSTEPS, BM_OUT_XTI, BM_OUT_STRIDE = 0, 1, 2, 3, 4, 5, 6
 (BM_PROBE_FFMA, BM_PROBE_MUFU_COS, BM_PROBE_MUFU_LG2, BM_PROBE_MUFU_SQRT, BM_PROBE_IMAD_WIDE, BM_PROBE_LOP3,
  BM_PROBE_DFMA, BM_PROBE_I2F, BM_PROBE_FADD, BM_PROBE_MIX, BM_PROBE_COUNT) = range(11)

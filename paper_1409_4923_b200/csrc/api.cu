@@ -32,14 +32,20 @@ bool valid_cfg(const bm_config *c) {
   if (c->scheme != BM_SCHEME_JUMP_ADAPTED && c->scheme != BM_SCHEME_PAPER_LITERAL) return false;
   if (c->noise < 0 || c->noise > 7) return false;
   if (c->block_threads != 0 && (c->block_threads < 32 || c->block_threads > 256 || (c->block_threads & 31))) return false;
-  if (c->gauss < BM_GAUSS_AUTO || c->gauss > BM_GAUSS_W16) return false;
+  if (c->gauss < BM_GAUSS_AUTO || c->gauss > BM_GAUSS_W16P) return false;
   if (c->n_discard < 0 || c->trace_steps < 0 || c->trace_paths < 0) return false;
   return true;
 }
 
-int block_threads_of(const bm_config *c) {
+// Default block size: a function of the problem size only (never of the device), because the block size fixes the
+// reduction tree.  fp32: 256 threads when the whole job is at most LOW_OCCUPANCY_WARPS warps (8 per SM sub-partition
+// of a 148-SM part) -- measured 4 % faster than 128 on C1/C2, 2.5 % slower on C4.
+constexpr long long LOW_OCCUPANCY_WARPS = 8LL * 4 * 148;
+int block_threads_of(const bm_config *c, int32_t n_points, int64_t n_paths) {
   if (c->block_threads) return c->block_threads;
-  return c->prec == BM_F64 ? DEFAULT_BLOCK_F64 : DEFAULT_BLOCK_F32;
+  if (c->prec == BM_F64) return DEFAULT_BLOCK_F64;
+  const long long warps = (long long)n_points * ((n_paths + 31) / 32);
+  return (n_paths >= 256 && warps <= LOW_OCCUPANCY_WARPS) ? 256 : DEFAULT_BLOCK_F32;
 }
 
 int resolve_sincos(const bm_config *c) {
@@ -48,8 +54,9 @@ int resolve_sincos(const bm_config *c) {
 }
 
 int resolve_gauss(const bm_config *c) {
-  // AUTO: eight normals per Philox call measured faster on B200 for every config
-  return c->gauss == BM_GAUSS_W32 ? BM_GAUSS_W32 : BM_GAUSS_W16;
+  // AUTO: eight normals per Philox call with the Box-Muller angle on the SFU: W16 and W16P measure within 1 % of
+  // each other on the over-damped configs, W16 is 3-4 % faster on the inertial ones
+  return c->gauss == BM_GAUSS_AUTO ? BM_GAUSS_W16 : c->gauss;
 }
 
 struct Launch {
@@ -58,31 +65,30 @@ struct Launch {
   int gauss = 0;    // bm_gauss selected (fp32), 0 for fp64
 };
 
-bm_status pick_kernel(const bm_config *c, Launch *L) {
+bm_status pick_kernel(const bm_config *c, int32_t n_points, int64_t n_paths, Launch *L) {
   *L = Launch();
   if (c->scheme == BM_SCHEME_PAPER_LITERAL) return BM_ERR_UNSUPPORTED;  // NEXT row f1, not built yet
   if (c->model == BM_INERTIAL && c->potential != BM_POT_SINE2) return BM_ERR_UNSUPPORTED;
-  L->threads = block_threads_of(c);
+  L->threads = block_threads_of(c, n_points, n_paths);
   if (c->prec == BM_F64) {
     L->fn = c->model == BM_OVERDAMPED ? pick_f64_overdamped(c->potential, c->noise)
                                       : pick_f64_inertial(c->potential, c->noise);
   } else {
-    const bool sfu = resolve_sincos(c) == BM_SINCOS_SFU;
-    const bool w16 = resolve_gauss(c) == BM_GAUSS_W16;
-    L->gauss = w16 ? BM_GAUSS_W16 : BM_GAUSS_W32;
-    if (c->model == BM_OVERDAMPED)
-      L->fn = sfu ? (w16 ? pick_f32_od_sfu_w16 : pick_f32_od_sfu_w32)(c->potential, c->noise)
-                  : (w16 ? pick_f32_od_fma_w16 : pick_f32_od_fma_w32)(c->potential, c->noise);
-    else
-      L->fn = sfu ? (w16 ? pick_f32_in_sfu_w16 : pick_f32_in_sfu_w32)(c->potential, c->noise)
-                  : (w16 ? pick_f32_in_fma_w16 : pick_f32_in_fma_w32)(c->potential, c->noise);
+    typedef KernelFn (*Picker)(int, int);
+    static const Picker table[2][2][3] = {  // [model][sincos fma][gauss - 1]
+        {{pick_f32_od_sfu_w32, pick_f32_od_sfu_w16, pick_f32_od_sfu_w16p},
+         {pick_f32_od_fma_w32, pick_f32_od_fma_w16, pick_f32_od_fma_w16p}},
+        {{pick_f32_in_sfu_w32, pick_f32_in_sfu_w16, pick_f32_in_sfu_w16p},
+         {pick_f32_in_fma_w32, pick_f32_in_fma_w16, pick_f32_in_fma_w16p}}};
+    L->gauss = resolve_gauss(c);
+    L->fn = table[c->model == BM_INERTIAL][resolve_sincos(c) == BM_SINCOS_FMA][L->gauss - 1](c->potential, c->noise);
   }
   if (!L->fn) return BM_ERR_UNSUPPORTED;
   return BM_OK;
 }
 
-long long blocks_per_point_of(const bm_config *c, int64_t n_paths) {
-  const int bt = block_threads_of(c);
+long long blocks_per_point_of(const bm_config *c, int32_t n_points, int64_t n_paths) {
+  const int bt = block_threads_of(c, n_points, n_paths);
   return (n_paths + bt - 1) / bt;
 }
 
@@ -105,7 +111,7 @@ BM_API const char *bm_status_string(bm_status s) {
 
 BM_API size_t bm_workspace_bytes(const bm_config *cfg, int32_t n_points, int64_t n_paths) {
   if (!valid_cfg(cfg) || n_points <= 0 || n_paths <= 0) return 0;
-  const long long bpp = blocks_per_point_of(cfg, n_paths);
+  const long long bpp = blocks_per_point_of(cfg, n_points, n_paths);
   const long long grid = bpp * (long long)n_points;
   if (grid > 0x7FFFFFFFLL) return 0;
   return (size_t)grid * PARTIAL_STRIDE * sizeof(double);
@@ -121,7 +127,7 @@ BM_API bm_status bm_simulate(const bm_config *cfg, const bm_params *params, int3
   if (out_trace && (cfg->trace_steps <= 0 || cfg->trace_paths <= 0)) return BM_ERR_INVALID_ARG;
   if (out_trace && cfg->prec != BM_F64) return BM_ERR_UNSUPPORTED;
   Launch L;
-  const bm_status ps = pick_kernel(cfg, &L);
+  const bm_status ps = pick_kernel(cfg, n_points, n_paths, &L);
   if (ps != BM_OK) return ps;
   const size_t need = bm_workspace_bytes(cfg, n_points, n_paths);
   if (need == 0) return BM_ERR_INVALID_ARG;
@@ -140,7 +146,7 @@ BM_API bm_status bm_simulate(const bm_config *cfg, const bm_params *params, int3
   a.trace_paths = out_trace ? cfg->trace_paths : 0;
   a.dt = dt;
   a.n_points = n_points;
-  a.blocks_per_point = (int)blocks_per_point_of(cfg, n_paths);
+  a.blocks_per_point = (int)blocks_per_point_of(cfg, n_points, n_paths);
   a.keys = make_keys(seed);
 
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
@@ -194,7 +200,7 @@ BM_API bm_status bm_philox_fill(uint64_t seed, uint64_t path0, int32_t n_paths, 
 BM_API bm_status bm_gauss_fill(int32_t prec, int32_t gauss, uint64_t seed, uint64_t path0, int32_t n_paths, uint64_t m0,
                         int32_t n_m, void *out, void *stream) {
   if (!out || n_paths <= 0 || n_m <= 0 || (m0 & 7)) return BM_ERR_INVALID_ARG;
-  if (gauss < BM_GAUSS_AUTO || gauss > BM_GAUSS_W16) return BM_ERR_INVALID_ARG;
+  if (gauss < BM_GAUSS_AUTO || gauss > BM_GAUSS_W16P) return BM_ERR_INVALID_ARG;
   if (prec != BM_F32 && prec != BM_F64) return BM_ERR_INVALID_ARG;
   const PhiloxKeys K = make_keys(seed);
   return launch_gauss_fill(prec, gauss, K, path0, n_paths, m0, n_m, out, reinterpret_cast<cudaStream_t>(stream)) ==
@@ -205,7 +211,7 @@ BM_API bm_status bm_kernel_info(const bm_config *cfg, int32_t n_points, int64_t 
                          int32_t *launch_threads, int32_t *blocks_per_sm, int32_t *sm_count, int32_t *gauss) {
   if (!valid_cfg(cfg) || n_points <= 0 || n_paths <= 0) return BM_ERR_INVALID_ARG;
   Launch L;
-  const bm_status ps = pick_kernel(cfg, &L);
+  const bm_status ps = pick_kernel(cfg, n_points, n_paths, &L);
   if (ps != BM_OK) return ps;
   cudaFuncAttributes attr;
   if (cudaFuncGetAttributes(&attr, (const void *)L.fn) != cudaSuccess) { cudaGetLastError(); return BM_ERR_CUDA; }

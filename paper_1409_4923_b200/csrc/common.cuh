@@ -57,6 +57,20 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
   return make_uint4(c0, c1, c2, c3);
 }
 
+// Rounds R0 .. R1-1 of the same function on a counter held in c (the path kernel spreads the ten rounds of the next
+// Gaussian call over a block of grid cells).
+template <int R0, int R1>
+__device__ __forceinline__ void philox_rounds(uint4 &c, const PhiloxKeys &K) {
+#pragma unroll
+  for (int r = R0; r < R1; ++r) {
+    const unsigned long long p0 = (unsigned long long)PHILOX_M0 * c.x;
+    const unsigned long long p1 = (unsigned long long)PHILOX_M1 * c.z;
+    const uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+    const uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+    c = make_uint4(hi1 ^ c.y ^ K.k0[r], lo1, hi0 ^ c.w ^ K.k1[r], lo0);
+  }
+}
+
 __device__ __forceinline__ uint4 philox_call(const PhiloxKeys &K, unsigned long long g, uint32_t stream,
                                              uint32_t idx) {
   return philox4x32_10(idx, stream, (uint32_t)g, (uint32_t)(g >> 32), K);

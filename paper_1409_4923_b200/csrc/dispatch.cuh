@@ -17,6 +17,10 @@ KernelFn pick_f32_in_sfu_w16(int potential, int noise);
 KernelFn pick_f32_in_sfu_w32(int potential, int noise);
 KernelFn pick_f32_in_fma_w16(int potential, int noise);
 KernelFn pick_f32_in_fma_w32(int potential, int noise);
+KernelFn pick_f32_od_sfu_w16p(int potential, int noise);
+KernelFn pick_f32_od_fma_w16p(int potential, int noise);
+KernelFn pick_f32_in_sfu_w16p(int potential, int noise);
+KernelFn pick_f32_in_fma_w16p(int potential, int noise);
 
 // fills (fill.cu)
 cudaError_t launch_philox_fill(const PhiloxKeys &K, unsigned long long path0, int n_paths, uint32_t stream_id,

@@ -28,7 +28,7 @@ cudaError_t launch_philox_fill(const PhiloxKeys &K, unsigned long long path0, in
 template <int PREC, int GW>
 __global__ void gauss_fill_kernel(const __grid_constant__ PhiloxKeys K, unsigned long long path0, int n_paths,
                                   unsigned long long m0, int n_blocks, int n_m, void *out) {
-  constexpr int NB = (PREC == BM_F32 && GW == BM_GAUSS_W16) ? 8 : 4;
+  constexpr int NB = (PREC == BM_F32 && GW != BM_GAUSS_W32) ? 8 : 4;
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= (long long)n_paths * n_blocks) return;
   const int p = (int)(i / n_blocks), b = (int)(i - (long long)p * n_blocks);
@@ -62,7 +62,9 @@ cudaError_t launch_gauss_fill(int prec, int gauss, const PhiloxKeys &K, unsigned
     gauss_fill_kernel<BM_F64, BM_GAUSS_W32><<<blocks, threads, 0, st>>>(K, path0, n_paths, m0, n_blocks, n_m, out);
   else if (gauss == BM_GAUSS_W32)
     gauss_fill_kernel<BM_F32, BM_GAUSS_W32><<<blocks, threads, 0, st>>>(K, path0, n_paths, m0, n_blocks, n_m, out);
-  else
+  else if (gauss == BM_GAUSS_W16P)
+    gauss_fill_kernel<BM_F32, BM_GAUSS_W16P><<<blocks, threads, 0, st>>>(K, path0, n_paths, m0, n_blocks, n_m, out);
+  else  // W16, and AUTO (which resolves to it)
     gauss_fill_kernel<BM_F32, BM_GAUSS_W16><<<blocks, threads, 0, st>>>(K, path0, n_paths, m0, n_blocks, n_m, out);
   return cudaGetLastError();
 }

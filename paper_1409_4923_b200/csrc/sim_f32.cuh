@@ -157,9 +157,9 @@ __device__ __forceinline__ void schedule_f32(int n, float tau, float dt, float i
   float f = (q - c) * dt;
   if (f >= dt) { f = 0.0f; c += 1.0f; }
   if (c == 0.0f) f = fmaxf(f, tau);  // never schedule into the past of this cell
-  c = fminf(c, 2.0e9f);
-  const long long t = (long long)n + (long long)c;
-  cell = t > 0x7FFFFFFFLL ? 0x7FFFFFFF : (int)t;
+  c = fminf(c, 2.0e9f);  // < 2^31: the 32-bit conversion is exact, and n + c < 2^32 cannot wrap as unsigned
+  const unsigned t = (unsigned)n + (unsigned)__float2int_rz(c);
+  cell = (int)min(t, 0x7FFFFFFFu);
   off = f;
 }
 
@@ -189,34 +189,50 @@ __device__ __forceinline__ Pair pair_w16(uint32_t w, float cn) {
   return p;
 }
 
-// normals of NB = 4 (W32) or 8 (W16) consecutive grid cells: Gaussian-stream call b
-template <int GW> struct GaussBlock { Pair p[GW == BM_GAUSS_W16 ? 4 : 2]; };
+// W16P: the W16 assignment with the angle's sine and cosine on the FMA pipe: r = k/65536 - 1/2 turns (exact),
+// cos 2 pi r and sin 2 pi r / r as degree-5 polynomials in r^2 (Chebyshev-node fits on |r| <= 1/2; absolute error
+// with fp32 Horner evaluation 1.3e-6 and 6e-7: the class of MUFU.COS / MUFU.SIN).  Two MUFU per pair instead of four.
+__device__ __forceinline__ Pair pair_w16p(uint32_t w, float cn) {
+  Pair p;
+  p.r = sqrt_approx(cn * lg2_approx(u01_open0_f32(w)));
+  const float t = __uint_as_float((w & 0xFFFFu) | 0x3F800000u);
+  const float r = fmaf(t, 128.0f, -128.5f);
+  const float s = r * r;
+  // coefficients negated: the angle is 2 pi k / 65536 = 2 pi r + pi (the same angle as W16)
+  float c = 2.107110563e+01f, q = 1.247124353e+01f;
+  c = fmaf(c, s, -5.879049212e+01f); q = fmaf(q, s, -4.134288235e+01f);
+  c = fmaf(c, s, 8.527162153e+01f);  q = fmaf(q, s, 7.661447253e+01f);
+  c = fmaf(c, s, -6.492865742e+01f); q = fmaf(q, s, -8.159994333e+01f);
+  c = fmaf(c, s, 1.973898036e+01f);  q = fmaf(q, s, 4.134158923e+01f);
+  c = fmaf(c, s, -9.999992108e-01f); q = fmaf(q, s, -6.283184916e+00f);
+  p.c = c;
+  p.s = q * r;
+  return p;
+}
 
+// Gaussian-stream call b serves NB = 4 (W32) or 8 (W16, W16P) consecutive grid cells = NB/2 Box-Muller pairs
+template <int GW> struct GaussLayout {
+  static constexpr int NB = GW == BM_GAUSS_W32 ? 4 : 8;
+  static constexpr int NP = NB / 2;
+};
+
+// pair I of the call whose words are w (I is a compile-time constant at every use)
 template <int GW>
-__device__ __forceinline__ GaussBlock<GW> draw_block_f32(const PhiloxKeys &K, unsigned long long g, uint32_t b, float cn) {
-  GaussBlock<GW> q;
-  const uint4 w = philox_call(K, g, STREAM_GAUSS, b);
-  if (GW == BM_GAUSS_W16) {
-    q.p[0] = pair_w16(w.x, cn);
-    q.p[1] = pair_w16(w.y, cn);
-    q.p[2] = pair_w16(w.z, cn);
-    q.p[3] = pair_w16(w.w, cn);
-  } else {
-    q.p[0] = pair_w32(w.x, w.y, cn);
-    q.p[1] = pair_w32(w.z, w.w, cn);
-  }
-  return q;
+__device__ __forceinline__ Pair pair_of(const uint4 &w, int I, float cn) {
+  if (GW == BM_GAUSS_W32) return I == 0 ? pair_w32(w.x, w.y, cn) : pair_w32(w.z, w.w, cn);
+  const uint32_t ww = I == 0 ? w.x : I == 1 ? w.y : I == 2 ? w.z : w.w;
+  return GW == BM_GAUSS_W16P ? pair_w16p(ww, cn) : pair_w16(ww, cn);
 }
 
 // Standard normals of call b in cell order (bm_gauss_fill)
 template <int GW>
 __device__ __forceinline__ void gauss_block_standard_f32(const PhiloxKeys &K, unsigned long long g, uint32_t b, float *out) {
-  const GaussBlock<GW> q = draw_block_f32<GW>(K, g, b, -2.0f * LN2_F);
-  constexpr int NP = GW == BM_GAUSS_W16 ? 4 : 2;
+  const uint4 w = philox_call(K, g, STREAM_GAUSS, b);
 #pragma unroll
-  for (int i = 0; i < NP; ++i) {
-    out[2 * i] = q.p[i].r * q.p[i].c;
-    out[2 * i + 1] = q.p[i].r * q.p[i].s;
+  for (int i = 0; i < GaussLayout<GW>::NP; ++i) {
+    const Pair q = pair_of<GW>(w, i, -2.0f * LN2_F);
+    out[2 * i] = q.r * q.c;
+    out[2 * i + 1] = q.r * q.s;
   }
 }
 
@@ -238,7 +254,7 @@ template <int MODEL, int POT, int NOISE, int SINCOS, int GW>
 __global__ void __launch_bounds__(256) bm_paths_f32(const __grid_constant__ SimArgs a) {
   constexpr bool HAS_G = NOISE & BM_NOISE_GAUSS, HAS_P = NOISE & BM_NOISE_POISSON, HAS_D = NOISE & BM_NOISE_DICH;
   constexpr bool INERTIAL = MODEL == BM_INERTIAL;
-  constexpr int NB = GW == BM_GAUSS_W16 ? 8 : 4;  // grid cells per Gaussian call
+  constexpr int NB = GaussLayout<GW>::NB, NP = GaussLayout<GW>::NP;  // grid cells, pairs per Gaussian call
   constexpr float S = Units<POT>::SCALE;
   constexpr unsigned FULL = 0xffffffffu;
   constexpr int NEVER = 0x7FFFFFFF;
@@ -305,13 +321,16 @@ __global__ void __launch_bounds__(256) bm_paths_f32(const __grid_constant__ SimA
   int nP = NEVER, nD = NEVER;
   float fP = 0.f, fD = 0.f, z = 0.f;
   uint32_t kP = 0, kD = 0;
+  uint32_t gwP = 0, gwD = 0;  // Gaussian word of the sub-step that ends at the next kick / flip (R13)
   if (HAS_P && lam > 0.0) {
     const uint4 w = philox_call(K, g, STREAM_POISSON, 0);
+    gwP = w.z;
     schedule_f32(0, 0.f, dt, inv_dt, neg_log_u_f32(w.x) * P.inv_lam_dt, nP, fP);
     z = P.zeta * neg_log_u_f32(w.y);
   }
   if (HAS_D) {
     const uint4 w = philox_call(K, g, STREAM_DICH, 0);
+    gwD = w.z;
     schedule_f32(0, 0.f, dt, inv_dt, neg_log_u_f32(w.x) * (d ? P.inv_mub_dt : P.inv_mua_dt), nD, fD);
   }
 
@@ -336,7 +355,7 @@ __global__ void __launch_bounds__(256) bm_paths_f32(const __grid_constant__ SimA
   float k0f = dt * cst, k0h = hh_full * cst;
 
   // ---- FAST: a full grid step without events in this lane (h = dt) --------------------------------------------
-  auto fast_cell = [&](float gr, float gc, bool do_fold) {
+  auto fast_cell = [&](float gr, float gc, bool do_fold) {  // noise = gr * gc
     float xf = x;
     if (do_fold || POT != BM_POT_SINE2) fold_f32<POT>(xf, wraps);
     if (!INERTIAL) {
@@ -364,7 +383,7 @@ __global__ void __launch_bounds__(256) bm_paths_f32(const __grid_constant__ SimA
   };
 
   // ---- SLOW: a cell in which at least one lane of the warp has a kick or a flip --------------------------------
-  auto slow_cell = [&](int n, float gr, float gc) {
+  auto slow_cell = [&](int n, float gnoise) {
     float tau = 0.f;         // the lane's offset inside cell n
     float dr_tau = drive0;   // drive at that time
     const float phf = INERTIAL ? __uint_as_float((uint32_t)(ph >> 41) | 0x3F800000u) : 0.f;  // 1 + frac(omega n dt / 2 pi)
@@ -374,12 +393,16 @@ __global__ void __launch_bounds__(256) bm_paths_f32(const __grid_constant__ SimA
       const bool isP = inP && (!inD || fP <= fD);  // a tie applies the kick first (R5)
       const float te = isP ? fP : fD;
       const float h = fmaxf(te - tau, 0.f);
-      // the event's own Philox call: .x next waiting time, .y next amplitude, .z Gaussian of this sub-step (R13)
+      // Philox call k+1 of the event's stream: .x waiting time to event k+1, .y amplitude of kick k+1, .z Gaussian
+      // of the sub-step that will end at event k+1 (R13).  The sub-step that ends now uses the word drawn one event
+      // earlier, so the Philox rounds and the predictor-corrector chain are independent instruction streams.
       const uint4 w = philox_call(K, g, isP ? STREAM_POISSON : STREAM_DICH, (isP ? kP : kD) + 1u);
+      const uint32_t gw = isP ? gwP : gwD;
+      if (isP) gwP = w.z; else gwD = w.z;
       float noise = 0.f;
       if (HAS_G) {
-        const float r = sqrt_approx(P.cn * lg2_approx(u01_open0_f32(w.z)) * (h * inv_dt));  // Var ~ h (A9)
-        const float t = __uint_as_float((w.z & 0xFFFFu) | 0x3F800000u);
+        const float r = sqrt_approx(P.cn * lg2_approx(u01_open0_f32(gw)) * (h * inv_dt));  // Var ~ h (A9)
+        const float t = __uint_as_float((gw & 0xFFFFu) | 0x3F800000u);
         noise = r * cos_approx(fmaf(t, 128.0f * TWO_PI_F, -128.0f * TWO_PI_F));
       }
       float dr1 = 0.f;
@@ -406,7 +429,7 @@ __global__ void __launch_bounds__(256) bm_paths_f32(const __grid_constant__ SimA
     // every lane: the rest of the cell (the whole cell for a lane without events)
     const float h = dt - tau;
     float noise = 0.f;
-    if (HAS_G) noise = gr * gc * ((tau == 0.f) ? 1.0f : sqrt_approx(h * inv_dt));
+    if (HAS_G) noise = gnoise * ((tau == 0.f) ? 1.0f : sqrt_approx(h * inv_dt));
     float drive1 = 0.f;
     if (INERTIAL) {
       ph += dph;
@@ -416,45 +439,133 @@ __global__ void __launch_bounds__(256) bm_paths_f32(const __grid_constant__ SimA
     drive0 = drive1;
   };
 
+  // Events of this lane in cells [n, n+32) as a bit mask (bit = cell - n; shl.b32 clamps a shift >= 32 to zero, so
+  // NEVER and any far cell give 0).
+  auto ev_bits = [&](int n) -> unsigned {
+    unsigned bits = 0, t;
+    if (HAS_P) { asm("shl.b32 %0, 1, %1;" : "=r"(t) : "r"((unsigned)(nP - n))); bits |= t; }
+    if (HAS_D) { asm("shl.b32 %0, 1, %1;" : "=r"(t) : "r"((unsigned)(nD - n))); bits |= t; }
+    return bits;
+  };
+
   // ---- time loop: blocks of NB cells = one Gaussian call -------------------------------------------------------
-  GaussBlock<GW> qn;
-#pragma unroll
-  for (int i = 0; i < NB / 2; ++i) qn.p[i] = Pair{0.f, 0.f, 0.f};
-  if (HAS_G) qn = draw_block_f32<GW>(K, g, 0, P.cn);
+  // A block is CLEAN when no lane of the warp has an event in it and it holds neither t_i nor the end of the run:
+  // NB fast cells, one vote.  Otherwise the warp builds a uniform control word (bit j: some lane has an event in
+  // cell n+j; bit 8+j: cell n+j is the snapshot cell or lies beyond the end) and tests one bit pair per cell.
+  // The Box-Muller pair of cells (2i+2, 2i+3) is formed while cells (2i, 2i+1) run (its consumer is near, so the
+  // instruction scheduler fills the stalls of the serial predictor-corrector chain with it), and the Philox call of
+  // the next block is issued at the top of the block.
+  constexpr bool ROLLED = INERTIAL;  // non-clean blocks: one rolled copy of the cell code (measured, DESIGN.md s.6)
+  __shared__ float s_noise[ROLLED ? NB : 1][ROLLED ? 256 : 1];
+  uint4 w = make_uint4(0u, 0u, 0u, 0u);
+  Pair cur = Pair{0.f, 0.f, 0.f};
+  if (HAS_G) {
+    w = philox_call(K, g, STREAM_GAUSS, 0);
+    cur = pair_of<GW>(w, 0, P.cn);
+  }
+  // rounds of the next Gaussian call done in pair slot i: NP = 4: 4 + 3 + 3 + 0, NP = 2: 10 + 0
+  auto next_rounds = [&](uint4 &c, int i) {
+    if (NP == 4) {
+      if (i == 0) philox_rounds<0, 4>(c, K);
+      if (i == 1) philox_rounds<4, 7>(c, K);
+      if (i == 2) philox_rounds<7, 10>(c, K);
+    } else if (i == 0) {
+      philox_rounds<0, 10>(c, K);
+    }
+  };
   uint32_t blk = 0;
   for (int n = 0; n < n_steps; n += NB) {
-    const GaussBlock<GW> q = qn;
     blk++;
-    const int nEv = min(nP, nD);
-    const bool boundary = (n + NB > n_steps) || (n < n_discard && n_discard < n + NB);
-    const bool clean = !boundary && !__any_sync(FULL, nEv < n + NB);
-    if (n == n_discard) {  // a10: t_i on a block boundary
-      fold_f32<POT>(x, wraps);
-      snap_x = x;
-      snap_w = wraps;
-    }
+    const bool special = ((unsigned)(n_discard - n) < (unsigned)NB) || (n + NB > n_steps);
+    const bool clean = !special && !((HAS_P || HAS_D) && __any_sync(FULL, min(nP, nD) < n + NB));
+    // counter of the next Gaussian call; its ten rounds are spread over the pair slots of this block
+    uint4 wn = make_uint4(blk, (uint32_t)STREAM_GAUSS, (uint32_t)g, (uint32_t)(g >> 32));
     if (clean) {
-      if (HAS_G) qn = draw_block_f32<GW>(K, g, blk, P.cn);
 #pragma unroll
-      for (int j = 0; j < NB; ++j) fast_cell(q.p[j >> 1].r, (j & 1) ? q.p[j >> 1].s : q.p[j >> 1].c, j == 0);
+      for (int i = 0; i < NP; ++i) {
+        Pair nxt = cur;
+        if (HAS_G) {
+          next_rounds(wn, i);
+          nxt = (i + 1 < NP) ? pair_of<GW>(w, i + 1, P.cn) : pair_of<GW>(wn, 0, P.cn);
+        }
+        fast_cell(cur.r, cur.c, i == 0);
+        fast_cell(cur.r, cur.s, false);
+        cur = nxt;
+      }
     } else {
-      if (HAS_G) qn = draw_block_f32<GW>(K, g, blk, P.cn);
+      unsigned ctl = 0;
+      if (HAS_P || HAS_D) ctl = __reduce_or_sync(FULL, ev_bits(n)) & 0xFFu;
+      if (special) {
+        if ((unsigned)(n_discard - n) < (unsigned)NB) ctl |= 0x100u << (n_discard - n);
+        if (n + NB > n_steps) ctl |= (0xFF00u << (n_steps - n)) & 0xFF00u;
+      }
+      fold_f32<POT>(x, wraps);
+      if (!ROLLED) {
 #pragma unroll
-      for (int j = 0; j < NB; ++j) {
-        const int nc = n + j;
-        if (nc < n_steps) {
-          if (j > 0 && nc == n_discard) {  // a10: t_i inside a block
-            fold_f32<POT>(x, wraps);
+        for (int i = 0; i < NP; ++i) {
+          Pair nxt = cur;
+          if (HAS_G) {
+            next_rounds(wn, i);
+            nxt = (i + 1 < NP) ? pair_of<GW>(w, i + 1, P.cn) : pair_of<GW>(wn, 0, P.cn);
+          }
+#pragma unroll
+          for (int jj = 0; jj < 2; ++jj) {
+            const int j = 2 * i + jj;
+            const unsigned m = ctl >> j;
+            bool run = true;
+            if (m & 0x100u) {
+              if (n + j >= n_steps) {
+                run = false;
+              } else {  // a10: t_i
+                fold_f32<POT>(x, wraps);
+                snap_x = x;
+                snap_w = wraps;
+              }
+            }
+            if (run) {
+              const float gc = jj ? cur.s : cur.c;
+              if ((HAS_P || HAS_D) && (m & 1u)) {
+                slow_cell(n + j, cur.r * gc);
+                ctl |= __reduce_or_sync(FULL, ev_bits(n)) & 0xFFu;  // events re-scheduled into this block
+              } else {
+                fast_cell(cur.r, gc, false);
+              }
+            }
+          }
+          cur = nxt;
+        }
+      } else {
+        // the block's NB noise values go through shared memory (each thread reads back only what it wrote: no
+        // barrier), so the cell loop stays rolled
+        if (HAS_G) {
+          philox_rounds<0, 10>(wn, K);
+#pragma unroll
+          for (int i = 0; i < NP; ++i) {
+            s_noise[2 * i][threadIdx.x] = cur.r * cur.c;
+            s_noise[2 * i + 1][threadIdx.x] = cur.r * cur.s;
+            cur = (i + 1 < NP) ? pair_of<GW>(w, i + 1, P.cn) : pair_of<GW>(wn, 0, P.cn);
+          }
+        }
+#pragma unroll 1
+        for (int j = 0; j < NB; ++j) {
+          const unsigned m = ctl >> j;
+          if (m & 0x100u) {
+            if (n + j >= n_steps) break;
+            fold_f32<POT>(x, wraps);  // a10: t_i
             snap_x = x;
             snap_w = wraps;
           }
-          const float gr = q.p[j >> 1].r, gc = (j & 1) ? q.p[j >> 1].s : q.p[j >> 1].c;
-          const bool ev = (HAS_P && nP == nc) || (HAS_D && nD == nc);
-          if ((HAS_P || HAS_D) && __any_sync(FULL, ev)) slow_cell(nc, gr, gc);
-          else fast_cell(gr, gc, true);
+          const float gnoise = HAS_G ? s_noise[j][threadIdx.x] : 0.f;
+          if ((HAS_P || HAS_D) && (m & 1u)) {
+            slow_cell(n + j, gnoise);
+            ctl |= __reduce_or_sync(FULL, ev_bits(n)) & 0xFFu;  // events re-scheduled into this block
+          } else {
+            fast_cell(gnoise, 1.0f, false);
+          }
         }
       }
     }
+    w = wn;
   }
 
   Partial mine = partial_zero();

@@ -102,8 +102,9 @@ def test_gauss_f32_w32_tracks_oracle_and_has_unit_moments(B, orc):
     assert abs((got ** 4).mean() - 3) < 4 * math.sqrt(96 / n)
 
 
-def test_gauss_f32_w16_is_standard_normal(B, orc):
-    """W16 (R13): eight normals per Philox call, radius from the top 23 bits and angle from the low 16 bits of one
+@pytest.mark.parametrize("gauss", ["W16", "W16P"])
+def test_gauss_f32_w16_is_standard_normal(B, orc, gauss):
+    """W16 / W16P (R13): eight normals per Philox call, radius from the top 23 bits and angle from the low 16 bits of one
     word.  Checked against what the mathematics fixes: moments up to order 6, independence of the two members of a
     pair and of neighbouring normals, Kolmogorov distance to Phi; and against the oracle's Philox words directly
     (the pair of word w is sqrt(-2 ln u) (cos, sin)(2 pi k/65536) with u, k read off w)."""
@@ -111,7 +112,7 @@ def test_gauss_f32_w16_is_standard_normal(B, orc):
     from scipy import stats as st
     n_paths, n_m = 256, 8192
     out = torch.zeros((n_paths, n_m), dtype=torch.float32, device="cuda")
-    B.bm_gauss_fill(B.BM_F32, B.BM_GAUSS_AUTO, W.SEED, 7, n_paths, 16, n_m, out)
+    B.bm_gauss_fill(B.BM_F32, B.BM_GAUSS_W16P if gauss == "W16P" else B.BM_GAUSS_AUTO, W.SEED, 7, n_paths, 16, n_m, out)
     got = out.cpu().numpy().astype(np.float64)
     n = got.size
     assert abs(got.mean()) < 4 / math.sqrt(n)
@@ -235,12 +236,12 @@ def cached_oracle_run(orc, name, w):
     return _ORACLE_CACHE[name]
 
 
-@pytest.mark.parametrize("sincos", ["SFU", "FMA", "SFU-W32"])
+@pytest.mark.parametrize("sincos", ["SFU", "FMA", "SFU-W32", "SFU-W16P"])
 @pytest.mark.parametrize("name,make,_", FP32_CASES, ids=[c[0] for c in FP32_CASES])
 def test_fp32_within_3_combined_se(B, orc, name, make, _, sincos):
     w = make()
     sc = B.BM_SINCOS_FMA if sincos == "FMA" else B.BM_SINCOS_SFU
-    gs = B.BM_GAUSS_W32 if sincos.endswith("W32") else B.BM_GAUSS_AUTO
+    gs = B.BM_GAUSS_W32 if sincos.endswith("W32") else B.BM_GAUSS_W16P if sincos.endswith("W16P") else B.BM_GAUSS_AUTO
     stats, paths, _ = B.run_workload(w, B.BM_F32, want_paths=True, sincos=sc, gauss=gs)
     ref = cached_oracle_run(orc, name, w)
     for pt in range(w.n_points):
