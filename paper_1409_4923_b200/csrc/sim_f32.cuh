@@ -501,34 +501,44 @@ __global__ void __launch_bounds__(256) bm_paths_f32(const __grid_constant__ SimA
       }
       fold_f32<POT>(x, wraps);
       if (!ROLLED) {
+        // pair slot by pair slot: a slot without event or special cell is the clean path's code for two cells
 #pragma unroll
         for (int i = 0; i < NP; ++i) {
           Pair nxt = cur;
-          if (HAS_G) {
-            next_rounds(wn, i);
-            nxt = (i + 1 < NP) ? pair_of<GW>(w, i + 1, P.cn) : pair_of<GW>(wn, 0, P.cn);
-          }
-#pragma unroll
-          for (int jj = 0; jj < 2; ++jj) {
-            const int j = 2 * i + jj;
-            const unsigned m = ctl >> j;
-            bool run = true;
-            if (m & 0x100u) {
-              if (n + j >= n_steps) {
-                run = false;
-              } else {  // a10: t_i
-                fold_f32<POT>(x, wraps);
-                snap_x = x;
-                snap_w = wraps;
-              }
+          if (((ctl >> (2 * i)) & 0x303u) == 0u) {
+            if (HAS_G) {
+              next_rounds(wn, i);
+              nxt = (i + 1 < NP) ? pair_of<GW>(w, i + 1, P.cn) : pair_of<GW>(wn, 0, P.cn);
             }
-            if (run) {
-              const float gc = jj ? cur.s : cur.c;
-              if ((HAS_P || HAS_D) && (m & 1u)) {
-                slow_cell(n + j, cur.r * gc);
-                ctl |= __reduce_or_sync(FULL, ev_bits(n)) & 0xFFu;  // events re-scheduled into this block
-              } else {
-                fast_cell(cur.r, gc, false);
+            fast_cell(cur.r, cur.c, false);
+            fast_cell(cur.r, cur.s, false);
+          } else {
+            if (HAS_G) {
+              next_rounds(wn, i);
+              nxt = (i + 1 < NP) ? pair_of<GW>(w, i + 1, P.cn) : pair_of<GW>(wn, 0, P.cn);
+            }
+#pragma unroll
+            for (int jj = 0; jj < 2; ++jj) {
+              const int j = 2 * i + jj;
+              const unsigned m = ctl >> j;
+              bool run = true;
+              if (m & 0x100u) {
+                if (n + j >= n_steps) {
+                  run = false;
+                } else {  // a10: t_i
+                  fold_f32<POT>(x, wraps);
+                  snap_x = x;
+                  snap_w = wraps;
+                }
+              }
+              if (run) {
+                const float gc = jj ? cur.s : cur.c;
+                if ((HAS_P || HAS_D) && (m & 1u)) {
+                  slow_cell(n + j, cur.r * gc);
+                  ctl |= __reduce_or_sync(FULL, ev_bits(n)) & 0xFFu;  // events re-scheduled into this block
+                } else {
+                  fast_cell(cur.r, gc, false);
+                }
               }
             }
           }
