@@ -67,10 +67,12 @@ struct Launch {
 
 bm_status pick_kernel(const bm_config *c, int32_t n_points, int64_t n_paths, Launch *L) {
   *L = Launch();
-  if (c->scheme == BM_SCHEME_PAPER_LITERAL) return BM_ERR_UNSUPPORTED;  // NEXT row f1, not built yet
+  if (c->scheme == BM_SCHEME_PAPER_LITERAL && c->model != BM_OVERDAMPED) return BM_ERR_UNSUPPORTED;
   if (c->model == BM_INERTIAL && c->potential != BM_POT_SINE2) return BM_ERR_UNSUPPORTED;
   L->threads = block_threads_of(c, n_points, n_paths);
-  if (c->prec == BM_F64) {
+  if (c->scheme == BM_SCHEME_PAPER_LITERAL) {
+    L->fn = pick_literal(c->prec, c->potential, c->noise);
+  } else if (c->prec == BM_F64) {
     L->fn = c->model == BM_OVERDAMPED ? pick_f64_overdamped(c->potential, c->noise)
                                       : pick_f64_inertial(c->potential, c->noise);
   } else {

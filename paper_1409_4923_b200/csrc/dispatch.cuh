@@ -22,6 +22,9 @@ KernelFn pick_f32_od_fma_w16p(int potential, int noise);
 KernelFn pick_f32_in_sfu_w16p(int potential, int noise);
 KernelFn pick_f32_in_fma_w16p(int potential, int noise);
 
+// the paper's own scheme as printed (sim_literal.cu); over-damped only
+KernelFn pick_literal(int prec, int potential, int noise);
+
 // fills (fill.cu)
 cudaError_t launch_philox_fill(const PhiloxKeys &K, unsigned long long path0, int n_paths, uint32_t stream_id,
                                uint32_t idx0, int n_idx, uint32_t *out, cudaStream_t st);

@@ -295,3 +295,77 @@ def test_quad_ou_fp64_matches_closed_form_and_oracle(B, orc):
     _, p16, _ = B.run_workload(w, B.BM_F32, want_paths=True)          # W16: other normals, same law
     assert abs(p16[:, B.BM_OUT_XT].mean() - x0 * R ** n) < 4 * math.sqrt(var_n / 4096)
     assert abs(p16[:, B.BM_OUT_XT].var(ddof=1) - var_n) < 4 * var_n * math.sqrt(2 / 4095)
+
+
+# ---- row f1: the paper's own scheme as printed (Alg. 1-4), CUDA against the oracle ------------------------------
+
+def literal_workloads():
+    a, DP = 1.5, 1.0
+    zeta, lam = DP / a, a * a / DP
+    Fa, Fb, tau = 3.0, 1.6, 0.3
+    mu_a, mu_b = Fa / (tau * (Fa + Fb)), Fb / (tau * (Fa + Fb))
+    L = W.SCHEME_PAPER_LITERAL
+    return {
+        # model I of the paper: piece-wise linear potential + white Poissonian noise (+ thermal)
+        "I": W.Workload("lit-I", W.OVERDAMPED, W.params_table(1, A1=1.0, D=0.05, lambda_=lam, zeta=zeta), 777, 8000,
+                        (1 / lam) / 400, 800, potential=W.POT_PWL, scheme=L),
+        # model II: piece-wise linear potential + dichotomous noise
+        "II": W.Workload("lit-II", W.OVERDAMPED, W.params_table(1, A1=1.0, D=0.0, Fa=Fa, Fb=Fb, mu_a=mu_a, mu_b=mu_b),
+                         640, 8000, min(1 / mu_a, 1 / mu_b) / 200, 800, potential=W.POT_PWL, scheme=L),
+        # all three sources on the smooth two-harmonic potential, a two-point sweep with a switched-off point
+        "all": W.Workload("lit-all", W.OVERDAMPED,
+                          W.params_table(2, A1=1.0, A2=0.25, F=0.05, D=[0.02, 0.0], lambda_=[2.0, 0.0], zeta=0.3,
+                                         Fa=0.4, Fb=0.8, mu_a=1.5, mu_b=3.0), 300, 5000, 1e-3, 500, scheme=L),
+    }
+
+
+@pytest.mark.parametrize("name", ["I", "II", "all"])
+def test_literal_scheme_fp64_matches_oracle_per_path(B, orc, name):
+    w = literal_workloads()[name]
+    stats, paths, _ = B.run_workload(w, B.BM_F64, want_paths=True)
+    ref, _ = oracle_run(orc, w)
+    assert np.array_equal(paths[:, B.BM_OUT_JUMPS], ref[:, orc.OUT_JUMPS]), "kick / flip counts differ"
+    assert np.array_equal(paths[:, B.BM_OUT_SUBSTEPS], ref[:, orc.OUT_SUBSTEPS])
+    dx = np.abs(paths[:, B.BM_OUT_XT] - ref[:, orc.OUT_XT])
+    bad = np.nonzero(dx > 1e-8 * (1 + np.abs(ref[:, orc.OUT_XT])))[0]
+    # the piece-wise linear force is discontinuous: a 1-ulp difference at a kink flips a stage force
+    assert bad.size <= (4 if w.potential == W.POT_PWL else 0), f"{bad.size} paths beyond tolerance, max {dx.max():.3e}"
+    good = np.setdiff1d(np.arange(dx.size), bad)
+    assert np.abs(paths[good, B.BM_OUT_VBAR] - ref[good, orc.OUT_VBAR]).max() < 1e-8
+    if bad.size == 0:
+        for pt in range(w.n_points):
+            o = orc.reduce(ref[pt * w.n_paths:(pt + 1) * w.n_paths])
+            assert abs(stats[pt, 1] - o["mean_v"]) <= 1e-9 * abs(o["mean_v"]) + 1e-12
+            assert abs(stats[pt, 5] - o["mean_jumps"]) <= 1e-12 * max(1.0, o["mean_jumps"])
+
+
+def test_literal_scheme_fp64_trace(B, orc):
+    w = literal_workloads()["all"].scaled(n_paths=64, n_steps=600)
+    ref, tr_ref = oracle_run(orc, w, trace_paths=64, trace_steps=600)
+    _, _, tr = B.run_workload(w, B.BM_F64, want_paths=True, trace_steps=600, trace_paths=64)
+    assert np.abs(tr[:, :, 0] - tr_ref[:, :, 0]).max() < 1e-9 and np.all(tr[:, :, 1] == 0.0)
+
+
+@pytest.mark.parametrize("name", ["I", "II", "all"])
+def test_literal_scheme_fp32_within_3_combined_se(B, orc, name):
+    w = literal_workloads()[name].scaled(n_paths=2048)
+    _, paths, _ = B.run_workload(w, B.BM_F32, want_paths=True)
+    ref, _ = oracle_run(orc, w)
+    for pt in range(w.n_points):
+        sl = slice(pt * w.n_paths, (pt + 1) * w.n_paths)
+        assert_3se(paths[sl], ref[sl], B.BM_OUT_VBAR, f"literal {name} point {pt} <v>")
+        assert_3se(paths[sl], ref[sl], B.BM_OUT_XT, f"literal {name} point {pt} x(T)")
+        # same words, countdowns quantised to the grid: the counts agree up to fp32 rounding of a few waiting times
+        assert abs(paths[sl, B.BM_OUT_JUMPS].mean() - ref[sl, orc.OUT_JUMPS].mean()) <= 0.02 * max(1.0, ref[sl, orc.OUT_JUMPS].mean())
+
+
+def test_literal_scheme_rejects_inertial(B):
+    import torch
+    w = W.c2().scaled(n_paths=32, n_steps=16)
+    cfg = B.config_for(w, B.BM_F64)
+    cfg.scheme = B.BM_SCHEME_PAPER_LITERAL
+    p = torch.from_numpy(np.ascontiguousarray(w.params)).cuda()
+    st = torch.zeros((1, 8), dtype=torch.float64, device="cuda")
+    with pytest.raises(B.BmError) as e:
+        B.bm_simulate(cfg, p, 1, w.n_paths, w.n_steps, w.dt, w.seed, st)
+    assert e.value.status == B.BM_ERR_UNSUPPORTED
