@@ -35,6 +35,9 @@ UNIT = "path-steps/s"
 # A kick adds 2 lg2 (waiting time, amplitude), a flip 1; sub-steps and events are COUNTED by the kernel.
 XU_OPS_PER_SUBSTEP = {0: 5.0, 1: 6.0}
 XU_LANES_PER_SM = 16          # MUFU lanes per SM per clock (4 per SM sub-partition); confirmed by bm_pipe_probe
+# dram__bytes_read.sum + dram__bytes_write.sum of one path-kernel launch from the committed `ncu --set full` captures
+# (profiles/r1_f32_v5.md): parameters and per-block partials only, the path is register-resident.  Bytes per launch.
+NCU_DRAM_BYTES = {("C1", "f32"): 56832, ("C2", "f32"): 36096}
 
 
 def parse():
@@ -52,7 +55,7 @@ def parse():
     ap.add_argument("--scale-steps", type=float, default=1.0, help="shrink n_steps (profiling runs only; flagged)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-fp64", action="store_true")
-    ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
     return ap.parse_args()
 
 
@@ -91,7 +94,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
         except OSError:
             self.proc = None
@@ -304,7 +307,7 @@ def run_ours(args):
         e2e_total = float(tt.item())
     e2e = {"value": world * w.path_steps / (e2e_total * 1e-3), "unit": UNIT,
            "h2d_bytes_per_step": int(run.h_params.numel() * 8), "d2h_bytes_per_step": int(run.h_stats.numel() * 8),
-           "ms_per_step": e2e_total, "call": "bm_simulate_host (cudaMalloc + H2D + kernels + D2H + sync per call)"}
+           "ms_per_step": e2e_total, "call": "bm_simulate_host (stream-ordered alloc + H2D + kernels + D2H + sync per call)"}
     if world == 1 and not np.array_equal(run.h_stats.numpy(), stats):
         raise SystemExit("bench.py: host-pointer call and device-pointer call disagree (determinism contract broken)")
 
@@ -322,7 +325,9 @@ def run_ours(args):
     peak = XU_LANES_PER_SM * info["sm_count"] * sm_mhz * 1e6 / 1e9
     achieved = xu_ops / (ms_per_step * 1e-3) / 1e9
     roof = {"bound": "alu", "pipe": "xu (MUFU) for fp32; fp64 runs the same algorithm on the FP64 pipe",
-            "achieved": achieved, "peak": peak, "unit": "Gop/s", "frac": achieved / peak, "traffic": None,
+            "achieved": achieved, "peak": peak, "unit": "Gop/s", "frac": achieved / peak,
+            "traffic": NCU_DRAM_BYTES.get((w.name, args.prec)) if args.scale_steps == 1.0 else None,
+            "traffic_source": "profiles/r1_f32_v5.md (ncu --set full, dram bytes of one launch; independent of n_steps)",
             "peak_source": f"derived: {XU_LANES_PER_SM} MUFU lanes/SM/clk x {info['sm_count']} SMs x {sm_mhz:.0f} MHz "
                            "(max SM clock; lane count confirmed by bm_pipe_probe, DESIGN.md section 6)",
             "ops_per_path_step": xu_per_path / w.n_steps, "kernel": "bm_paths_f32" if prec == B.BM_F32 else "bm_paths_f64",

@@ -170,11 +170,11 @@ BM_API bm_status bm_simulate_host(const bm_config *cfg, const bm_params *params,
   const size_t ob = out_paths ? (size_t)n_points * (size_t)n_paths * BM_OUT_STRIDE * sizeof(double) : 0;
   void *d_params = nullptr, *d_stats = nullptr, *d_ws = nullptr, *d_paths = nullptr;
   bm_status rc = BM_ERR_CUDA;
-  do {
-    if (cudaMalloc(&d_params, pb) != cudaSuccess) break;
-    if (cudaMalloc(&d_stats, sb) != cudaSuccess) break;
-    if (cudaMalloc(&d_ws, ws) != cudaSuccess) break;
-    if (ob && cudaMalloc(&d_paths, ob) != cudaSuccess) break;
+  do {  // stream-ordered allocation: after the first call the blocks come from the device's memory pool
+    if (cudaMallocAsync(&d_params, pb, st) != cudaSuccess) break;
+    if (cudaMallocAsync(&d_stats, sb, st) != cudaSuccess) break;
+    if (cudaMallocAsync(&d_ws, ws, st) != cudaSuccess) break;
+    if (ob && cudaMallocAsync(&d_paths, ob, st) != cudaSuccess) break;
     if (cudaMemcpyAsync(d_params, params, pb, cudaMemcpyHostToDevice, st) != cudaSuccess) break;
     rc = bm_simulate(cfg, (const bm_params *)d_params, n_points, n_paths, n_steps, dt, seed, (bm_stats *)d_stats,
                      (double *)d_paths, nullptr, d_ws, ws, stream);
@@ -182,11 +182,14 @@ BM_API bm_status bm_simulate_host(const bm_config *cfg, const bm_params *params,
     rc = BM_ERR_CUDA;
     if (cudaMemcpyAsync(out_stats, d_stats, sb, cudaMemcpyDeviceToHost, st) != cudaSuccess) break;
     if (ob && cudaMemcpyAsync(out_paths, d_paths, ob, cudaMemcpyDeviceToHost, st) != cudaSuccess) break;
-    if (cudaStreamSynchronize(st) != cudaSuccess) break;
     rc = BM_OK;
   } while (0);
+  if (d_params) cudaFreeAsync(d_params, st);
+  if (d_stats) cudaFreeAsync(d_stats, st);
+  if (d_ws) cudaFreeAsync(d_ws, st);
+  if (d_paths) cudaFreeAsync(d_paths, st);
+  if (cudaStreamSynchronize(st) != cudaSuccess && rc == BM_OK) rc = BM_ERR_CUDA;
   if (rc == BM_ERR_CUDA) cudaGetLastError();
-  cudaFree(d_params); cudaFree(d_stats); cudaFree(d_ws); cudaFree(d_paths);
   return rc;
 }
 

@@ -1,8 +1,8 @@
-// sim_f32.cuh -- fp32 path kernel (the throughput kernel), v3.  One thread = one realization; position, clocks,
+// sim_f32.cuh -- fp32 path kernel (the throughput kernel), v5.  One thread = one realization; position, clocks,
 // Gaussian cache and observable snapshot stay in registers for the whole run.
 //
 // Same method as the fp64 kernel (R1-R9), arranged for fp32 accuracy and for the SM's pipes
-// (profiles/r1_c1_f32_v2.md is the measurement this layout answers):
+// (profiles/r1_c1_f32_v3.md and profiles/r1_f32_v5.md are the measurements this layout answers):
 //  * the position is carried as theta = 2 pi x / L (radians of the potential's phase), folded to [-pi, pi) with an
 //    int32 wrap counter by a round-to-nearest "magic add" (no F2I/FRND, which share the 16-lane XU
 //    pipe with MUFU).  In these units a force cosine is FMUL.RZ + MUFU.COS with no scaling multiply in front;
@@ -10,18 +10,25 @@
 //    x1 = (xs + h K0) + c (h K1 + h K2 c), so every stage is 2 FFMA behind its cosine;
 //  * ALL lanes of a warp are always in the SAME grid cell n (the cell counter is warp-uniform).  A cell without a
 //    kick or flip in any lane is one FAST step with loop-invariant constants; NB such cells (one Philox call of
-//    normals) form one basic block when no lane has an event within them (one vote per block);
+//    normals) form one basic block when no lane has an event within them (one vote per block).  Otherwise the warp
+//    forms a uniform control word (REDUX.OR of the lanes' event bits) and runs the block pair slot by pair slot: a
+//    slot without an event is the clean path's two-cell code, a cell with an event in some lane is a SLOW cell;
+//  * the Box-Muller pair of cells (2i+2, 2i+3) is formed while cells (2i, 2i+1) run, and the ten Philox rounds of
+//    the next Gaussian call are spread over the pair slots, so the integer and MUFU work of the Gaussians sits in
+//    the stalls of the serial cosine chain of Alg. 1 instead of in a phase of its own;
 //  * a lane with events inside the current cell integrates up to each event on its own (a divergent loop:
 //    sub-step of length h, a8, redraw of the clock), then every lane finishes the cell together with its own
 //    remaining length (a5).  The Gaussian of a grid cell comes from the Gaussian stream indexed by the CELL, the
-//    Gaussian of a sub-step that ends at an event from the spare word of that event's own Philox call (R13), so
-//    the normal cache never gets out of phase between lanes;
+//    Gaussian of a sub-step that ends at event k from the spare word of call k of that event's stream, drawn one
+//    event earlier (R13), so the normal cache never gets out of phase between lanes and the Philox rounds of a
+//    redraw do not sit in front of the sub-step that needs the normal;
 //  * a jump clock is (cell index, offset in that cell), so nothing small is ever subtracted from something large;
 //  * the Box-Muller radius carries the noise amplitude (sqrt(-2 ln u) * sqrt(2 D dt) in one MUFU.SQRT);
 //  * uniforms come from Philox words through a mantissa splice (no I2F).  BM_GAUSS_W32: one word per uniform,
 //    four normals per call (the oracle's assignment R3, so a jump-free fp32 path follows the oracle's path);
 //    BM_GAUSS_W16: radius from the top 23 bits and angle from the low 16 bits of ONE word, eight normals per
 //    call -- half the integer work (IMAD.WIDE is a quarter-rate instruction on sm_100, DESIGN.md s.6);
+//    BM_GAUSS_W16P: W16 with the angle's sine and cosine as polynomials on the FMA pipe (two MUFU per pair);
 //  * transcendental functions: MUFU.{COS,SIN,LG2,SQRT} (SFU variant) or, for the force cosine,
 //    an even polynomial on the FMA pipe (FMA variant) -- a measured choice (DESIGN.md s.6).
 // fp32 results are judged statistically against the fp64 oracle (3 combined standard errors).
