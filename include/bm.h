@@ -133,8 +133,9 @@ BM_API bm_status bm_simulate(const bm_config *cfg, const bm_params *params, int3
 
 /*
  * HOST-pointer convenience entry (the end-to-end path): params, out_stats and out_paths (optional) are HOST
- * buffers.  Allocates device memory, copies params in, runs bm_simulate on `stream`, copies the results
- * out, synchronises the stream and frees the device memory.
+ * buffers.  Takes device scratch from a private stream-ordered pool (one per device, kept between calls: an
+ * allocation cache with no influence on results), copies params in, runs bm_simulate on `stream`, copies the
+ * results out, returns the scratch to the pool and synchronises the stream.
  */
 BM_API bm_status bm_simulate_host(const bm_config *cfg, const bm_params *params, int32_t n_points, int64_t n_paths,
                            int64_t n_steps, double dt, uint64_t seed, bm_stats *out_stats, double *out_paths,

@@ -89,6 +89,28 @@ bm_status pick_kernel(const bm_config *c, int32_t n_points, int64_t n_paths, Lau
   return BM_OK;
 }
 
+// Scratch pool of the HOST-pointer entry: one private stream-ordered pool per device that keeps its blocks between
+// calls (release threshold = never), so that only the first call pays for device allocations.  A cache only: it has
+// no influence on any result.
+cudaMemPool_t host_entry_pool() {
+  static cudaMemPool_t pools[64] = {};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
+  if (!pools[dev]) {
+    cudaMemPoolProps props = {};
+    props.allocType = cudaMemAllocationTypePinned;
+    props.handleTypes = cudaMemHandleTypeNone;
+    props.location.type = cudaMemLocationTypeDevice;
+    props.location.id = dev;
+    cudaMemPool_t pool = nullptr;
+    if (cudaMemPoolCreate(&pool, &props) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    unsigned long long keep = ~0ULL;
+    cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    pools[dev] = pool;
+  }
+  return pools[dev];
+}
+
 long long blocks_per_point_of(const bm_config *c, int32_t n_points, int64_t n_paths) {
   const int bt = block_threads_of(c, n_points, n_paths);
   return (n_paths + bt - 1) / bt;
@@ -170,11 +192,13 @@ BM_API bm_status bm_simulate_host(const bm_config *cfg, const bm_params *params,
   const size_t ob = out_paths ? (size_t)n_points * (size_t)n_paths * BM_OUT_STRIDE * sizeof(double) : 0;
   void *d_params = nullptr, *d_stats = nullptr, *d_ws = nullptr, *d_paths = nullptr;
   bm_status rc = BM_ERR_CUDA;
-  do {  // stream-ordered allocation: after the first call the blocks come from the device's memory pool
-    if (cudaMallocAsync(&d_params, pb, st) != cudaSuccess) break;
-    if (cudaMallocAsync(&d_stats, sb, st) != cudaSuccess) break;
-    if (cudaMallocAsync(&d_ws, ws, st) != cudaSuccess) break;
-    if (ob && cudaMallocAsync(&d_paths, ob, st) != cudaSuccess) break;
+  cudaMemPool_t pool = host_entry_pool();
+  if (!pool) return BM_ERR_CUDA;
+  do {  // stream-ordered allocation: after the first call the blocks come from the library's pool
+    if (cudaMallocFromPoolAsync(&d_params, pb, pool, st) != cudaSuccess) break;
+    if (cudaMallocFromPoolAsync(&d_stats, sb, pool, st) != cudaSuccess) break;
+    if (cudaMallocFromPoolAsync(&d_ws, ws, pool, st) != cudaSuccess) break;
+    if (ob && cudaMallocFromPoolAsync(&d_paths, ob, pool, st) != cudaSuccess) break;
     if (cudaMemcpyAsync(d_params, params, pb, cudaMemcpyHostToDevice, st) != cudaSuccess) break;
     rc = bm_simulate(cfg, (const bm_params *)d_params, n_points, n_paths, n_steps, dt, seed, (bm_stats *)d_stats,
                      (double *)d_paths, nullptr, d_ws, ws, stream);
