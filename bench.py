@@ -260,7 +260,8 @@ def run_ours(args):
     w = workload_of(args)
     prec = B.BM_F32 if args.prec == "f32" else B.BM_F64
     sc = sincos_of(B, args.sincos)
-    seed = w.seed + rank                                # replicas only: independent ensembles, no collective
+    from paper_1409_4923_b200 import replicas
+    seed = replicas.replica_seed(w.seed, rank)          # replicas only: independent ensembles, no collective
     run = Runner(B, torch, w, prec, sc, args.block_threads, seed, dev, stream,
                  {"auto": B.BM_GAUSS_AUTO, "w32": B.BM_GAUSS_W32, "w16": B.BM_GAUSS_W16, "w16p": B.BM_GAUSS_W16P}[args.gauss])
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
@@ -288,24 +289,16 @@ def run_ours(args):
     t_wall1 = time.time()
     clocks = sampler.stop(t_wall0, t_wall1)
     stats = run.stats.cpu().numpy().copy()
-    total_ms = float(sum(ms))
-    if dist is not None:
-        tt = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)       # timing plumbing only (max over ranks)
-        total_ms = float(tt.item())
+    total_ms = replicas.max_over_ranks(float(sum(ms)), dist, dev)   # timing plumbing only (max over ranks)
     ms_per_step = total_ms / args.steps
-    value = world * w.path_steps / (ms_per_step * 1e-3)
+    value = replicas.whole_job_value(w.path_steps, world, ms_per_step)
 
     # e2e: same metric through the HOST-pointer C-ABI call (copies inside the timed region)
     run.host_step()
     barrier()
     e2e_ms = [run.host_step() for _ in range(max(2, min(args.steps, 5)))]
-    e2e_total = float(np.mean(e2e_ms))
-    if dist is not None:
-        tt = torch.tensor([e2e_total], dtype=torch.float64, device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        e2e_total = float(tt.item())
-    e2e = {"value": world * w.path_steps / (e2e_total * 1e-3), "unit": UNIT,
+    e2e_total = replicas.max_over_ranks(float(np.mean(e2e_ms)), dist, dev)
+    e2e = {"value": replicas.whole_job_value(w.path_steps, world, e2e_total), "unit": UNIT,
            "h2d_bytes_per_step": int(run.h_params.numel() * 8), "d2h_bytes_per_step": int(run.h_stats.numel() * 8),
            "ms_per_step": e2e_total, "call": "bm_simulate_host (stream-ordered alloc + H2D + kernels + D2H + sync per call)"}
     if world == 1 and not np.array_equal(run.h_stats.numpy(), stats):
