@@ -132,6 +132,29 @@ BM_API bm_status bm_simulate(const bm_config *cfg, const bm_params *params, int3
                       double *out_trace, void *workspace, size_t workspace_bytes, void *stream);
 
 /*
+ * Chunked runs and checkpoint / resume (Alg. 5 steps 2 and 6: "load the state
+ * ... advance `samples` steps ... save the state").  bm_simulate_chunk performs grid steps
+ * [step_begin, step_begin + step_count) of a run of n_steps steps.  step_begin == 0 initialises the paths (the
+ * contents of `state` are ignored); any other chunk continues from `state` as the previous chunk left it.  Every chunk
+ * rewrites `state`; the chunk that reaches n_steps also writes out_stats (and out_paths, if given) -- for the other
+ * chunks they are not touched.  A run cut into chunks gives bit-identical results to the single bm_simulate call
+ * with the same arguments.  The Philox generator is stateless, so the state of a path is its position, clocks,
+ * counters and snapshot: BM_STATE_SLOTS 8-byte words per path, slot-major ([slot][n_points*n_paths], coalesced).
+ *   state      device, >= bm_state_bytes(...) bytes, 16-byte aligned; owned by the caller, may be copied to the host
+ *              and back between chunks (that is the checkpoint)
+ * step_begin, and step_begin + step_count unless it equals n_steps, must be multiples of BM_CHUNK_ALIGN.  All other
+ * arguments as bm_simulate and the same in every chunk of a run (not checked).  No trace output in chunked runs.
+ * Errors: as bm_simulate; BM_ERR_INVALID_ARG for a misaligned or out-of-range chunk or a null / misaligned state;
+ * BM_ERR_WORKSPACE for a state buffer that is too small.
+ */
+enum { BM_STATE_SLOTS = 16, BM_CHUNK_ALIGN = 8 };
+BM_API size_t bm_state_bytes(const bm_config *cfg, int32_t n_points, int64_t n_paths);
+BM_API bm_status bm_simulate_chunk(const bm_config *cfg, const bm_params *params, int32_t n_points, int64_t n_paths,
+                            int64_t n_steps, double dt, uint64_t seed, int64_t step_begin, int64_t step_count,
+                            void *state, size_t state_bytes, bm_stats *out_stats, double *out_paths, void *workspace,
+                            size_t workspace_bytes, void *stream);
+
+/*
  * HOST-pointer convenience entry (the end-to-end path): params, out_stats and out_paths (optional) are HOST
  * buffers.  Takes device scratch from a private stream-ordered pool (one per device, kept between calls: an
  * allocation cache with no influence on results), copies params in, runs bm_simulate on `stream`, copies the

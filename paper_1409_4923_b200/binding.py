@@ -25,7 +25,8 @@ BM_OUT_XT, BM_OUT_VT, BM_OUT_VBAR, BM_OUT_JUMPS, BM_OUT_SUBSTEPS, BM_OUT_XTI, BM
 (BM_PROBE_FFMA, BM_PROBE_MUFU_COS, BM_PROBE_MUFU_LG2, BM_PROBE_MUFU_SQRT, BM_PROBE_IMAD_WIDE, BM_PROBE_LOP3,
  BM_PROBE_DFMA, BM_PROBE_I2F, BM_PROBE_FADD, BM_PROBE_MIX, BM_PROBE_COUNT) = range(11)
 
-EXPORTS = ("bm_workspace_bytes", "bm_simulate", "bm_simulate_host", "bm_philox_fill", "bm_gauss_fill",
+BM_STATE_SLOTS, BM_CHUNK_ALIGN = 16, 8
+EXPORTS = ("bm_workspace_bytes", "bm_simulate", "bm_state_bytes", "bm_simulate_chunk", "bm_simulate_host", "bm_philox_fill", "bm_gauss_fill",
            "bm_kernel_info", "bm_pipe_probe", "bm_status_string", "bm_version")
 STATS_FIELDS = ("n", "mean_v", "var_v", "mean_xT", "var_xT", "mean_jumps", "mean_substeps", "rsv")
 
@@ -59,6 +60,10 @@ def lib():
         L.bm_workspace_bytes.restype = C.c_size_t
         L.bm_simulate.argtypes = [cfgp, vp, i32, i64, i64, dbl, u64, vp, vp, vp, vp, C.c_size_t, vp]
         L.bm_simulate.restype = C.c_int
+        L.bm_state_bytes.argtypes = [cfgp, i32, i64]
+        L.bm_state_bytes.restype = C.c_size_t
+        L.bm_simulate_chunk.argtypes = [cfgp, vp, i32, i64, i64, dbl, u64, i64, i64, vp, C.c_size_t, vp, vp, vp, C.c_size_t, vp]
+        L.bm_simulate_chunk.restype = C.c_int
         L.bm_simulate_host.argtypes = [cfgp, vp, i32, i64, i64, dbl, u64, vp, vp, vp]
         L.bm_simulate_host.restype = C.c_int
         L.bm_philox_fill.argtypes = [u64, u64, i32, u32, u32, i32, vp, vp]
@@ -139,6 +144,30 @@ def bm_simulate(cfg, params, n_points, n_paths, n_steps, dt, seed, out_stats, ou
                            workspace.numel(), _stream_ptr(stream))
     if rc != BM_OK:
         raise BmError(rc, "bm_simulate")
+    return workspace
+
+
+def bm_state_bytes(cfg, n_points, n_paths):
+    return int(lib().bm_state_bytes(C.byref(cfg), n_points, n_paths))
+
+
+def bm_simulate_chunk(cfg, params, n_points, n_paths, n_steps, dt, seed, step_begin, step_count, state, out_stats,
+                      out_paths=None, workspace=None, stream=None):
+    """Grid steps [step_begin, step_begin + step_count) of a run of n_steps; `state` is a CUDA uint8 tensor of at least
+    bm_state_bytes(...) bytes that carries the run from chunk to chunk (the checkpoint)."""
+    import torch
+    assert params.is_cuda and params.dtype == torch.float64 and params.numel() == 16 * n_points
+    assert out_stats.is_cuda and out_stats.dtype == torch.float64 and out_stats.numel() == 8 * n_points
+    assert state.is_cuda and state.dtype == torch.uint8 and state.is_contiguous()
+    if workspace is None:
+        workspace = torch.empty(max(bm_workspace_bytes(cfg, n_points, n_paths), 16), dtype=torch.uint8, device=params.device)
+    op = C.c_void_p(out_paths.data_ptr()) if out_paths is not None else None
+    rc = lib().bm_simulate_chunk(C.byref(cfg), C.c_void_p(params.data_ptr()), n_points, n_paths, n_steps, float(dt),
+                                 int(seed), int(step_begin), int(step_count), C.c_void_p(state.data_ptr()),
+                                 state.numel(), C.c_void_p(out_stats.data_ptr()), op,
+                                 C.c_void_p(workspace.data_ptr()), workspace.numel(), _stream_ptr(stream))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_simulate_chunk")
     return workspace
 
 

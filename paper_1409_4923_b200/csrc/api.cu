@@ -141,9 +141,11 @@ BM_API size_t bm_workspace_bytes(const bm_config *cfg, int32_t n_points, int64_t
   return (size_t)grid * PARTIAL_STRIDE * sizeof(double);
 }
 
-BM_API bm_status bm_simulate(const bm_config *cfg, const bm_params *params, int32_t n_points, int64_t n_paths,
-                      int64_t n_steps, double dt, uint64_t seed, bm_stats *out_stats, double *out_paths,
-                      double *out_trace, void *workspace, size_t workspace_bytes, void *stream) {
+// the launch behind bm_simulate (state == nullptr: the whole run) and bm_simulate_chunk
+static bm_status simulate_range(const bm_config *cfg, const bm_params *params, int32_t n_points, int64_t n_paths,
+                                int64_t n_steps, double dt, uint64_t seed, int64_t step_begin, int64_t step_end,
+                                void *state, bm_stats *out_stats, double *out_paths, double *out_trace, void *workspace,
+                                size_t workspace_bytes, void *stream) {
   if (!valid_cfg(cfg) || !params || !out_stats || n_points <= 0 || n_paths <= 0 || n_steps <= 0) return BM_ERR_INVALID_ARG;
   if (!(dt > 0.0) || !(dt < 1e300)) return BM_ERR_INVALID_ARG;
   if (cfg->n_discard >= n_steps) return BM_ERR_INVALID_ARG;
@@ -171,14 +173,45 @@ BM_API bm_status bm_simulate(const bm_config *cfg, const bm_params *params, int3
   a.dt = dt;
   a.n_points = n_points;
   a.blocks_per_point = (int)blocks_per_point_of(cfg, n_points, n_paths);
+  a.state = reinterpret_cast<unsigned long long *>(state);
+  a.step_begin = step_begin;
+  a.step_end = step_end;
   a.keys = make_keys(seed);
 
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   const unsigned grid = (unsigned)((long long)a.blocks_per_point * n_points);
   L.fn<<<grid, L.threads, 0, st>>>(a);  // a1: (point x path) -> grid
   if (cudaGetLastError() != cudaSuccess) return BM_ERR_CUDA;
+  if (step_end < n_steps) return BM_OK;  // the ensemble reduction belongs to the last chunk
   if (launch_grid_reduce(a.partials, n_points, a.blocks_per_point, out_stats, st) != cudaSuccess) return BM_ERR_CUDA;
   return BM_OK;
+}
+
+BM_API bm_status bm_simulate(const bm_config *cfg, const bm_params *params, int32_t n_points, int64_t n_paths,
+                      int64_t n_steps, double dt, uint64_t seed, bm_stats *out_stats, double *out_paths,
+                      double *out_trace, void *workspace, size_t workspace_bytes, void *stream) {
+  return simulate_range(cfg, params, n_points, n_paths, n_steps, dt, seed, 0, n_steps, nullptr, out_stats, out_paths,
+                        out_trace, workspace, workspace_bytes, stream);
+}
+
+BM_API size_t bm_state_bytes(const bm_config *cfg, int32_t n_points, int64_t n_paths) {
+  if (!valid_cfg(cfg) || n_points <= 0 || n_paths <= 0) return 0;
+  return (size_t)STATE_SLOTS * sizeof(unsigned long long) * (size_t)n_points * (size_t)n_paths;
+}
+
+BM_API bm_status bm_simulate_chunk(const bm_config *cfg, const bm_params *params, int32_t n_points, int64_t n_paths,
+                            int64_t n_steps, double dt, uint64_t seed, int64_t step_begin, int64_t step_count,
+                            void *state, size_t state_bytes, bm_stats *out_stats, double *out_paths, void *workspace,
+                            size_t workspace_bytes, void *stream) {
+  if (step_begin < 0 || step_count <= 0 || n_steps <= 0 || step_begin > n_steps - step_count) return BM_ERR_INVALID_ARG;
+  const int64_t step_end = step_begin + step_count;
+  // chunk boundaries inside a run sit on multiples of BM_CHUNK_ALIGN grid steps (one Gaussian call of the fp32 kernel)
+  if ((step_begin % BM_CHUNK_ALIGN) != 0 || (step_end != n_steps && (step_end % BM_CHUNK_ALIGN) != 0)) return BM_ERR_INVALID_ARG;
+  if (!state || ((uintptr_t)state & 15)) return BM_ERR_INVALID_ARG;
+  const size_t need = bm_state_bytes(cfg, n_points, n_paths);
+  if (need == 0 || state_bytes < need) return BM_ERR_WORKSPACE;
+  return simulate_range(cfg, params, n_points, n_paths, n_steps, dt, seed, step_begin, step_end, state, out_stats,
+                        out_paths, nullptr, workspace, workspace_bytes, stream);
 }
 
 BM_API bm_status bm_simulate_host(const bm_config *cfg, const bm_params *params, int32_t n_points, int64_t n_paths,

@@ -31,8 +31,29 @@ struct SimArgs {
   double dt;
   int n_points;
   int blocks_per_point;
+  // chunked runs (row f2): this launch does grid steps [step_begin, step_end) of a run of n_steps.  state == nullptr:
+  // a whole run in one launch (step_begin = 0, step_end = n_steps).
+  unsigned long long *state;  // [STATE_SLOTS][n_points * n_paths], 8-byte slots, slot-major (coalesced)
+  long long step_begin, step_end;
   PhiloxKeys keys;
 };
+
+// The resumable state of a path (Alg. 5 steps 2 and 6, without the RNG state: Philox is stateless,
+// so the draw counters are the RNG state).  Every kernel uses at most STATE_SLOTS 8-byte slots per path.
+constexpr int STATE_SLOTS = 16;
+struct StateIO {
+  unsigned long long *base;
+  long long stride;  // paths in the launch
+  __device__ __forceinline__ void put(int slot, unsigned long long v) const { base[(long long)slot * stride] = v; }
+  __device__ __forceinline__ unsigned long long get(int slot) const { return base[(long long)slot * stride]; }
+  __device__ __forceinline__ void put2(int slot, uint32_t lo, uint32_t hi) const { put(slot, (unsigned long long)lo | ((unsigned long long)hi << 32)); }
+  __device__ __forceinline__ void get2(int slot, uint32_t &lo, uint32_t &hi) const { const unsigned long long v = get(slot); lo = (uint32_t)v; hi = (uint32_t)(v >> 32); }
+  __device__ __forceinline__ void putd(int slot, double v) const { put(slot, (unsigned long long)__double_as_longlong(v)); }
+  __device__ __forceinline__ double getd(int slot) const { return __longlong_as_double((long long)get(slot)); }
+};
+__device__ __forceinline__ StateIO state_io(const SimArgs &a, unsigned long long g) {
+  return StateIO{a.state + g, (long long)a.n_points * a.n_paths};
+}
 
 constexpr uint32_t PHILOX_M0 = 0xD2511F53u, PHILOX_M1 = 0xCD9E8D57u;
 constexpr uint32_t PHILOX_W0 = 0x9E3779B9u, PHILOX_W1 = 0xBB67AE85u;

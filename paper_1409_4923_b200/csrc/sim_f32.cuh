@@ -323,7 +323,7 @@ __global__ void __launch_bounds__(256) bm_paths_f32(const __grid_constant__ SimA
   int d = 0;
   if (HAS_D) d = ((((double)wi.z + 0.5) * (1.0 / 4294967296.0)) < bp.mu_a / (bp.mu_a + bp.mu_b)) ? 1 : 0;
 
-  const int n_steps = (int)a.n_steps, n_discard = (int)a.n_discard;
+  const int n_discard = (int)a.n_discard;
   // jump clocks: (cell index, offset inside that cell); NEVER = switched off at this point
   int nP = NEVER, nD = NEVER;
   float fP = 0.f, fD = 0.f, z = 0.f;
@@ -355,6 +355,23 @@ __global__ void __launch_bounds__(256) bm_paths_f32(const __grid_constant__ SimA
   int jumps = 0;  // events applied = sub-steps that ended inside a cell
   float snap_x = x;
   int snap_w = wraps;
+  // row f2: a launch that continues a run reloads everything the lines above initialised (the Philox calls of the
+  // initialisation are wasted then, once per launch)
+  const int n_begin = (int)a.step_begin, n_end = (int)a.step_end;
+  if (a.state != nullptr && n_begin > 0) {
+    const StateIO io = state_io(a, g);
+    uint32_t lo, hi;
+    io.get2(0, lo, hi); x = __uint_as_float(lo); wraps = (int)hi;
+    io.get2(1, lo, hi); v = __uint_as_float(lo); jumps = (int)hi;
+    io.get2(2, lo, hi); nP = (int)lo; fP = __uint_as_float(hi);
+    io.get2(3, lo, hi); z = __uint_as_float(lo); kP = hi;
+    io.get2(4, gwP, gwD);
+    io.get2(5, lo, hi); nD = (int)lo; fD = __uint_as_float(hi);
+    io.get2(6, lo, hi); kD = lo; d = (int)hi;
+    ph = io.get(7);
+    io.get2(8, lo, hi); drive0 = __uint_as_float(lo); snap_x = __uint_as_float(hi);
+    io.get2(9, lo, hi); snap_w = (int)lo;
+  }
   float cst = P.base + (HAS_D ? (d ? P.Gb : P.Ga) : 0.f);
   const float hh_full = 0.5f * dt;
   // full-step constants of Alg. 1 (loop invariant; k0f, k0h follow cst across a flip)
@@ -467,7 +484,7 @@ __global__ void __launch_bounds__(256) bm_paths_f32(const __grid_constant__ SimA
   uint4 w = make_uint4(0u, 0u, 0u, 0u);
   Pair cur = Pair{0.f, 0.f, 0.f};
   if (HAS_G) {
-    w = philox_call(K, g, STREAM_GAUSS, 0);
+    w = philox_call(K, g, STREAM_GAUSS, (uint32_t)(n_begin / NB));
     cur = pair_of<GW>(w, 0, P.cn);
   }
   // rounds of the next Gaussian call done in pair slot i: NP = 4: 4 + 3 + 3 + 0, NP = 2: 10 + 0
@@ -480,10 +497,10 @@ __global__ void __launch_bounds__(256) bm_paths_f32(const __grid_constant__ SimA
       philox_rounds<0, 10>(c, K);
     }
   };
-  uint32_t blk = 0;
-  for (int n = 0; n < n_steps; n += NB) {
+  uint32_t blk = (uint32_t)(n_begin / NB);
+  for (int n = n_begin; n < n_end; n += NB) {
     blk++;
-    const bool special = ((unsigned)(n_discard - n) < (unsigned)NB) || (n + NB > n_steps);
+    const bool special = ((unsigned)(n_discard - n) < (unsigned)NB) || (n + NB > n_end);
     const bool clean = !special && !((HAS_P || HAS_D) && __any_sync(FULL, min(nP, nD) < n + NB));
     // counter of the next Gaussian call; its ten rounds are spread over the pair slots of this block
     uint4 wn = make_uint4(blk, (uint32_t)STREAM_GAUSS, (uint32_t)g, (uint32_t)(g >> 32));
@@ -504,7 +521,7 @@ __global__ void __launch_bounds__(256) bm_paths_f32(const __grid_constant__ SimA
       if (HAS_P || HAS_D) ctl = __reduce_or_sync(FULL, ev_bits(n)) & 0xFFu;
       if (special) {
         if ((unsigned)(n_discard - n) < (unsigned)NB) ctl |= 0x100u << (n_discard - n);
-        if (n + NB > n_steps) ctl |= (0xFF00u << (n_steps - n)) & 0xFF00u;
+        if (n + NB > n_end) ctl |= (0xFF00u << (n_end - n)) & 0xFF00u;
       }
       fold_f32<POT>(x, wraps);
       if (!ROLLED) {
@@ -530,7 +547,7 @@ __global__ void __launch_bounds__(256) bm_paths_f32(const __grid_constant__ SimA
               const unsigned m = ctl >> j;
               bool run = true;
               if (m & 0x100u) {
-                if (n + j >= n_steps) {
+                if (n + j >= n_end) {
                   run = false;
                 } else {  // a10: t_i
                   fold_f32<POT>(x, wraps);
@@ -567,7 +584,7 @@ __global__ void __launch_bounds__(256) bm_paths_f32(const __grid_constant__ SimA
         for (int j = 0; j < NB; ++j) {
           const unsigned m = ctl >> j;
           if (m & 0x100u) {
-            if (n + j >= n_steps) break;
+            if (n + j >= n_end) break;
             fold_f32<POT>(x, wraps);  // a10: t_i
             snap_x = x;
             snap_w = wraps;
@@ -584,6 +601,21 @@ __global__ void __launch_bounds__(256) bm_paths_f32(const __grid_constant__ SimA
     }
     w = wn;
   }
+
+  if (a.state != nullptr && valid) {  // row f2: checkpoint
+    const StateIO io = state_io(a, g);
+    io.put2(0, __float_as_uint(x), (uint32_t)wraps);
+    io.put2(1, __float_as_uint(v), (uint32_t)jumps);
+    io.put2(2, (uint32_t)nP, __float_as_uint(fP));
+    io.put2(3, __float_as_uint(z), kP);
+    io.put2(4, gwP, gwD);
+    io.put2(5, (uint32_t)nD, __float_as_uint(fD));
+    io.put2(6, kD, (uint32_t)d);
+    io.put(7, ph);
+    io.put2(8, __float_as_uint(drive0), __float_as_uint(snap_x));
+    io.put2(9, (uint32_t)snap_w, 0u);
+  }
+  if (a.step_end < a.n_steps) return;  // not the last chunk: no outputs yet (uniform over the grid)
 
   Partial mine = partial_zero();
   if (valid) {

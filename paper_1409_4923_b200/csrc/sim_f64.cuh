@@ -114,13 +114,28 @@ __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimA
     const bool tracing = a.out_trace != nullptr && (long long)g < a.trace_paths;
     double *trace = tracing ? a.out_trace + (long long)g * a.trace_steps * 2 : nullptr;
 
-    long long n = 0;
+    long long n = a.step_begin;
     unsigned long long m = 0;
     double rem = dt, jumps = 0.0;
     double gq[4] = {0.0, 0.0, 0.0, 0.0};
     StateF64 snap = s;
+    if (a.state != nullptr && a.step_begin > 0) {  // row f2: continue a run from its checkpoint
+      const StateIO io = state_io(a, g);
+      uint32_t lo, hi;
+      s.xi = io.getd(0); s.wraps = (long long)io.get(1); s.v = io.getd(2);
+      rP = io.getd(3); rD = io.getd(4); z = io.getd(5);
+      io.get2(6, kP, kD);
+      io.get2(7, lo, hi); d = (int)lo;
+      m = io.get(8); jumps = io.getd(9);
+      snap.xi = io.getd(10); snap.wraps = (long long)io.get(11); snap.v = io.getd(12);
+      if (HAS_G && (m & 3ull) != 0) {  // the Gaussian call in progress is recomputed, not stored
+        const uint4 w = philox_call(a.keys, g, STREAM_GAUSS, (uint32_t)(m >> 2));
+        box_muller_f64(w.x, w.y, gq[0], gq[1]);
+        box_muller_f64(w.z, w.w, gq[2], gq[3]);
+      }
+    }
     // R5: three countdown clocks; every sub-step has length h = min(rem, rP, rD)
-    while (n < a.n_steps) {
+    while (n < a.step_end) {
       double h = rem;
       if (HAS_P && onP && rP < h) h = rP;
       if (HAS_D && onD && rD < h) h = rD;
@@ -197,17 +212,27 @@ __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimA
         if (n == a.n_discard) snap = s;
       }
     }
+    if (a.state != nullptr) {  // row f2: checkpoint (chunks end on completed grid steps, so rem = dt)
+      const StateIO io = state_io(a, g);
+      io.putd(0, s.xi); io.put(1, (unsigned long long)s.wraps); io.putd(2, s.v);
+      io.putd(3, rP); io.putd(4, rD); io.putd(5, z);
+      io.put2(6, kP, kD);
+      io.put2(7, (uint32_t)d, 0u);
+      io.put(8, m); io.putd(9, jumps);
+      io.putd(10, snap.xi); io.put(11, (unsigned long long)snap.wraps); io.putd(12, snap.v);
+    }
     // a10: eq. (30)
     const double span = (double)(a.n_steps - a.n_discard) * dt;
     const double xT = unfolded_f64<POT>(s);
     const double vbar = ((double)(s.wraps - snap.wraps) * period_f64<POT>() + (s.xi - snap.xi)) / span;
-    if (a.out_paths) {
+    if (a.out_paths && a.step_end >= a.n_steps) {
       double *o = a.out_paths + g * BM_OUT_STRIDE;
       o[BM_OUT_XT] = xT; o[BM_OUT_VT] = s.v; o[BM_OUT_VBAR] = vbar; o[BM_OUT_JUMPS] = jumps;
       o[BM_OUT_SUBSTEPS] = (double)m; o[BM_OUT_XTI] = unfolded_f64<POT>(snap);
     }
     mine = leaf(vbar, xT, jumps, (double)m);
   }
+  if (a.step_end < a.n_steps) return;  // not the last chunk: the partials are not used (uniform over the grid)
   block_reduce_store(mine, a.partials + (long long)blockIdx.x * PARTIAL_STRIDE);
 }
 

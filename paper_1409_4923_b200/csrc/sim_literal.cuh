@@ -136,7 +136,19 @@ __global__ void __launch_bounds__(256) bm_paths_literal(const __grid_constant__ 
     T snap_x = x;
     long long snap_w = wraps;
     uint4 wg = make_uint4(0u, 0u, 0u, 0u);
-    for (long long n = 0; n < a.n_steps; ++n) {
+    if (a.state != nullptr && a.step_begin > 0) {  // row f2: continue a run from its checkpoint
+      const StateIO io = state_io(a, g);
+      uint32_t lo, hi;
+      x = (T)io.getd(0); wraps = (long long)io.get(1);
+      sP = (long long)io.get(2); sD = (long long)io.get(3);
+      z = (T)io.getd(4);
+      io.get2(5, kP, kD);
+      io.get2(6, lo, hi); d = (int)lo;
+      jumps = io.getd(7);
+      snap_x = (T)io.getd(8); snap_w = (long long)io.get(9);
+      if (HAS_G && (a.step_begin & 3) != 0) wg = philox_call(a.keys, g, STREAM_GAUSS, (uint32_t)(a.step_begin >> 2));
+    }
+    for (long long n = a.step_begin; n < a.step_end; ++n) {
       // Alg. 2: three-point increment with the first moments of a Gaussian of variance 2 D dt
       T dxi = (T)0;
       if (HAS_G) {
@@ -188,17 +200,28 @@ __global__ void __launch_bounds__(256) bm_paths_literal(const __grid_constant__ 
       }
       if (n + 1 == a.n_discard) { snap_x = x; snap_w = wraps; }
     }
+    if (a.state != nullptr) {  // row f2: checkpoint (a float converts to double and back exactly)
+      const StateIO io = state_io(a, g);
+      io.putd(0, (double)x); io.put(1, (unsigned long long)wraps);
+      io.put(2, (unsigned long long)sP); io.put(3, (unsigned long long)sD);
+      io.putd(4, (double)z);
+      io.put2(5, kP, kD);
+      io.put2(6, (uint32_t)d, 0u);
+      io.putd(7, jumps);
+      io.putd(8, (double)snap_x); io.put(9, (unsigned long long)snap_w);
+    }
     // a10: eq. (30)
     const double span = (double)(a.n_steps - a.n_discard) * a.dt;
     const double xT = (double)wraps * Ld + (double)x;
     const double vbar = ((double)(wraps - snap_w) * Ld + ((double)x - (double)snap_x)) / span;
-    if (a.out_paths) {
+    if (a.out_paths && a.step_end >= a.n_steps) {
       double *o = a.out_paths + g * BM_OUT_STRIDE;
       o[BM_OUT_XT] = xT; o[BM_OUT_VT] = 0.0; o[BM_OUT_VBAR] = vbar; o[BM_OUT_JUMPS] = jumps;
       o[BM_OUT_SUBSTEPS] = (double)a.n_steps; o[BM_OUT_XTI] = (double)snap_w * Ld + (double)snap_x;
     }
     mine = leaf(vbar, xT, jumps, (double)a.n_steps);
   }
+  if (a.step_end < a.n_steps) return;  // not the last chunk (uniform over the grid)
   block_reduce_store(mine, a.partials + (long long)blockIdx.x * PARTIAL_STRIDE);
 }
 
