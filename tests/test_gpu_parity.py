@@ -369,3 +369,41 @@ def test_literal_scheme_rejects_inertial(B):
     with pytest.raises(B.BmError) as e:
         B.bm_simulate(cfg, p, 1, w.n_paths, w.n_steps, w.dt, w.seed, st)
     assert e.value.status == B.BM_ERR_UNSUPPORTED
+
+
+# ---- the paper's own validation (Fig. 3) on the GPU, against the closed forms of eq. (21)-(23) ----
+
+@pytest.mark.parametrize("scheme", ["literal", "jump-adapted"])
+def test_gpu_reproduces_paper_fig3a_model_I(B, scheme):
+    """Fig. 3a: <v> vs D_P at a = 1.5, D_G = 0, 1024 paths, t_f = 1e3/lambda, spp = 400, 10 % discarded (:418-423);
+    <v> = L J_I with J_I of eq. (21a).  Both the scheme as printed and the exact-time hot path must land on it."""
+    from test_oracle_physics import J_model_I
+    a = 1.5
+    for DP in (0.5, 1.0, 2.0):
+        zeta, lam = DP / a, a * a / DP
+        n = 400_000
+        w = W.Workload("fig3a", W.OVERDAMPED, W.params_table(1, A1=1.0, D=0.0, lambda_=lam, zeta=zeta), 1024, n,
+                       (1 / lam) / 400, n // 10, potential=W.POT_PWL,
+                       scheme=W.SCHEME_PAPER_LITERAL if scheme == "literal" else W.SCHEME_JUMP_ADAPTED)
+        stats, _, _ = B.run_workload(w, B.BM_F32)
+        v_th = 2 * J_model_I(a, DP)
+        se = math.sqrt(stats[0, 2] / 1024)
+        # literal scheme: O(dt) bias of the grid-quantised kick rate (A2), a few 1e-3 at spp = 400
+        bias = 0.01 if scheme == "literal" else 0.002
+        assert abs(stats[0, 1] - v_th) < 4 * se + bias, (scheme, DP, stats[0, 1], v_th, se)
+
+
+def test_gpu_reproduces_paper_fig3b_model_II(B):
+    """Fig. 3b: <v> vs tau at F_a = 3, F_b = 1.6, spp = 200 (:425); <v> = L J_II, eq. (21b) with reading R12."""
+    from test_oracle_physics import J_model_II
+    Fa, Fb = 3.0, 1.6
+    for tau in (0.1, 0.3, 1.0):
+        mu_a, mu_b = Fa / (tau * (Fa + Fb)), Fb / (tau * (Fa + Fb))
+        n = 200_000
+        w = W.Workload("fig3b", W.OVERDAMPED, W.params_table(1, A1=1.0, D=0.0, Fa=Fa, Fb=Fb, mu_a=mu_a, mu_b=mu_b),
+                       1024, n, min(1 / mu_a, 1 / mu_b) / 200, n // 10, potential=W.POT_PWL,
+                       scheme=W.SCHEME_PAPER_LITERAL)
+        stats, _, _ = B.run_workload(w, B.BM_F32)
+        v_th = 2 * J_model_II(Fa, Fb, tau)
+        se = math.sqrt(stats[0, 2] / 1024)
+        assert abs(stats[0, 1] - v_th) < 4 * se + 0.01, (tau, stats[0, 1], v_th, se)
