@@ -65,7 +65,7 @@ struct Launch {
   int gauss = 0;    // bm_gauss selected (fp32), 0 for fp64
 };
 
-bm_status pick_kernel(const bm_config *c, int32_t n_points, int64_t n_paths, Launch *L) {
+bm_status pick_kernel(const bm_config *c, int32_t n_points, int64_t n_paths, Launch *L, bool chunked = false) {
   *L = Launch();
   if (c->scheme == BM_SCHEME_PAPER_LITERAL && c->model != BM_OVERDAMPED) return BM_ERR_UNSUPPORTED;
   if (c->model == BM_INERTIAL && c->potential != BM_POT_SINE2) return BM_ERR_UNSUPPORTED;
@@ -73,8 +73,8 @@ bm_status pick_kernel(const bm_config *c, int32_t n_points, int64_t n_paths, Lau
   if (c->scheme == BM_SCHEME_PAPER_LITERAL) {
     L->fn = pick_literal(c->prec, c->potential, c->noise);
   } else if (c->prec == BM_F64) {
-    L->fn = c->model == BM_OVERDAMPED ? pick_f64_overdamped(c->potential, c->noise)
-                                      : pick_f64_inertial(c->potential, c->noise);
+    L->fn = c->model == BM_OVERDAMPED ? pick_f64_overdamped(c->potential, c->noise, chunked)
+                                      : pick_f64_inertial(c->potential, c->noise, chunked);
   } else {
     typedef KernelFn (*Picker)(int, int);
     static const Picker table[2][2][3] = {  // [model][sincos fma][gauss - 1]
@@ -153,7 +153,7 @@ static bm_status simulate_range(const bm_config *cfg, const bm_params *params, i
   if (out_trace && (cfg->trace_steps <= 0 || cfg->trace_paths <= 0)) return BM_ERR_INVALID_ARG;
   if (out_trace && cfg->prec != BM_F64) return BM_ERR_UNSUPPORTED;
   Launch L;
-  const bm_status ps = pick_kernel(cfg, n_points, n_paths, &L);
+  const bm_status ps = pick_kernel(cfg, n_points, n_paths, &L, state != nullptr);
   if (ps != BM_OK) return ps;
   const size_t need = bm_workspace_bytes(cfg, n_points, n_paths);
   if (need == 0) return BM_ERR_INVALID_ARG;

@@ -6,8 +6,8 @@ namespace bm {
 
 typedef void (*KernelFn)(const SimArgs);
 
-KernelFn pick_f64_overdamped(int potential, int noise);
-KernelFn pick_f64_inertial(int potential, int noise);
+KernelFn pick_f64_overdamped(int potential, int noise, bool chunked);
+KernelFn pick_f64_inertial(int potential, int noise, bool chunked);
 // fp32: one family per (model, sincos, gauss) triple (BM_SINCOS_AUTO / BM_GAUSS_AUTO are resolved by the caller)
 KernelFn pick_f32_od_sfu_w16(int potential, int noise);
 KernelFn pick_f32_od_sfu_w32(int potential, int noise);

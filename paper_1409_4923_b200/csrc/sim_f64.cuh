@@ -22,6 +22,42 @@ __device__ __forceinline__ void box_muller_f64(uint32_t wa, uint32_t wb, double 
   g1 = r * s;
 }
 
+// the Gaussian call in progress at a checkpoint is recomputed, not stored (kept out of line: it runs once per launch)
+static __device__ __noinline__ void regen_gauss_block_f64(const PhiloxKeys &K, unsigned long long g, uint32_t call, double *gq) {
+  const uint4 w = philox_call(K, g, STREAM_GAUSS, call);
+  box_muller_f64(w.x, w.y, gq[0], gq[1]);
+  box_muller_f64(w.z, w.w, gq[2], gq[3]);
+}
+
+// Checkpoint record of the fp64 kernel (row f2).  Loading and storing stay out of line so that the code of the time
+// loop is the same whether or not a launch is a chunk (inlined, they cost the whole kernel 6 % on C1).
+struct CkptF64 {
+  double xi, v, rP, rD, z, jumps, sxi, sv;
+  long long wraps, swraps;
+  unsigned long long m;
+  uint32_t kP, kD;
+  int d;
+};
+static __device__ __noinline__ void ckpt_load_f64(const SimArgs &a, unsigned long long g, CkptF64 &c) {
+  const StateIO io = state_io(a, g);
+  uint32_t lo, hi;
+  c.xi = io.getd(0); c.wraps = (long long)io.get(1); c.v = io.getd(2);
+  c.rP = io.getd(3); c.rD = io.getd(4); c.z = io.getd(5);
+  io.get2(6, c.kP, c.kD);
+  io.get2(7, lo, hi); c.d = (int)lo;
+  c.m = io.get(8); c.jumps = io.getd(9);
+  c.sxi = io.getd(10); c.swraps = (long long)io.get(11); c.sv = io.getd(12);
+}
+static __device__ __noinline__ void ckpt_store_f64(const SimArgs &a, unsigned long long g, const CkptF64 &c) {
+  const StateIO io = state_io(a, g);
+  io.putd(0, c.xi); io.put(1, (unsigned long long)c.wraps); io.putd(2, c.v);
+  io.putd(3, c.rP); io.putd(4, c.rD); io.putd(5, c.z);
+  io.put2(6, c.kP, c.kD);
+  io.put2(7, (uint32_t)c.d, 0u);
+  io.put(8, c.m); io.putd(9, c.jumps);
+  io.putd(10, c.sxi); io.put(11, (unsigned long long)c.swraps); io.putd(12, c.sv);
+}
+
 struct PointF64 {
   double A1, A2, c0, D, lambda, zeta, Fa, Fb, mu_a, mu_b, gamma, amp, omega;
 };
@@ -65,7 +101,9 @@ __device__ __forceinline__ double unfolded_f64(const StateF64 &s) {
   return (double)s.wraps * period_f64<POT>() + s.xi;
 }
 
-template <int MODEL, int POT, int NOISE>
+// CHUNKED: the launch may be one chunk of a run (row f2).  A separate instantiation, because the checkpoint code in
+// the same kernel changes the register allocation of the time loop (111 -> 102 registers, 6 % slower on C1).
+template <int MODEL, int POT, int NOISE, bool CHUNKED>
 __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimArgs a) {
   constexpr bool HAS_G = NOISE & BM_NOISE_GAUSS, HAS_P = NOISE & BM_NOISE_POISSON, HAS_D = NOISE & BM_NOISE_DICH;
   constexpr bool INERTIAL = MODEL == BM_INERTIAL;
@@ -114,28 +152,24 @@ __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimA
     const bool tracing = a.out_trace != nullptr && (long long)g < a.trace_paths;
     double *trace = tracing ? a.out_trace + (long long)g * a.trace_steps * 2 : nullptr;
 
-    long long n = a.step_begin;
+    long long n = CHUNKED ? a.step_begin : 0;
     unsigned long long m = 0;
     double rem = dt, jumps = 0.0;
     double gq[4] = {0.0, 0.0, 0.0, 0.0};
     StateF64 snap = s;
-    if (a.state != nullptr && a.step_begin > 0) {  // row f2: continue a run from its checkpoint
-      const StateIO io = state_io(a, g);
-      uint32_t lo, hi;
-      s.xi = io.getd(0); s.wraps = (long long)io.get(1); s.v = io.getd(2);
-      rP = io.getd(3); rD = io.getd(4); z = io.getd(5);
-      io.get2(6, kP, kD);
-      io.get2(7, lo, hi); d = (int)lo;
-      m = io.get(8); jumps = io.getd(9);
-      snap.xi = io.getd(10); snap.wraps = (long long)io.get(11); snap.v = io.getd(12);
-      if (HAS_G && (m & 3ull) != 0) {  // the Gaussian call in progress is recomputed, not stored
-        const uint4 w = philox_call(a.keys, g, STREAM_GAUSS, (uint32_t)(m >> 2));
-        box_muller_f64(w.x, w.y, gq[0], gq[1]);
-        box_muller_f64(w.z, w.w, gq[2], gq[3]);
+    if (CHUNKED && a.state != nullptr && a.step_begin > 0) {  // row f2: continue a run from its checkpoint
+      CkptF64 c;
+      ckpt_load_f64(a, g, c);
+      s.xi = c.xi; s.wraps = c.wraps; s.v = c.v; rP = c.rP; rD = c.rD; z = c.z; kP = c.kP; kD = c.kD; d = c.d;
+      m = c.m; jumps = c.jumps; snap.xi = c.sxi; snap.wraps = c.swraps; snap.v = c.sv;
+      if (HAS_G && (m & 3ull) != 0) {
+        double t[4];
+        regen_gauss_block_f64(a.keys, g, (uint32_t)(m >> 2), t);
+        gq[0] = t[0]; gq[1] = t[1]; gq[2] = t[2]; gq[3] = t[3];
       }
     }
-    // R5: three countdown clocks; every sub-step has length h = min(rem, rP, rD)
-    while (n < a.step_end) {
+    const long long n_end = CHUNKED ? a.step_end : a.n_steps;
+    while (n < n_end) {
       double h = rem;
       if (HAS_P && onP && rP < h) h = rP;
       if (HAS_D && onD && rD < h) h = rD;
@@ -212,27 +246,24 @@ __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimA
         if (n == a.n_discard) snap = s;
       }
     }
-    if (a.state != nullptr) {  // row f2: checkpoint (chunks end on completed grid steps, so rem = dt)
-      const StateIO io = state_io(a, g);
-      io.putd(0, s.xi); io.put(1, (unsigned long long)s.wraps); io.putd(2, s.v);
-      io.putd(3, rP); io.putd(4, rD); io.putd(5, z);
-      io.put2(6, kP, kD);
-      io.put2(7, (uint32_t)d, 0u);
-      io.put(8, m); io.putd(9, jumps);
-      io.putd(10, snap.xi); io.put(11, (unsigned long long)snap.wraps); io.putd(12, snap.v);
+    if (CHUNKED && a.state != nullptr) {  // row f2: checkpoint (chunks end on completed grid steps, so rem = dt)
+      CkptF64 c;
+      c.xi = s.xi; c.wraps = s.wraps; c.v = s.v; c.rP = rP; c.rD = rD; c.z = z; c.kP = kP; c.kD = kD; c.d = d;
+      c.m = m; c.jumps = jumps; c.sxi = snap.xi; c.swraps = snap.wraps; c.sv = snap.v;
+      ckpt_store_f64(a, g, c);
     }
     // a10: eq. (30)
     const double span = (double)(a.n_steps - a.n_discard) * dt;
     const double xT = unfolded_f64<POT>(s);
     const double vbar = ((double)(s.wraps - snap.wraps) * period_f64<POT>() + (s.xi - snap.xi)) / span;
-    if (a.out_paths && a.step_end >= a.n_steps) {
+    if (a.out_paths && (!CHUNKED || a.step_end >= a.n_steps)) {
       double *o = a.out_paths + g * BM_OUT_STRIDE;
       o[BM_OUT_XT] = xT; o[BM_OUT_VT] = s.v; o[BM_OUT_VBAR] = vbar; o[BM_OUT_JUMPS] = jumps;
       o[BM_OUT_SUBSTEPS] = (double)m; o[BM_OUT_XTI] = unfolded_f64<POT>(snap);
     }
     mine = leaf(vbar, xT, jumps, (double)m);
   }
-  if (a.step_end < a.n_steps) return;  // not the last chunk: the partials are not used (uniform over the grid)
+  if (CHUNKED && a.step_end < a.n_steps) return;  // not the last chunk: the partials are not used (uniform over the grid)
   block_reduce_store(mine, a.partials + (long long)blockIdx.x * PARTIAL_STRIDE);
 }
 
