@@ -46,7 +46,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C1", choices=["C0", "C1", "C2", "C3", "C4"])
+    ap.add_argument("--workload", default="C1", choices=["C0", "C1", "C2", "C3", "C4", "M1", "M2"])
     ap.add_argument("--prec", default="f32", choices=["f32", "f64"])
     ap.add_argument("--sincos", default="auto", choices=["auto", "sfu", "fma"])
     ap.add_argument("--block-threads", type=int, default=0)
@@ -313,6 +313,8 @@ def run_ours(args):
     substeps = float(stats[:, 6].mean())                # counted by the kernel
     jumps = float(stats[:, 5].mean())
     xu_per_path = XU_OPS_PER_SUBSTEP[w.model] * substeps + 2.0 * jumps
+    if w.scheme == 1:   # the paper's scheme as printed: no Gaussian transcendental; 3 force cosines only for SINE2
+        xu_per_path = (3.0 if w.potential == 0 else 0.0) * substeps + 2.0 * jumps
     xu_ops = xu_per_path * w.n_points * w.n_paths       # algorithmic MUFU-class ops per launch (fp32 accounting)
     sm_mhz = clocks.get("sm_max_mhz") or 1965.0
     peak = XU_LANES_PER_SM * info["sm_count"] * sm_mhz * 1e6 / 1e9
@@ -323,7 +325,7 @@ def run_ours(args):
             "traffic_source": "profiles/r1_f32_v5.md (ncu --set full, dram bytes of one launch; independent of n_steps)",
             "peak_source": f"derived: {XU_LANES_PER_SM} MUFU lanes/SM/clk x {info['sm_count']} SMs x {sm_mhz:.0f} MHz "
                            "(max SM clock; lane count confirmed by bm_pipe_probe, DESIGN.md section 6)",
-            "ops_per_path_step": xu_per_path / w.n_steps, "kernel": "bm_paths_f32" if prec == B.BM_F32 else "bm_paths_f64",
+            "ops_per_path_step": xu_per_path / w.n_steps, "kernel": "bm_paths_literal" if w.scheme == 1 else ("bm_paths_f32" if prec == B.BM_F32 else "bm_paths_f64"),
             "kernel_ms": ms_per_step, "regs_per_thread": info["regs_per_thread"],
             "launch_threads": info["launch_threads"], "gauss": {1: "w32", 2: "w16", 3: "w16p"}.get(info["gauss"], "n/a"),
             "blocks_per_sm": info["blocks_per_sm"]}

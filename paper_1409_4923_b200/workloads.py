@@ -106,4 +106,22 @@ def c4():
                     4096, 20_000, 1e-3, 2_000)
 
 
-CONFIGS = {"C0": c0, "C1": c1, "C2": c2, "C3": c3, "C4": c4}
+def m1():
+    """The paper's own benchmark program `poisson` (Model I): piece-wise linear potential,
+    white Poissonian noise a = 1.5, D_P = 1, D_G = 0, scheme as printed (Alg. 1-4), spp = 400; N = 131072 paths (the
+    paper's speed-up saturates "around N = 1e5"), 4e4 steps = 100 characteristic times.  Context, not a BASELINE config."""
+    a, DP = 1.5, 1.0
+    zeta, lam = DP / a, a * a / DP
+    return Workload("M1", OVERDAMPED, params_table(1, A1=1.0, D=0.0, lambda_=lam, zeta=zeta), 131_072, 40_000,
+                    (1 / lam) / 400, 4_000, potential=POT_PWL, scheme=SCHEME_PAPER_LITERAL)
+
+
+def m2():
+    """The paper's program `dich` (Model II): dichotomous noise F_a = 3, F_b = 1.6, tau = 0.3, spp = 200."""
+    Fa, Fb, tau = 3.0, 1.6, 0.3
+    mu_a, mu_b = Fa / (tau * (Fa + Fb)), Fb / (tau * (Fa + Fb))
+    return Workload("M2", OVERDAMPED, params_table(1, A1=1.0, D=0.0, Fa=Fa, Fb=Fb, mu_a=mu_a, mu_b=mu_b), 131_072,
+                    40_000, min(1 / mu_a, 1 / mu_b) / 200, 4_000, potential=POT_PWL, scheme=SCHEME_PAPER_LITERAL)
+
+
+CONFIGS = {"C0": c0, "C1": c1, "C2": c2, "C3": c3, "C4": c4, "M1": m1, "M2": m2}
