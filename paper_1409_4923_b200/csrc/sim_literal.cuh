@@ -35,7 +35,8 @@ template <typename T, int POT>
 __device__ __forceinline__ T lit_force(T x, T A1, T A2, T F) {
   if (POT == BM_POT_SINE2) {
     if (sizeof(T) == 8) {
-      return (T)(-(2.0 * M_PI * (double)A1 * cospi(2.0 * (double)x) + 4.0 * M_PI * (double)A2 * cospi(4.0 * (double)x)) + (double)F);
+      const double c = cospi(2.0 * (double)x);  // cos 4 pi x = 2 c^2 - 1
+      return (T)(-(2.0 * M_PI * (double)A1 * c + 4.0 * M_PI * (double)A2 * fma(2.0 * c, c, -1.0)) + (double)F);
     } else {
       const float c = cos_approx(TWO_PI_F * (float)x);  // -V' = -2 pi A1 c - 4 pi A2 (2 c^2 - 1)
       return (T)fmaf(c, fmaf(-8.0f * 3.14159265358979f * (float)A2, c, -TWO_PI_F * (float)A1),
