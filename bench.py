@@ -321,11 +321,24 @@ def run_ours(args):
     if w.scheme == 1:   # the paper's scheme as printed: no Gaussian transcendental; 3 force cosines only for SINE2
         xu_per_path = (3.0 if w.potential == 0 else 0.0) * substeps + 2.0 * jumps
     xu_ops = xu_per_path * w.n_points * w.n_paths       # algorithmic MUFU-class ops per launch (fp32 accounting)
+    # the XU peak measured live with the library's probe kernel (8 independent MUFU chains per thread), beside the
+    # derived one: lane-operations per second of MUFU.COS on this device at its current clocks
+    sink = torch.zeros(info["sm_count"] * 4 * 256, dtype=torch.float32, device=dev)
+    probe_ms = []
+    for r in range(3):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        B.bm_pipe_probe(B.BM_PROBE_MUFU_COS, 1000, info["sm_count"] * 4, 256, sink)
+        e1.record()
+        e1.synchronize()
+        probe_ms.append(e0.elapsed_time(e1))
+    peak_probe = info["sm_count"] * 4 * 256 * 1000 * 64 / (min(probe_ms) * 1e-3) / 1e9
     sm_mhz = clocks.get("sm_max_mhz") or 1965.0
     peak = XU_LANES_PER_SM * info["sm_count"] * sm_mhz * 1e6 / 1e9
     achieved = xu_ops / (ms_per_step * 1e-3) / 1e9
     roof = {"bound": "alu", "pipe": "xu (MUFU) for fp32; fp64 runs the same algorithm on the FP64 pipe",
             "achieved": achieved, "peak": peak, "unit": "Gop/s", "frac": achieved / peak,
+            "peak_probe": peak_probe, "frac_of_probe": achieved / peak_probe,
             "traffic": NCU_DRAM_BYTES.get((w.name, args.prec)) if args.scale_steps == 1.0 else None,
             "traffic_source": "profiles/r1_f32_v5.md (ncu --set full, dram bytes of one launch; independent of n_steps)",
             "peak_source": f"derived: {XU_LANES_PER_SM} MUFU lanes/SM/clk x {info['sm_count']} SMs x {sm_mhz:.0f} MHz "
