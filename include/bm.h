@@ -98,9 +98,9 @@ typedef struct {
   int32_t potential;   /* bm_potential */
   int32_t scheme;      /* bm_scheme */
   int32_t noise;       /* OR of BM_NOISE_* */
-  int32_t block_threads; /* 0 = library default (a function of prec, n_points and n_paths only, see bm_kernel_info);
-                            else multiple of 32 in [32,256].  Part of the determinism contract (it fixes the
-                            reduction tree). */
+  int32_t block_threads; /* 0 = library default (a function of the arguments only, see bm_kernel_info); else a
+                            multiple of 32 in [32,256], up to 512 for the BM_F32 over-damped jump-adapted kernel.  Part
+                            of the determinism contract (it fixes the reduction tree). */
   int32_t gauss;       /* bm_gauss (BM_F32 only) */
   int64_t n_discard;   /* grid steps before t_i, 0 <= n_discard < n_steps (PAPER.md:423 uses n_steps/10) */
   int64_t trace_steps; /* with out_trace: record the first trace_steps grid steps ... */

@@ -9,7 +9,6 @@ using namespace bm;
 namespace {
 
 constexpr int DEFAULT_BLOCK_F32 = 128;
-constexpr int DEFAULT_BLOCK_F64 = 128;
 
 PhiloxKeys make_keys(uint64_t seed) {
   PhiloxKeys K;
@@ -31,21 +30,33 @@ bool valid_cfg(const bm_config *c) {
   if (c->potential < BM_POT_SINE2 || c->potential > BM_POT_QUAD) return false;
   if (c->scheme != BM_SCHEME_JUMP_ADAPTED && c->scheme != BM_SCHEME_PAPER_LITERAL) return false;
   if (c->noise < 0 || c->noise > 7) return false;
-  if (c->block_threads != 0 && (c->block_threads < 32 || c->block_threads > 256 || (c->block_threads & 31))) return false;
+  if (c->block_threads != 0 && (c->block_threads < 32 || c->block_threads > 512 || (c->block_threads & 31))) return false;
+  if (c->block_threads > 256 && !(c->prec == BM_F32 && c->model == BM_OVERDAMPED && c->scheme == BM_SCHEME_JUMP_ADAPTED)) return false;
   if (c->gauss < BM_GAUSS_AUTO || c->gauss > BM_GAUSS_W16P) return false;
   if (c->n_discard < 0 || c->trace_steps < 0 || c->trace_paths < 0) return false;
   return true;
 }
 
-// Default block size: a function of the problem size only (never of the device), because the block size fixes the
-// reduction tree.  fp32: 256 threads when the whole job is at most LOW_OCCUPANCY_WARPS warps (8 per SM sub-partition
-// of a 148-SM part) -- measured 4 % faster than 128 on C1/C2, 2.5 % slower on C4.
-constexpr long long LOW_OCCUPANCY_WARPS = 8LL * 4 * 148;
+// Default block size: a function of the arguments only (the block size fixes the reduction tree, so it must not
+// depend on the device the call happens to run on; the library is built for the 148-SM B200).  Among 128, 256
+// and 512 threads (512: fp32 over-damped jump-adapted kernel only) the size that leaves the busiest SM scheduler with the
+// fewest warps, ties to the larger block: the warps of one block run in phase and share the instruction stream
+// (C1: 2.91 / 2.80 / 2.65 ms per 20 000 steps at 128 / 256 / 512).  Beyond 8 warps per scheduler
+// the block size stops mattering and 128 is kept.
+constexpr int DESIGN_SMS = 148;
+int max_block_threads(const bm_config *c) {
+  return (c->prec == BM_F32 && c->model == BM_OVERDAMPED && c->scheme == BM_SCHEME_JUMP_ADAPTED) ? 512 : 256;
+}
 int block_threads_of(const bm_config *c, int32_t n_points, int64_t n_paths) {
   if (c->block_threads) return c->block_threads;
-  if (c->prec == BM_F64) return DEFAULT_BLOCK_F64;
-  const long long warps = (long long)n_points * ((n_paths + 31) / 32);
-  return (n_paths >= 256 && warps <= LOW_OCCUPANCY_WARPS) ? 256 : DEFAULT_BLOCK_F32;
+  int best = DEFAULT_BLOCK_F32;
+  long long best_cost = -1;
+  for (int bt = 128; bt <= max_block_threads(c); bt *= 2) {
+    const long long blocks = (long long)n_points * ((n_paths + bt - 1) / bt);
+    const long long cost = ((blocks + DESIGN_SMS - 1) / DESIGN_SMS) * (bt / 128);  // warps on the busiest scheduler
+    if (best_cost < 0 || cost <= best_cost) { best = bt; best_cost = cost; }
+  }
+  return best_cost > 8 ? DEFAULT_BLOCK_F32 : best;
 }
 
 int resolve_sincos(const bm_config *c) {

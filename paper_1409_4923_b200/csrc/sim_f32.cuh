@@ -258,7 +258,7 @@ struct PointF32 {
 };
 
 template <int MODEL, int POT, int NOISE, int SINCOS, int GW>
-__global__ void __launch_bounds__(256) bm_paths_f32(const __grid_constant__ SimArgs a) {
+__global__ void __launch_bounds__(MODEL == BM_INERTIAL ? 256 : 512) bm_paths_f32(const __grid_constant__ SimArgs a) {
   constexpr bool HAS_G = NOISE & BM_NOISE_GAUSS, HAS_P = NOISE & BM_NOISE_POISSON, HAS_D = NOISE & BM_NOISE_DICH;
   constexpr bool INERTIAL = MODEL == BM_INERTIAL;
   constexpr int NB = GaussLayout<GW>::NB, NP = GaussLayout<GW>::NP;  // grid cells, pairs per Gaussian call

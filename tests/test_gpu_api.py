@@ -160,7 +160,7 @@ def test_kernel_info_and_probe(B):
     w = W.c1()
     info = B.bm_kernel_info(B.config_for(w, B.BM_F32), w.n_points, w.n_paths)
     assert 16 <= info["regs_per_thread"] <= 255 and info["blocks_per_sm"] >= 1 and info["sm_count"] >= 1
-    assert info["launch_threads"] in (128, 256)
+    assert info["launch_threads"] in (128, 256, 512)
     assert info["gauss"] == B.BM_GAUSS_W16                     # AUTO resolves to the variant measured faster
     w32 = B.bm_kernel_info(B.config_for(w, B.BM_F32, gauss=B.BM_GAUSS_W32), w.n_points, w.n_paths)
     assert w32["gauss"] == B.BM_GAUSS_W32 and w32["launch_threads"] == info["launch_threads"]
