@@ -37,7 +37,7 @@ XU_OPS_PER_SUBSTEP = {0: 5.0, 1: 6.0}
 XU_LANES_PER_SM = 16          # MUFU lanes per SM per clock (4 per SM sub-partition); confirmed by bm_pipe_probe
 # dram__bytes_read.sum + dram__bytes_write.sum of one path-kernel launch from the committed `ncu --set full` captures
 # (profiles/r1_f32_v5.md): parameters and per-block partials only, the path is register-resident.  Bytes per launch.
-NCU_DRAM_BYTES = {("C1", "f32"): 58368, ("C2", "f32"): 37376}
+NCU_DRAM_BYTES = {("C1", "f32"): 58880, ("C2", "f32"): 37376}
 
 
 def parse():
