@@ -583,6 +583,12 @@ __global__ void __launch_bounds__(MODEL == BM_INERTIAL ? 256 : 512) bm_paths_f32
 #pragma unroll 1
         for (int j = 0; j < NB; ++j) {
           const unsigned m = ctl >> j;
+          if ((j & 1) == 0 && (m & 0x303u) == 0u) {  // a pair of cells without event or special cell
+            fast_cell(HAS_G ? s_noise[j][threadIdx.x] : 0.f, 1.0f, false);
+            fast_cell(HAS_G ? s_noise[j + 1][threadIdx.x] : 0.f, 1.0f, false);
+            ++j;
+            continue;
+          }
           if (m & 0x100u) {
             if (n + j >= n_end) break;
             fold_f32<POT>(x, wraps);  // a10: t_i
