@@ -155,6 +155,18 @@ BM_API bm_status bm_simulate_chunk(const bm_config *cfg, const bm_params *params
                             size_t workspace_bytes, void *stream);
 
 /*
+ * More observables from the same pass: the stationary density p(x mod L) of eq. (19),
+ * PAPER.md:183, as a histogram.  Adds, for every path of the checkpoint `state` (as bm_simulate_chunk left it), one
+ * count to counts[point][bin], bin = floor(n_bins * frac(x / L)): called after every chunk of a chunked run it
+ * accumulates the occupation of the reduced coordinate at the chunk boundaries t = k * chunk * dt.  Integer counts
+ * (device, uint64 [n_points][n_bins], zeroed by the caller): independent of the order of accumulation.
+ * Errors: BM_ERR_INVALID_ARG (null / misaligned pointers, n_bins outside [1, 4096]); BM_ERR_UNSUPPORTED for
+ * BM_POT_QUAD (no period); BM_ERR_WORKSPACE for a state buffer smaller than bm_state_bytes(...).
+ */
+BM_API bm_status bm_state_histogram(const bm_config *cfg, int32_t n_points, int64_t n_paths, const void *state,
+                             size_t state_bytes, int32_t n_bins, uint64_t *counts, void *stream);
+
+/*
  * HOST-pointer convenience entry (the end-to-end path): params, out_stats and out_paths (optional) are HOST
  * buffers.  Takes device scratch from a private stream-ordered pool (one per device, kept between calls: an
  * allocation cache with no influence on results), copies params in, runs bm_simulate on `stream`, copies the

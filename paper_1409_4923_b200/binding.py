@@ -26,7 +26,7 @@ BM_OUT_XT, BM_OUT_VT, BM_OUT_VBAR, BM_OUT_JUMPS, BM_OUT_SUBSTEPS, BM_OUT_XTI, BM
  BM_PROBE_DFMA, BM_PROBE_I2F, BM_PROBE_FADD, BM_PROBE_MIX, BM_PROBE_COUNT) = range(11)
 
 BM_STATE_SLOTS, BM_CHUNK_ALIGN = 16, 8
-EXPORTS = ("bm_workspace_bytes", "bm_simulate", "bm_state_bytes", "bm_simulate_chunk", "bm_simulate_host", "bm_philox_fill", "bm_gauss_fill",
+EXPORTS = ("bm_workspace_bytes", "bm_simulate", "bm_state_bytes", "bm_simulate_chunk", "bm_state_histogram", "bm_simulate_host", "bm_philox_fill", "bm_gauss_fill",
            "bm_kernel_info", "bm_pipe_probe", "bm_status_string", "bm_version")
 STATS_FIELDS = ("n", "mean_v", "var_v", "mean_xT", "var_xT", "mean_jumps", "mean_substeps", "rsv")
 
@@ -64,6 +64,8 @@ def lib():
         L.bm_state_bytes.restype = C.c_size_t
         L.bm_simulate_chunk.argtypes = [cfgp, vp, i32, i64, i64, dbl, u64, i64, i64, vp, C.c_size_t, vp, vp, vp, C.c_size_t, vp]
         L.bm_simulate_chunk.restype = C.c_int
+        L.bm_state_histogram.argtypes = [cfgp, i32, i64, vp, C.c_size_t, i32, vp, vp]
+        L.bm_state_histogram.restype = C.c_int
         L.bm_simulate_host.argtypes = [cfgp, vp, i32, i64, i64, dbl, u64, vp, vp, vp]
         L.bm_simulate_host.restype = C.c_int
         L.bm_philox_fill.argtypes = [u64, u64, i32, u32, u32, i32, vp, vp]
@@ -169,6 +171,17 @@ def bm_simulate_chunk(cfg, params, n_points, n_paths, n_steps, dt, seed, step_be
     if rc != BM_OK:
         raise BmError(rc, "bm_simulate_chunk")
     return workspace
+
+
+def bm_state_histogram(cfg, n_points, n_paths, state, n_bins, counts, stream=None):
+    """counts (CUDA int64 tensor [n_points, n_bins]) += occupation of the reduced coordinate in the checkpoint `state`."""
+    import torch
+    assert state.is_cuda and state.dtype == torch.uint8
+    assert counts.is_cuda and counts.dtype == torch.int64 and counts.is_contiguous() and counts.numel() == n_points * n_bins
+    rc = lib().bm_state_histogram(C.byref(cfg), n_points, n_paths, C.c_void_p(state.data_ptr()), state.numel(), n_bins,
+                                  C.c_void_p(counts.data_ptr()), _stream_ptr(stream))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_state_histogram")
 
 
 def bm_simulate_host(cfg, params, n_points, n_paths, n_steps, dt, seed, out_stats, out_paths=None, stream=None):

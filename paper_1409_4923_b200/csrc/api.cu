@@ -225,6 +225,21 @@ BM_API bm_status bm_simulate_chunk(const bm_config *cfg, const bm_params *params
                         out_paths, nullptr, workspace, workspace_bytes, stream);
 }
 
+BM_API bm_status bm_state_histogram(const bm_config *cfg, int32_t n_points, int64_t n_paths, const void *state,
+                             size_t state_bytes, int32_t n_bins, uint64_t *counts, void *stream) {
+  if (!valid_cfg(cfg) || n_points <= 0 || n_paths <= 0 || !state || !counts || n_bins <= 0 || n_bins > 4096) return BM_ERR_INVALID_ARG;
+  if (((uintptr_t)state & 15) || ((uintptr_t)counts & 7)) return BM_ERR_INVALID_ARG;
+  if (cfg->potential == BM_POT_QUAD) return BM_ERR_UNSUPPORTED;  // no period to fold into
+  const size_t need = bm_state_bytes(cfg, n_points, n_paths);
+  if (need == 0 || state_bytes < need) return BM_ERR_WORKSPACE;
+  const double period = cfg->potential == BM_POT_SINE2 ? 1.0 : 2.0;
+  const bool theta = cfg->prec == BM_F32 && cfg->scheme == BM_SCHEME_JUMP_ADAPTED;   // position kept as scale * x
+  const double scale = (theta && cfg->potential == BM_POT_SINE2) ? 6.283185307179586 : 1.0;
+  return launch_state_hist(reinterpret_cast<const unsigned long long *>(state), n_points, n_paths, theta ? 0 : 1,
+                           1.0 / (period * scale), n_bins, reinterpret_cast<unsigned long long *>(counts),
+                           reinterpret_cast<cudaStream_t>(stream)) == cudaSuccess ? BM_OK : BM_ERR_CUDA;
+}
+
 BM_API bm_status bm_simulate_host(const bm_config *cfg, const bm_params *params, int32_t n_points, int64_t n_paths,
                            int64_t n_steps, double dt, uint64_t seed, bm_stats *out_stats, double *out_paths,
                            void *stream) {

@@ -32,6 +32,8 @@ cudaError_t launch_gauss_fill(int prec, int gauss, const PhiloxKeys &K, unsigned
                               unsigned long long m0, int n_m, void *out, cudaStream_t st);
 cudaError_t launch_grid_reduce(const double *partials, int n_points, int blocks_per_point, bm_stats *out,
                                cudaStream_t st);
+cudaError_t launch_state_hist(const unsigned long long *state, int n_points, long long n_paths, int kind, double inv_period,
+                              int n_bins, unsigned long long *counts, cudaStream_t st);
 cudaError_t launch_probe(int op, int iters, int blocks, int threads, float *sink, cudaStream_t st);
 
 }  // namespace bm

@@ -98,6 +98,41 @@ __global__ void grid_reduce_kernel(const double *__restrict__ partials, int n_po
   }
 }
 
+// Row f3: histogram of the folded positions held in a checkpoint (the state of bm_simulate_chunk), one block-private
+// histogram in shared memory, integer atomics only (the counts do not depend on the order of the additions).
+// kind 0: fp32 jump-adapted kernel (slot 0 low word = theta as float, theta = scale * x);  kind 1: fp64 kernel and
+// both literal kernels (slot 0 = position as double).  u = position / period, reduced to [0, 1).
+__global__ void state_hist_kernel(const unsigned long long *__restrict__ state, long long n_paths, int blocks_per_point,
+                                  int kind, double inv_period, int n_bins, unsigned long long *__restrict__ counts) {
+  extern __shared__ unsigned int sh[];
+  for (int i = threadIdx.x; i < n_bins; i += blockDim.x) sh[i] = 0u;
+  __syncthreads();
+  const int point = blockIdx.x / blocks_per_point;
+  const long long p = (long long)(blockIdx.x - point * blocks_per_point) * blockDim.x + threadIdx.x;
+  if (p < n_paths) {
+    const unsigned long long v = __ldcg(state + (long long)point * n_paths + p);  // slot 0
+    const double pos = kind == 0 ? (double)__uint_as_float((uint32_t)v) : __longlong_as_double((long long)v);
+    double u = pos * inv_period;
+    u -= floor(u);
+    int b = (int)(u * (double)n_bins);
+    b = b < 0 ? 0 : (b >= n_bins ? n_bins - 1 : b);
+    atomicAdd(&sh[b], 1u);
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < n_bins; i += blockDim.x)
+    if (sh[i]) atomicAdd(counts + (long long)point * n_bins + i, (unsigned long long)sh[i]);
+}
+
+cudaError_t launch_state_hist(const unsigned long long *state, int n_points, long long n_paths, int kind, double inv_period,
+                              int n_bins, unsigned long long *counts, cudaStream_t st) {
+  const int threads = 256;
+  const long long bpp = (n_paths + threads - 1) / threads;
+  if (bpp * n_points > 0x7FFFFFFFLL) return cudaErrorInvalidValue;
+  state_hist_kernel<<<(unsigned)(bpp * n_points), threads, (size_t)n_bins * sizeof(unsigned int), st>>>(
+      state, n_paths, (int)bpp, kind, inv_period, n_bins, counts);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_grid_reduce(const double *partials, int n_points, int blocks_per_point, bm_stats *out,
                                cudaStream_t st) {
   const int threads = 128;  // 4 points per block
