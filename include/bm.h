@@ -132,6 +132,16 @@ BM_API bm_status bm_simulate(const bm_config *cfg, const bm_params *params, int3
                       double *out_trace, void *workspace, size_t workspace_bytes, void *stream);
 
 /*
+ * bm_simulate with one step length per parameter point ("per-point dt"; the paper fixes the step
+ * as a number of steps per characteristic time, dt = tau_char / spp, so a sweep over the noise parameters
+ * is a sweep over dt).  dt_points [n_points] device, read only, each > 0 (not checked on the device: a non-positive
+ * entry gives NaN statistics for that point).  Everything else as bm_simulate; no trace output.
+ */
+BM_API bm_status bm_simulate_dt(const bm_config *cfg, const bm_params *params, const double *dt_points, int32_t n_points,
+                         int64_t n_paths, int64_t n_steps, uint64_t seed, bm_stats *out_stats, double *out_paths,
+                         void *workspace, size_t workspace_bytes, void *stream);
+
+/*
  * Chunked runs and checkpoint / resume (Alg. 5 steps 2 and 6: "load the state
  * ... advance `samples` steps ... save the state").  bm_simulate_chunk performs grid steps
  * [step_begin, step_begin + step_count) of a run of n_steps steps.  step_begin == 0 initialises the paths (the

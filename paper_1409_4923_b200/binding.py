@@ -26,7 +26,7 @@ BM_OUT_XT, BM_OUT_VT, BM_OUT_VBAR, BM_OUT_JUMPS, BM_OUT_SUBSTEPS, BM_OUT_XTI, BM
  BM_PROBE_DFMA, BM_PROBE_I2F, BM_PROBE_FADD, BM_PROBE_MIX, BM_PROBE_COUNT) = range(11)
 
 BM_STATE_SLOTS, BM_CHUNK_ALIGN = 16, 8
-EXPORTS = ("bm_workspace_bytes", "bm_simulate", "bm_state_bytes", "bm_simulate_chunk", "bm_state_histogram", "bm_simulate_host", "bm_philox_fill", "bm_gauss_fill",
+EXPORTS = ("bm_workspace_bytes", "bm_simulate", "bm_simulate_dt", "bm_state_bytes", "bm_simulate_chunk", "bm_state_histogram", "bm_simulate_host", "bm_philox_fill", "bm_gauss_fill",
            "bm_kernel_info", "bm_pipe_probe", "bm_status_string", "bm_version")
 STATS_FIELDS = ("n", "mean_v", "var_v", "mean_xT", "var_xT", "mean_jumps", "mean_substeps", "rsv")
 
@@ -60,6 +60,8 @@ def lib():
         L.bm_workspace_bytes.restype = C.c_size_t
         L.bm_simulate.argtypes = [cfgp, vp, i32, i64, i64, dbl, u64, vp, vp, vp, vp, C.c_size_t, vp]
         L.bm_simulate.restype = C.c_int
+        L.bm_simulate_dt.argtypes = [cfgp, vp, vp, i32, i64, i64, u64, vp, vp, vp, C.c_size_t, vp]
+        L.bm_simulate_dt.restype = C.c_int
         L.bm_state_bytes.argtypes = [cfgp, i32, i64]
         L.bm_state_bytes.restype = C.c_size_t
         L.bm_simulate_chunk.argtypes = [cfgp, vp, i32, i64, i64, dbl, u64, i64, i64, vp, C.c_size_t, vp, vp, vp, C.c_size_t, vp]
@@ -146,6 +148,24 @@ def bm_simulate(cfg, params, n_points, n_paths, n_steps, dt, seed, out_stats, ou
                            workspace.numel(), _stream_ptr(stream))
     if rc != BM_OK:
         raise BmError(rc, "bm_simulate")
+    return workspace
+
+
+def bm_simulate_dt(cfg, params, dt_points, n_points, n_paths, n_steps, seed, out_stats, out_paths=None, workspace=None,
+                   stream=None):
+    """bm_simulate with one step length per parameter point (dt_points: CUDA float64 tensor [n_points])."""
+    import torch
+    assert params.is_cuda and params.dtype == torch.float64 and params.numel() == 16 * n_points
+    assert dt_points.is_cuda and dt_points.dtype == torch.float64 and dt_points.is_contiguous() and dt_points.numel() == n_points
+    assert out_stats.is_cuda and out_stats.dtype == torch.float64 and out_stats.numel() == 8 * n_points
+    if workspace is None:
+        workspace = torch.empty(max(bm_workspace_bytes(cfg, n_points, n_paths), 16), dtype=torch.uint8, device=params.device)
+    op = C.c_void_p(out_paths.data_ptr()) if out_paths is not None else None
+    rc = lib().bm_simulate_dt(C.byref(cfg), C.c_void_p(params.data_ptr()), C.c_void_p(dt_points.data_ptr()), n_points,
+                              n_paths, n_steps, int(seed), C.c_void_p(out_stats.data_ptr()), op,
+                              C.c_void_p(workspace.data_ptr()), workspace.numel(), _stream_ptr(stream))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_simulate_dt")
     return workspace
 
 

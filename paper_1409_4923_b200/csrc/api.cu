@@ -154,7 +154,8 @@ BM_API size_t bm_workspace_bytes(const bm_config *cfg, int32_t n_points, int64_t
 
 // the launch behind bm_simulate (state == nullptr: the whole run) and bm_simulate_chunk
 static bm_status simulate_range(const bm_config *cfg, const bm_params *params, int32_t n_points, int64_t n_paths,
-                                int64_t n_steps, double dt, uint64_t seed, int64_t step_begin, int64_t step_end,
+                                int64_t n_steps, double dt, const double *dt_points, uint64_t seed, int64_t step_begin,
+                                int64_t step_end,
                                 void *state, bm_stats *out_stats, double *out_paths, double *out_trace, void *workspace,
                                 size_t workspace_bytes, void *stream) {
   if (!valid_cfg(cfg) || !params || !out_stats || n_points <= 0 || n_paths <= 0 || n_steps <= 0) return BM_ERR_INVALID_ARG;
@@ -182,6 +183,7 @@ static bm_status simulate_range(const bm_config *cfg, const bm_params *params, i
   a.trace_steps = out_trace ? cfg->trace_steps : 0;
   a.trace_paths = out_trace ? cfg->trace_paths : 0;
   a.dt = dt;
+  a.dt_points = dt_points;
   a.n_points = n_points;
   a.blocks_per_point = (int)blocks_per_point_of(cfg, n_points, n_paths);
   a.state = reinterpret_cast<unsigned long long *>(state);
@@ -201,8 +203,17 @@ static bm_status simulate_range(const bm_config *cfg, const bm_params *params, i
 BM_API bm_status bm_simulate(const bm_config *cfg, const bm_params *params, int32_t n_points, int64_t n_paths,
                       int64_t n_steps, double dt, uint64_t seed, bm_stats *out_stats, double *out_paths,
                       double *out_trace, void *workspace, size_t workspace_bytes, void *stream) {
-  return simulate_range(cfg, params, n_points, n_paths, n_steps, dt, seed, 0, n_steps, nullptr, out_stats, out_paths,
-                        out_trace, workspace, workspace_bytes, stream);
+  return simulate_range(cfg, params, n_points, n_paths, n_steps, dt, nullptr, seed, 0, n_steps, nullptr, out_stats,
+                        out_paths, out_trace, workspace, workspace_bytes, stream);
+}
+
+BM_API bm_status bm_simulate_dt(const bm_config *cfg, const bm_params *params, const double *dt_points, int32_t n_points,
+                         int64_t n_paths, int64_t n_steps, uint64_t seed, bm_stats *out_stats, double *out_paths,
+                         void *workspace, size_t workspace_bytes, void *stream) {
+  if (!dt_points || ((uintptr_t)dt_points & 7)) return BM_ERR_INVALID_ARG;
+  // dt = 1 passes the scalar checks; every kernel reads its step length from dt_points[point]
+  return simulate_range(cfg, params, n_points, n_paths, n_steps, 1.0, dt_points, seed, 0, n_steps, nullptr, out_stats,
+                        out_paths, nullptr, workspace, workspace_bytes, stream);
 }
 
 BM_API size_t bm_state_bytes(const bm_config *cfg, int32_t n_points, int64_t n_paths) {
@@ -221,7 +232,7 @@ BM_API bm_status bm_simulate_chunk(const bm_config *cfg, const bm_params *params
   if (!state || ((uintptr_t)state & 15)) return BM_ERR_INVALID_ARG;
   const size_t need = bm_state_bytes(cfg, n_points, n_paths);
   if (need == 0 || state_bytes < need) return BM_ERR_WORKSPACE;
-  return simulate_range(cfg, params, n_points, n_paths, n_steps, dt, seed, step_begin, step_end, state, out_stats,
+  return simulate_range(cfg, params, n_points, n_paths, n_steps, dt, nullptr, seed, step_begin, step_end, state, out_stats,
                         out_paths, nullptr, workspace, workspace_bytes, stream);
 }
 

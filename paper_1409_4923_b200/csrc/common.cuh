@@ -29,6 +29,7 @@ struct SimArgs {
   long long trace_steps;
   long long trace_paths;
   double dt;
+  const double *dt_points;  // optional [n_points]: per-point step length (overrides dt); nullptr = one dt for all
   int n_points;
   int blocks_per_point;
   // chunked runs (row f2): this launch does grid steps [step_begin, step_end) of a run of n_steps.  state == nullptr:
@@ -51,6 +52,11 @@ struct StateIO {
   __device__ __forceinline__ void putd(int slot, double v) const { put(slot, (unsigned long long)__double_as_longlong(v)); }
   __device__ __forceinline__ double getd(int slot) const { return __longlong_as_double((long long)get(slot)); }
 };
+// step length of a parameter point
+__device__ __forceinline__ double step_length(const SimArgs &a, int point) {
+  const double *src = a.dt_points ? a.dt_points + point : &a.dt;  // &a.dt: the kernel parameter itself
+  return *src;
+}
 __device__ __forceinline__ StateIO state_io(const SimArgs &a, unsigned long long g) {
   return StateIO{a.state + g, (long long)a.n_points * a.n_paths};
 }

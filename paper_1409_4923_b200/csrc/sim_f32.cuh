@@ -276,8 +276,9 @@ __global__ void __launch_bounds__(MODEL == BM_INERTIAL ? 256 : 512) bm_paths_f32
   const PhiloxKeys &K = a.keys;
   const bm_params bp = a.params[point];
   const double Dd = HAS_G ? bp.D : 0.0;
-  const float dt = (float)a.dt;
-  const float inv_dt = (float)(1.0 / a.dt);
+  const double dtd = step_length(a, point);
+  const float dt = (float)dtd;
+  const float inv_dt = (float)(1.0 / dtd);
   const double lam = HAS_P ? bp.lambda : 0.0, zet = HAS_P ? bp.zeta : 0.0;
   PointF32 P;
   if (POT == BM_POT_SINE2) {
@@ -292,11 +293,11 @@ __global__ void __launch_bounds__(MODEL == BM_INERTIAL ? 256 : 512) bm_paths_f32
   }
   P.Ga = (float)((double)S * (-bp.Fa));
   P.Gb = (float)((double)S * bp.Fb);
-  P.cn = (float)(-2.0 * M_LN2 * (double)S * (double)S * 2.0 * Dd * a.dt);
-  P.inv_lam_dt = (lam > 0.0) ? (float)(1.0 / (lam * a.dt)) : 0.f;
+  P.cn = (float)(-2.0 * M_LN2 * (double)S * (double)S * 2.0 * Dd * dtd);
+  P.inv_lam_dt = (lam > 0.0) ? (float)(1.0 / (lam * dtd)) : 0.f;
   P.zeta = (float)((double)S * zet);
-  P.inv_mua_dt = (HAS_D && bp.mu_a > 0.0) ? (float)(1.0 / (bp.mu_a * a.dt)) : 0.f;
-  P.inv_mub_dt = (HAS_D && bp.mu_b > 0.0) ? (float)(1.0 / (bp.mu_b * a.dt)) : 0.f;
+  P.inv_mua_dt = (HAS_D && bp.mu_a > 0.0) ? (float)(1.0 / (bp.mu_a * dtd)) : 0.f;
+  P.inv_mub_dt = (HAS_D && bp.mu_b > 0.0) ? (float)(1.0 / (bp.mu_b * dtd)) : 0.f;
   P.gamma = (float)bp.gamma;
   P.amp = (float)((double)S * bp.amp);
   P.w_turns = (float)(bp.omega / (2.0 * M_PI));
@@ -346,7 +347,7 @@ __global__ void __launch_bounds__(MODEL == BM_INERTIAL ? 256 : 512) bm_paths_f32
   unsigned long long ph = 0, dph = 0;
   float drive0 = 0.f;  // SCALE * amp * cos(omega n dt)
   if (INERTIAL) {
-    double turns_per_cell = bp.omega * a.dt / (2.0 * M_PI);
+    double turns_per_cell = bp.omega * dtd / (2.0 * M_PI);
     turns_per_cell -= floor(turns_per_cell);
     dph = (unsigned long long)(turns_per_cell * 18446744073709551616.0);
     drive0 = P.amp;  // cos(0)
@@ -628,7 +629,7 @@ __global__ void __launch_bounds__(MODEL == BM_INERTIAL ? 256 : 512) bm_paths_f32
     // a10: eq. (30), assembled once per path in fp64
     fold_f32<POT>(x, wraps);
     const double Ld = Units<POT>::PERIOD_X, iS = 1.0 / (double)S;
-    const double span = (double)(a.n_steps - a.n_discard) * a.dt;
+    const double span = (double)(a.n_steps - a.n_discard) * dtd;
     const double xT = (double)wraps * Ld + (double)x * iS;
     const double xTi = (double)snap_w * Ld + (double)snap_x * iS;
     const double vbar = ((double)(wraps - snap_w) * Ld + ((double)x - (double)snap_x) * iS) / span;

@@ -121,7 +121,7 @@ __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimA
     P.Fa = bp.Fa; P.Fb = bp.Fb; P.mu_a = bp.mu_a; P.mu_b = bp.mu_b;
     P.gamma = bp.gamma; P.amp = bp.amp; P.omega = bp.omega;
     P.c0 = bp.F - P.lambda * P.zeta;  // constant part of the drift a(x), all three stages (R6)
-    const double dt = a.dt;
+    const double dt = step_length(a, point);
     const double L0 = (POT == BM_POT_QUAD) ? 1.0 : period_f64<POT>();
 
     // R4: initial condition from init-stream call 0

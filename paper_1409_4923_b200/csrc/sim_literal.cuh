@@ -72,12 +72,13 @@ __global__ void __launch_bounds__(256) bm_paths_literal(const __grid_constant__ 
     const bm_params bp = a.params[point];
     const double Ld = POT == BM_POT_SINE2 ? 1.0 : (POT == BM_POT_PWL ? 2.0 : 0.0);
     const double L0 = (POT == BM_POT_QUAD) ? 1.0 : Ld;
-    const T A1 = (T)bp.A1, A2 = (T)bp.A2, F = (T)bp.F, dt = (T)a.dt;
-    const T inv_dt = (T)(1.0 / a.dt);
+    const double dtd = step_length(a, point);
+    const T A1 = (T)bp.A1, A2 = (T)bp.A2, F = (T)bp.F, dt = (T)dtd;
+    const T inv_dt = (T)(1.0 / dtd);
     const double lam = HAS_P ? bp.lambda : 0.0, zet = HAS_P ? bp.zeta : 0.0;
     const bool onP = HAS_P && lam > 0.0;
-    const T a_dt = (T)(lam * zet * a.dt);  // a dt, eq. (6): the bias -lambda zeta of the shot noise over one step
-    const T step3 = HAS_G ? (T)(sqrt(2.0 * bp.D) * sqrt(3.0 * a.dt)) : (T)0;  // G sqrt(3 dt), Alg. 2
+    const T a_dt = (T)(lam * zet * dtd);  // a dt, eq. (6): the bias -lambda zeta of the shot noise over one step
+    const T step3 = HAS_G ? (T)(sqrt(2.0 * bp.D) * sqrt(3.0 * dtd)) : (T)0;  // G sqrt(3 dt), Alg. 2
 
     // R4: initial condition (same init-stream call as the jump-adapted kernels)
     const uint4 wi = philox_call(a.keys, g, STREAM_INIT, 0);
@@ -212,7 +213,7 @@ __global__ void __launch_bounds__(256) bm_paths_literal(const __grid_constant__ 
       io.putd(8, (double)snap_x); io.put(9, (unsigned long long)snap_w);
     }
     // a10: eq. (30)
-    const double span = (double)(a.n_steps - a.n_discard) * a.dt;
+    const double span = (double)(a.n_steps - a.n_discard) * dtd;
     const double xT = (double)wraps * Ld + (double)x;
     const double vbar = ((double)(wraps - snap_w) * Ld + ((double)x - (double)snap_x)) / span;
     if (a.out_paths && a.step_end >= a.n_steps) {

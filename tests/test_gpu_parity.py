@@ -407,3 +407,59 @@ def test_gpu_reproduces_paper_fig3b_model_II(B):
         v_th = 2 * J_model_II(Fa, Fb, tau)
         se = math.sqrt(stats[0, 2] / 1024)
         assert abs(stats[0, 1] - v_th) < 4 * se + 0.01, (tau, stats[0, 1], v_th, se)
+
+
+# ---- per-point step length (row f2): a sweep over noise parameters at fixed steps per characteristic time --------
+
+def test_per_point_dt_sweep_matches_oracle_and_fig3a(B, orc):
+    """Fig. 3a in ONE launch: three values of D_P at a = 1.5, each with its own dt = (1/lambda)/400.
+    fp64 per path against the oracle (run point by point with that point's dt and the same global path ids), the
+    ensemble against eq. (21a); fp32 within 3 combined standard errors."""
+    import torch
+    from test_oracle_physics import J_model_I
+    a, DPs = 1.5, np.array([0.5, 1.0, 2.0])
+    lam, zeta = a * a / DPs, DPs / a
+    params = W.params_table(3, A1=1.0, D=0.0, lambda_=lam, zeta=zeta)
+    dts = (1.0 / lam) / 400
+    n_paths, n_steps, nd = 512, 40_000, 4_000
+    dev = torch.device("cuda:0")
+    res = {}
+    for prec in (B.BM_F64, B.BM_F32):
+        cfg = B.make_config(prec=prec, potential=B.BM_POT_PWL, scheme=B.BM_SCHEME_PAPER_LITERAL, noise=B.BM_NOISE_POISSON,
+                            n_discard=nd)
+        st = torch.zeros((3, 8), dtype=torch.float64, device=dev)
+        pa = torch.zeros((3 * n_paths, B.BM_OUT_STRIDE), dtype=torch.float64, device=dev)
+        B.bm_simulate_dt(cfg, torch.from_numpy(params).to(dev), torch.from_numpy(dts).to(dev), 3, n_paths, n_steps, W.SEED, st, pa)
+        torch.cuda.synchronize()
+        res[prec] = (st.cpu().numpy(), pa.cpu().numpy())
+    for pt in range(3):
+        ids = pt * n_paths + np.arange(n_paths)
+        ref, _ = orc.simulate(params, n_paths, n_steps, float(dts[pt]), W.SEED, potential=orc.POT_PWL,
+                              scheme=orc.SCHEME_PAPER_LITERAL, n_discard=nd, ids=ids)
+        s64, p64 = res[B.BM_F64]
+        got = p64[ids]
+        assert np.array_equal(got[:, B.BM_OUT_JUMPS], ref[:, orc.OUT_JUMPS])
+        dx = np.abs(got[:, B.BM_OUT_XT] - ref[:, orc.OUT_XT])
+        assert (dx > 1e-8 * (1 + np.abs(ref[:, orc.OUT_XT]))).sum() <= 4, f"point {pt}: max {dx.max():.3e}"
+        v_th = 2 * J_model_I(a, float(DPs[pt]))
+        se = math.sqrt(s64[pt, 2] / n_paths)
+        assert abs(s64[pt, 1] - v_th) < 4 * se + 0.01, (pt, s64[pt, 1], v_th)
+        _, p32 = res[B.BM_F32]
+        assert_3se(p32[ids], ref, B.BM_OUT_VBAR, f"per-point dt, fp32, point {pt}")
+
+
+def test_per_point_dt_equal_entries_reproduce_scalar_dt(B):
+    """dt_points all equal to dt must give bit-identical results to bm_simulate(dt) for both hot-path kernels."""
+    import torch
+    for w, prec in ((W.c4().scaled(n_paths=64, n_steps=400, points=[3, 9000, 16383]), B.BM_F32),
+                    (W.c3().scaled(n_paths=64, n_steps=240, points=[0, 200]), B.BM_F64)):
+        s0, p0, _ = B.run_workload(w, prec, want_paths=True)
+        cfg = B.config_for(w, prec)
+        dev = torch.device("cuda:0")
+        st = torch.zeros((w.n_points, 8), dtype=torch.float64, device=dev)
+        pa = torch.zeros((w.n_points * w.n_paths, B.BM_OUT_STRIDE), dtype=torch.float64, device=dev)
+        B.bm_simulate_dt(cfg, torch.from_numpy(np.ascontiguousarray(w.params)).to(dev),
+                         torch.full((w.n_points,), w.dt, dtype=torch.float64, device=dev), w.n_points, w.n_paths, w.n_steps,
+                         w.seed, st, pa)
+        torch.cuda.synchronize()
+        assert np.array_equal(st.cpu().numpy(), s0) and np.array_equal(pa.cpu().numpy(), p0)
