@@ -11,6 +11,8 @@
 // (w <= 715827882, w <= 1431655764: the same sets as the comparisons of u(w) = (w + 1/2) 2^-32 with 1/6 and 1/3),
 // so both precisions and the oracle decide identically.
 #pragma once
+#include <type_traits>
+
 #include "sim_f32.cuh"
 #include "sim_f64.cuh"
 
@@ -62,6 +64,10 @@ __global__ void __launch_bounds__(256) bm_paths_literal(const __grid_constant__ 
   constexpr bool HAS_G = NOISE & BM_NOISE_GAUSS, HAS_P = NOISE & BM_NOISE_POISSON, HAS_D = NOISE & BM_NOISE_DICH;
   constexpr bool F64 = sizeof(T) == 8;
   typedef LitMath<T> M;
+  // step counters, countdowns and wrap counts: 32-bit in the fp32 kernel (n_steps < 2^31 there; a countdown beyond the
+  // run saturates, which is the same as never firing), 64-bit in the fp64 kernel
+  typedef typename std::conditional<F64, long long, int>::type Count;
+  constexpr Count COUNT_MAX = F64 ? (Count)0x7FFFFFFFFFFFFFFFLL : (Count)0x7FFFFFFF;
   const int point = blockIdx.x / a.blocks_per_point;
   const int chunk = blockIdx.x - point * a.blocks_per_point;
   const long long p = (long long)chunk * blockDim.x + threadIdx.x;
@@ -83,25 +89,25 @@ __global__ void __launch_bounds__(256) bm_paths_literal(const __grid_constant__ 
     // R4: initial condition (same init-stream call as the jump-adapted kernels)
     const uint4 wi = philox_call(a.keys, g, STREAM_INIT, 0);
     double x0 = (bp.x0_fixed >= 0.0) ? bp.x0_fixed : L0 * ((double)wi.x * (1.0 / 4294967296.0));
-    long long wraps = 0;
+    Count wraps = 0;
     if (POT != BM_POT_QUAD) {  // fp64: [0, L) as the oracle; fp32: [-L/2, L/2) (round-to-nearest fold)
       const double k = F64 ? floor(x0 / L0) : rint(x0 / L0);
       x0 -= k * Ld;
-      wraps = (long long)k;
+      wraps = (Count)k;
     }
     T x = (T)x0;
     int d = HAS_D ? ((u01_f64(wi.z) < bp.mu_a / (bp.mu_a + bp.mu_b)) ? 1 : 0) : 0;
 
     // countdowns in grid steps (integers: exact in both precisions)
-    long long sP = 0, sD = 0;
+    Count sP = 0, sD = 0;
     T z = (T)0;
     uint32_t kP = 0, kD = 0;
     const T inv_lam = onP ? (T)(1.0 / lam) : (T)0, zeta = (T)zet;
     const T inv_mua = (HAS_D && bp.mu_a > 0.0) ? (T)(1.0 / bp.mu_a) : (T)0;
     const T inv_mub = (HAS_D && bp.mu_b > 0.0) ? (T)(1.0 / bp.mu_b) : (T)0;
-    auto to_steps = [&](T wait) -> long long {  // [wait / dt], Alg. 3 line 5 / Alg. 4
+    auto to_steps = [&](T wait) -> Count {  // [wait / dt], Alg. 3 line 5 / Alg. 4
       const T q = M::floor_(F64 ? wait / dt : wait * inv_dt);
-      return q < (T)9.0e18 ? (long long)q : 0x7FFFFFFFFFFFFFFFLL;
+      return q < (F64 ? (T)9.0e18 : (T)2.0e9) ? (Count)q : COUNT_MAX;
     };
     if (onP) {
       const uint4 w = philox_call(a.keys, g, STREAM_POISSON, 0);
@@ -122,7 +128,7 @@ __global__ void __launch_bounds__(256) bm_paths_literal(const __grid_constant__ 
         const double k = floor((double)x / L0);
         if (k != 0.0) {
           double xx = (double)x - k * Ld;
-          wraps += (long long)k;
+          wraps += (Count)k;
           if (xx < 0.0) { xx += Ld; wraps -= 1; }
           if (xx >= Ld) { xx -= Ld; wraps += 1; }
           x = (T)xx;
@@ -134,23 +140,24 @@ __global__ void __launch_bounds__(256) bm_paths_literal(const __grid_constant__ 
       }
     };
 
-    double jumps = 0.0;
+    Count jumps = 0;
     T snap_x = x;
-    long long snap_w = wraps;
+    Count snap_w = wraps;
     uint4 wg = make_uint4(0u, 0u, 0u, 0u);
     if (a.state != nullptr && a.step_begin > 0) {  // row f2: continue a run from its checkpoint
       const StateIO io = state_io(a, g);
       uint32_t lo, hi;
-      x = (T)io.getd(0); wraps = (long long)io.get(1);
-      sP = (long long)io.get(2); sD = (long long)io.get(3);
+      x = (T)io.getd(0); wraps = (Count)(long long)io.get(1);
+      sP = (Count)(long long)io.get(2); sD = (Count)(long long)io.get(3);
       z = (T)io.getd(4);
       io.get2(5, kP, kD);
       io.get2(6, lo, hi); d = (int)lo;
-      jumps = io.getd(7);
-      snap_x = (T)io.getd(8); snap_w = (long long)io.get(9);
+      jumps = (Count)io.getd(7);
+      snap_x = (T)io.getd(8); snap_w = (Count)(long long)io.get(9);
       if (HAS_G && (a.step_begin & 3) != 0) wg = philox_call(a.keys, g, STREAM_GAUSS, (uint32_t)(a.step_begin >> 2));
     }
-    for (long long n = a.step_begin; n < a.step_end; ++n) {
+    const Count n_end = (Count)a.step_end, n_snap = (Count)a.n_discard, n_trace = tracing ? (Count)a.trace_steps : 0;
+    for (Count n = (Count)a.step_begin; n < n_end; ++n) {
       // Alg. 2: three-point increment with the first moments of a Gaussian of variance 2 D dt
       T dxi = (T)0;
       if (HAS_G) {
@@ -164,7 +171,7 @@ __global__ void __launch_bounds__(256) bm_paths_literal(const __grid_constant__ 
       if (HAS_P && onP) {
         if (sP <= 0) {
           deta = z - a_dt;
-          jumps += 1.0;
+          jumps += 1;
           kP++;
           const uint4 w = philox_call(a.keys, g, STREAM_POISSON, kP);
           sP = to_steps(M::exp_variate(w.x, inv_lam));
@@ -179,7 +186,7 @@ __global__ void __launch_bounds__(256) bm_paths_literal(const __grid_constant__ 
       if (HAS_D) {
         if (sD <= 0) {
           d = 1 - d;
-          jumps += 1.0;
+          jumps += 1;
           kD++;
           const uint4 w = philox_call(a.keys, g, STREAM_DICH, kD);
           sD = to_steps(M::exp_variate(w.x, d ? inv_mub : inv_mua));
@@ -196,21 +203,21 @@ __global__ void __launch_bounds__(256) bm_paths_literal(const __grid_constant__ 
       F2 = lit_force<T, POT>(xb, A1, A2, F);
       x = x + (T)0.5 * (F1 + F2) * dt + dxi + deta + dGam;
       fold();
-      if (tracing && n + 1 <= a.trace_steps) {
+      if (tracing && n + 1 <= n_trace) {
         trace[2 * n] = (double)wraps * Ld + (double)x;
         trace[2 * n + 1] = 0.0;
       }
-      if (n + 1 == a.n_discard) { snap_x = x; snap_w = wraps; }
+      if (n + 1 == n_snap) { snap_x = x; snap_w = wraps; }
     }
     if (a.state != nullptr) {  // row f2: checkpoint (a float converts to double and back exactly)
       const StateIO io = state_io(a, g);
-      io.putd(0, (double)x); io.put(1, (unsigned long long)wraps);
-      io.put(2, (unsigned long long)sP); io.put(3, (unsigned long long)sD);
+      io.putd(0, (double)x); io.put(1, (unsigned long long)(long long)wraps);
+      io.put(2, (unsigned long long)(long long)sP); io.put(3, (unsigned long long)(long long)sD);
       io.putd(4, (double)z);
       io.put2(5, kP, kD);
       io.put2(6, (uint32_t)d, 0u);
-      io.putd(7, jumps);
-      io.putd(8, (double)snap_x); io.put(9, (unsigned long long)snap_w);
+      io.putd(7, (double)jumps);
+      io.putd(8, (double)snap_x); io.put(9, (unsigned long long)(long long)snap_w);
     }
     // a10: eq. (30)
     const double span = (double)(a.n_steps - a.n_discard) * dtd;
@@ -218,10 +225,10 @@ __global__ void __launch_bounds__(256) bm_paths_literal(const __grid_constant__ 
     const double vbar = ((double)(wraps - snap_w) * Ld + ((double)x - (double)snap_x)) / span;
     if (a.out_paths && a.step_end >= a.n_steps) {
       double *o = a.out_paths + g * BM_OUT_STRIDE;
-      o[BM_OUT_XT] = xT; o[BM_OUT_VT] = 0.0; o[BM_OUT_VBAR] = vbar; o[BM_OUT_JUMPS] = jumps;
+      o[BM_OUT_XT] = xT; o[BM_OUT_VT] = 0.0; o[BM_OUT_VBAR] = vbar; o[BM_OUT_JUMPS] = (double)jumps;
       o[BM_OUT_SUBSTEPS] = (double)a.n_steps; o[BM_OUT_XTI] = (double)snap_w * Ld + (double)snap_x;
     }
-    mine = leaf(vbar, xT, jumps, (double)a.n_steps);
+    mine = leaf(vbar, xT, (double)jumps, (double)a.n_steps);
   }
   if (a.step_end < a.n_steps) return;  // not the last chunk (uniform over the grid)
   block_reduce_store(mine, a.partials + (long long)blockIdx.x * PARTIAL_STRIDE);
