@@ -180,3 +180,32 @@ def test_p8_flip_times_replay(orc):
             k += 1
         assert out[g, orc.OUT_JUMPS] == k
         assert abs(out[g, orc.OUT_XT] - x) < 1e-12
+
+
+def test_r4_initial_velocity_is_uniform_and_independent(orc):
+    """Reading R4: v0 = v0_lo + (v0_hi - v0_lo) u(w1) of init-stream call 0 -- uniform on [v0_lo, v0_hi] and independent
+    of x0 (word 0) and of the initial dichotomous state d (word 2).  A force-free, friction-free particle keeps v0 and
+    moves by v0 dt in one step, so OUT_VT is v0 and OUT_XT - v0 dt is x0; with the two dichotomous forces switched on
+    (no flips within the step, no friction) v(dt) - v0 = +Fb dt or -Fa dt reads off d."""
+    from scipy import stats as st
+    N, lo, hi, dt = 20000, -2.0, 2.0, 1e-6
+    free = orc.params_array([dict(v0_lo=lo, v0_hi=hi)])
+    out, _ = orc.simulate(free, N, 1, dt, SEED, model=orc.INERTIAL)
+    v0 = out[:, orc.OUT_VT]
+    x0 = out[:, orc.OUT_XT] - v0 * dt
+    assert v0.min() >= lo and v0.max() <= hi
+    assert st.kstest((v0 - lo) / (hi - lo), "uniform").statistic < 1.63 / math.sqrt(N)      # 1 % critical value
+    assert abs(v0.mean() - 0.5 * (lo + hi)) < 4 * (hi - lo) / math.sqrt(12 * N)
+    assert abs(v0.var() - (hi - lo) ** 2 / 12) < 4 * (hi - lo) ** 2 / 12 * math.sqrt(0.8 / N)   # kurtosis 1.8
+    assert st.kstest(x0, "uniform").statistic < 1.63 / math.sqrt(N)
+    assert abs(np.corrcoef(v0, x0)[0, 1]) < 4 / math.sqrt(N)
+    # rank correlation too: a monotone but non-linear dependence would show here
+    assert abs(st.spearmanr(v0, x0).statistic) < 4 / math.sqrt(N)
+    dich = orc.params_array([dict(v0_lo=lo, v0_hi=hi, Fa=1.0, Fb=1.0, mu_a=1e-9, mu_b=3e-9)])
+    out2, _ = orc.simulate(dich, N, 1, dt, SEED, model=orc.INERTIAL)
+    assert np.all(out2[:, orc.OUT_JUMPS] == 0)
+    d = np.sign(out2[:, orc.OUT_VT] - v0)                       # +1: state +Fb, -1: state -Fa
+    assert np.all(np.abs(np.abs(out2[:, orc.OUT_VT] - v0) - dt) < 1e-12)
+    assert abs((d > 0).mean() - 0.25) < 4 * math.sqrt(0.25 * 0.75 / N)      # P(+Fb) = mu_a / (mu_a + mu_b)
+    assert abs(np.corrcoef(v0, d)[0, 1]) < 4 / math.sqrt(N)
+    assert abs(np.corrcoef(x0, d)[0, 1]) < 4 / math.sqrt(N)

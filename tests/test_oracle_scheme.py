@@ -155,3 +155,38 @@ def test_p11_inertial_single_step_in_high_precision(orc):
         xe, ve = x + (a1[0] + a2[0]) * h / 2, v + (a1[1] + a2[1]) * h / 2 + nv
         gx, gv = orc.substep_inertial(p, orc.POT_SINE2, d, t0, h0, g0, x0, v0)
         assert abs(gx - float(xe)) < 1e-15 and abs(gv - float(ve)) < 2e-15
+
+
+def test_p11_drive_time_inside_a_split_grid_step(orc):
+    """Reading R5 / SURVEY O7: a sub-step that starts inside a grid step sees the drive at t = n dt + tau, not at n dt.
+    The linear driven ODE of the test above with Poisson kicks of amplitude ZERO (lambda > 0, zeta = 0): the kicks split
+    grid steps (jump-adapted grid) but move nothing, so every path must still follow the closed form at
+    order 2 and stay within O(dt^2) of the unsplit run.  A drive evaluated at the start of the grid step instead of the
+    start of the sub-step is an O(dt) error per split and breaks both."""
+    gam, amp, om, F, x0, v0, T, lam = 0.9, 4.2, 4.9, 0.3, 0.2, -1.0, 3.0, 40.0
+    a = amp * gam / (gam * gam + om * om)
+    b = amp * om / (gam * gam + om * om)
+    c = v0 - F / gam - a
+    vT = F / gam + a * math.cos(om * T) + b * math.sin(om * T) + c * math.exp(-gam * T)
+    xT = x0 + F / gam * T + a / om * math.sin(om * T) - b / om * (math.cos(om * T) - 1) + c / gam * (1 - math.exp(-gam * T))
+    n_paths = 64
+    errs = []
+    for n in (300, 600, 1200):
+        base = dict(F=F, gamma=gam, amp=amp, omega=om, x0_fixed=x0, v0_lo=v0, v0_hi=v0)
+        split, _ = orc.simulate(orc.params_array([dict(base, lambda_=lam, zeta=0.0)]), n_paths, n, T / n, SEED,
+                                model=orc.INERTIAL)
+        plain, _ = orc.simulate(orc.params_array([base]), 1, n, T / n, SEED, model=orc.INERTIAL)
+        assert split[:, orc.OUT_JUMPS].min() >= 60            # ~120 kicks per path: most grid steps near them are split
+        assert np.all(split[:, orc.OUT_SUBSTEPS] == n + split[:, orc.OUT_JUMPS])
+        ex = np.abs(split[:, orc.OUT_XT] - xT).max()
+        ev = np.abs(split[:, orc.OUT_VT] - vT).max()
+        errs.append((ex, ev))
+        # splitting a step changes the result only at the order of the scheme's own error
+        e0 = max(abs(plain[0, orc.OUT_XT] - xT), abs(plain[0, orc.OUT_VT] - vT))
+        assert ex < 3 * e0 and ev < 3 * e0, (n, ex, ev, e0)
+    for i in range(2):
+        for k in range(2):
+            # order 2 or better (the share of split steps, lambda dt = 0.4 / 0.2 / 0.1, falls with dt; an O(dt) error
+            # of the drive time would give a ratio of 2 and errors sixty times larger)
+            assert 3.3 < errs[i][k] / errs[i + 1][k] < 7.0, errs
+    assert errs[-1][0] < 2e-5 and errs[-1][1] < 2e-5
