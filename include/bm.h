@@ -28,7 +28,7 @@
 extern "C" {
 #endif
 
-#define BM_VERSION 101 /* 0.1.1 */
+#define BM_VERSION 200 /* 0.2.0 */
 
 #if defined(__GNUC__)
 #define BM_API __attribute__((visibility("default")))
@@ -73,9 +73,11 @@ typedef struct {
   double A1, A2;            /* potential amplitudes (see bm_potential) */
   double F;                 /* static load (f of the inertial model) */
   double D;                 /* Gaussian intensity: overdamped sqrt(2D) dW (eq. 9-10); inertial D := gamma*Q */
-  double lambda, zeta;      /* Poisson rate (eq. 4) and mean amplitude (eq. 5); bias -lambda*zeta (eq. 3, 6) */
+  double lambda, zeta;      /* Poisson rate (eq. 4) and mean amplitude (eq. 5); bias -lambda*zeta (eq. 3, 6);
+                               lambda <= 0 switches the source off at this point */
   double Fa, Fb;            /* dichotomous values -Fa, +Fb (eq. 13), both > 0 */
-  double mu_a, mu_b;        /* rate of leaving -Fa, rate of leaving +Fb (eq. 14) */
+  double mu_a, mu_b;        /* rate of leaving -Fa, rate of leaving +Fb (eq. 14).  mu_a <= 0 switches the source off at
+                               this point (Gamma = 0); mu_b <= 0 with mu_a > 0 makes +Fb absorbing */
   double gamma, amp, omega; /* inertial: friction, drive amplitude, drive angular frequency */
   double x0_fixed;          /* >= 0: x0 = x0_fixed; < 0: x0 ~ U[0,L) */
   double v0_lo, v0_hi;      /* inertial: v0 ~ U[v0_lo, v0_hi] */
@@ -123,7 +125,9 @@ BM_API size_t bm_workspace_bytes(const bm_config *cfg, int32_t n_points, int64_t
  *   out_trace  [trace_paths][trace_steps][2] device, optional: (x unfolded, v) after each grid step
  *   workspace  device scratch of >= bm_workspace_bytes(...) bytes, 16-byte aligned
  * Kernels launched on `stream`: the path kernel (a1-a10 of DESIGN.md section 2) and the grid pass of the
- * reduction (a11).  Errors: BM_ERR_INVALID_ARG as listed above; BM_ERR_UNSUPPORTED for
+ * reduction (a11).  n_steps <= 2^31 - 16 for BM_F32 (32-bit cell counters), <= 2^33 for BM_F64 (the Gaussian stream is
+ * indexed by a 32-bit counter word).  Parameter VALUES are not checked here (params is a device pointer; see
+ * bm_simulate_host).  Errors: BM_ERR_INVALID_ARG as listed above; BM_ERR_UNSUPPORTED for
  * PAPER_LITERAL with BM_INERTIAL, BM_INERTIAL with a potential other than SINE2, out_trace with BM_F32;
  * BM_ERR_WORKSPACE; BM_ERR_CUDA.
  */
@@ -180,7 +184,11 @@ BM_API bm_status bm_state_histogram(const bm_config *cfg, int32_t n_points, int6
  * HOST-pointer convenience entry (the end-to-end path): params, out_stats and out_paths (optional) are HOST
  * buffers.  Takes device scratch from a private stream-ordered pool (one per device, kept between calls: an
  * allocation cache with no influence on results), copies params in, runs bm_simulate on `stream`, copies the
- * results out, returns the scratch to the pool and synchronises the stream.
+ * results out, returns the scratch to the pool and synchronises the stream.  May be called from several host threads
+ * (the pool table is guarded by a mutex; calls on the same stream serialise on that stream as usual).
+ * Having the values on the host, it also checks them: BM_ERR_INVALID_ARG for a non-finite entry, a negative D, lambda,
+ * mu_a, mu_b or gamma, zeta <= 0 where lambda > 0, Fa <= 0 or Fb <= 0 where mu_a > 0, v0_hi < v0_lo -- for the sources
+ * cfg->noise switches on and the model cfg->model selects.
  */
 BM_API bm_status bm_simulate_host(const bm_config *cfg, const bm_params *params, int32_t n_points, int64_t n_paths,
                            int64_t n_steps, double dt, uint64_t seed, bm_stats *out_stats, double *out_paths,

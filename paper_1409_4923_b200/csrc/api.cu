@@ -1,6 +1,8 @@
 // api.cu -- the C ABI of include/bm.h: argument validation, kernel selection, launches.  No compute here.
+#include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 
 #include "dispatch.cuh"
 
@@ -105,8 +107,10 @@ bm_status pick_kernel(const bm_config *c, int32_t n_points, int64_t n_paths, Lau
 // no influence on any result.
 cudaMemPool_t host_entry_pool() {
   static cudaMemPool_t pools[64] = {};
+  static std::mutex guard;  // the HOST entry may be called from several host threads at once
   int dev = 0;
   if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
+  std::lock_guard<std::mutex> lock(guard);
   if (!pools[dev]) {
     cudaMemPoolProps props = {};
     props.allocType = cudaMemAllocationTypePinned;
@@ -120,6 +124,24 @@ cudaMemPool_t host_entry_pool() {
     pools[dev] = pool;
   }
   return pools[dev];
+}
+
+// Parameter values as SURVEY.md s.8(b) lists them for BM_ERR_INVALID_ARG.  Only the HOST entry can check them (the
+// device-pointer calls never read `params` on the host): finite numbers, no negative rate or intensity, positive
+// amplitudes of a source that is switched on.
+bool valid_params_host(const bm_config *c, const bm_params *p, int32_t n_points) {
+  for (int32_t i = 0; i < n_points; ++i) {
+    const bm_params &q = p[i];
+    const double all[16] = {q.A1, q.A2, q.F, q.D, q.lambda, q.zeta, q.Fa, q.Fb, q.mu_a, q.mu_b, q.gamma, q.amp, q.omega,
+                            q.x0_fixed, q.v0_lo, q.v0_hi};
+    for (double v : all)
+      if (!std::isfinite(v)) return false;
+    if ((c->noise & BM_NOISE_GAUSS) && q.D < 0.0) return false;
+    if ((c->noise & BM_NOISE_POISSON) && (q.lambda < 0.0 || (q.lambda > 0.0 && !(q.zeta > 0.0)))) return false;
+    if ((c->noise & BM_NOISE_DICH) && (q.mu_a < 0.0 || q.mu_b < 0.0 || (q.mu_a > 0.0 && (!(q.Fa > 0.0) || !(q.Fb > 0.0))))) return false;
+    if (c->model == BM_INERTIAL && (q.gamma < 0.0 || q.v0_hi < q.v0_lo)) return false;
+  }
+  return true;
 }
 
 long long blocks_per_point_of(const bm_config *c, int32_t n_points, int64_t n_paths) {
@@ -161,7 +183,10 @@ static bm_status simulate_range(const bm_config *cfg, const bm_params *params, i
   if (!valid_cfg(cfg) || !params || !out_stats || n_points <= 0 || n_paths <= 0 || n_steps <= 0) return BM_ERR_INVALID_ARG;
   if (!(dt > 0.0) || !(dt < 1e300)) return BM_ERR_INVALID_ARG;
   if (cfg->n_discard >= n_steps) return BM_ERR_INVALID_ARG;
-  if (cfg->prec == BM_F32 && n_steps > 0x7FFFFFF0LL) return BM_ERR_INVALID_ARG;
+  // step and draw counters: the fp32 kernels count grid cells in 32 bits; the fp64 kernels index the Gaussian stream
+  // by (sub-step count)/4 in a 32-bit counter word (sub-steps = grid steps + events < 2^34)
+  const bool narrow = cfg->prec == BM_F32;
+  if (n_steps > (narrow ? 0x7FFFFFF0LL : (1LL << 33))) return BM_ERR_INVALID_ARG;
   if (out_trace && (cfg->trace_steps <= 0 || cfg->trace_paths <= 0)) return BM_ERR_INVALID_ARG;
   if (out_trace && cfg->prec != BM_F64) return BM_ERR_UNSUPPORTED;
   Launch L;
@@ -255,6 +280,7 @@ BM_API bm_status bm_simulate_host(const bm_config *cfg, const bm_params *params,
                            int64_t n_steps, double dt, uint64_t seed, bm_stats *out_stats, double *out_paths,
                            void *stream) {
   if (!valid_cfg(cfg) || !params || !out_stats || n_points <= 0 || n_paths <= 0) return BM_ERR_INVALID_ARG;
+  if (!valid_params_host(cfg, params, n_points)) return BM_ERR_INVALID_ARG;
   const size_t ws = bm_workspace_bytes(cfg, n_points, n_paths);
   if (ws == 0) return BM_ERR_INVALID_ARG;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);

@@ -162,9 +162,10 @@ __device__ __forceinline__ void schedule_f32(int n, float tau, float dt, float i
   const float q = fmaf(tau, inv_dt, Wcells);
   float c = floorf(q);
   float f = (q - c) * dt;
+  if (!(Wcells < 2.0e9f)) { cell = 0x7FFFFFFF; off = 0.0f; return; }  // beyond any run (also a rate of zero: never)
   if (f >= dt) { f = 0.0f; c += 1.0f; }
   if (c == 0.0f) f = fmaxf(f, tau);  // never schedule into the past of this cell
-  c = fminf(c, 2.0e9f);  // < 2^31: the 32-bit conversion is exact, and n + c < 2^32 cannot wrap as unsigned
+  // c <= 2e9 < 2^31: the 32-bit conversion is exact, and n + c < 2^32 cannot wrap as unsigned
   const unsigned t = (unsigned)n + (unsigned)__float2int_rz(c);
   cell = (int)min(t, 0x7FFFFFFFu);
   off = f;
@@ -291,13 +292,16 @@ __global__ void __launch_bounds__(MODEL == BM_INERTIAL ? 256 : 512) bm_paths_f32
     P.kk2 = 0.f;
     P.base = (float)(bp.F - lam * zet);
   }
-  P.Ga = (float)((double)S * (-bp.Fa));
-  P.Gb = (float)((double)S * bp.Fb);
+  // a non-positive rate of leaving -Fa switches the dichotomous source off at this point (Gamma = 0, as the oracle);
+  // a non-positive rate of leaving +Fb makes that state absorbing
+  const bool onD = HAS_D && bp.mu_a > 0.0;
+  P.Ga = onD ? (float)((double)S * (-bp.Fa)) : 0.f;
+  P.Gb = onD ? (float)((double)S * bp.Fb) : 0.f;
   P.cn = (float)(-2.0 * M_LN2 * (double)S * (double)S * 2.0 * Dd * dtd);
   P.inv_lam_dt = (lam > 0.0) ? (float)(1.0 / (lam * dtd)) : 0.f;
   P.zeta = (float)((double)S * zet);
-  P.inv_mua_dt = (HAS_D && bp.mu_a > 0.0) ? (float)(1.0 / (bp.mu_a * dtd)) : 0.f;
-  P.inv_mub_dt = (HAS_D && bp.mu_b > 0.0) ? (float)(1.0 / (bp.mu_b * dtd)) : 0.f;
+  P.inv_mua_dt = onD ? (float)(1.0 / (bp.mu_a * dtd)) : 0.f;
+  P.inv_mub_dt = (onD && bp.mu_b > 0.0) ? (float)(1.0 / (bp.mu_b * dtd)) : __int_as_float(0x7f800000);
   P.gamma = (float)bp.gamma;
   P.amp = (float)((double)S * bp.amp);
   P.w_turns = (float)(bp.omega / (2.0 * M_PI));
@@ -322,7 +326,7 @@ __global__ void __launch_bounds__(MODEL == BM_INERTIAL ? 256 : 512) bm_paths_f32
   if (INERTIAL)
     v = (float)((double)S * (bp.v0_lo + (bp.v0_hi - bp.v0_lo) * (((double)wi.y + 0.5) * (1.0 / 4294967296.0))));
   int d = 0;
-  if (HAS_D) d = ((((double)wi.z + 0.5) * (1.0 / 4294967296.0)) < bp.mu_a / (bp.mu_a + bp.mu_b)) ? 1 : 0;
+  if (onD) d = ((((double)wi.z + 0.5) * (1.0 / 4294967296.0)) < bp.mu_a / (bp.mu_a + bp.mu_b)) ? 1 : 0;
 
   const int n_discard = (int)a.n_discard;
   // jump clocks: (cell index, offset inside that cell); NEVER = switched off at this point
@@ -330,13 +334,14 @@ __global__ void __launch_bounds__(MODEL == BM_INERTIAL ? 256 : 512) bm_paths_f32
   float fP = 0.f, fD = 0.f, z = 0.f;
   uint32_t kP = 0, kD = 0;
   uint32_t gwP = 0, gwD = 0;  // Gaussian word of the sub-step that ends at the next kick / flip (R13)
-  if (HAS_P && lam > 0.0) {
+  // lanes past a ragged end stay inert: no events, no checkpoint traffic (they must not steer the warp's votes)
+  if (HAS_P && lam > 0.0 && valid) {
     const uint4 w = philox_call(K, g, STREAM_POISSON, 0);
     gwP = w.z;
     schedule_f32(0, 0.f, dt, inv_dt, neg_log_u_f32(w.x) * P.inv_lam_dt, nP, fP);
     z = P.zeta * neg_log_u_f32(w.y);
   }
-  if (HAS_D) {
+  if (onD && valid) {
     const uint4 w = philox_call(K, g, STREAM_DICH, 0);
     gwD = w.z;
     schedule_f32(0, 0.f, dt, inv_dt, neg_log_u_f32(w.x) * (d ? P.inv_mub_dt : P.inv_mua_dt), nD, fD);
@@ -359,7 +364,7 @@ __global__ void __launch_bounds__(MODEL == BM_INERTIAL ? 256 : 512) bm_paths_f32
   // row f2: a launch that continues a run reloads everything the lines above initialised (the Philox calls of the
   // initialisation are wasted then, once per launch)
   const int n_begin = (int)a.step_begin, n_end = (int)a.step_end;
-  if (a.state != nullptr && n_begin > 0) {
+  if (a.state != nullptr && n_begin > 0 && valid) {
     const StateIO io = state_io(a, g);
     uint32_t lo, hi;
     io.get2(0, lo, hi); x = __uint_as_float(lo); wraps = (int)hi;

@@ -131,11 +131,13 @@ __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimA
     s.wraps = 0;
     s.v = INERTIAL ? bp.v0_lo + (bp.v0_hi - bp.v0_lo) * u01_f64(wi.y) : 0.0;
     fold_f64<POT>(s);
-    int d = HAS_D ? ((u01_f64(wi.z) < P.mu_a / (P.mu_a + P.mu_b)) ? 1 : 0) : -1;
+    // a non-positive rate of leaving -Fa switches the dichotomous source off at this point (Gamma = 0, as the oracle)
+    const bool onD = HAS_D && P.mu_a > 0.0;
+    int d = onD ? ((u01_f64(wi.z) < P.mu_a / (P.mu_a + P.mu_b)) ? 1 : 0) : -1;
 
     uint32_t kP = 0, kD = 0;
     double rP = 0.0, rD = 0.0, z = 0.0;
-    bool onP = false, onD = HAS_D;
+    bool onP = false;
     if (HAS_P) {
       onP = P.lambda > 0.0;  // lambda == 0 at a point of a sweep: the clock never fires
       if (onP) {
@@ -144,7 +146,7 @@ __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimA
         z = -P.zeta * log(u01_f64(w.y));
       }
     }
-    if (HAS_D) {
+    if (HAS_D && onD) {
       const uint4 w = philox_call(a.keys, g, STREAM_DICH, 0);
       rD = -log(u01_f64(w.x)) / (d ? P.mu_b : P.mu_a);
     }
@@ -184,7 +186,7 @@ __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimA
         gn = (j == 0) ? gq[0] : (j == 1) ? gq[1] : (j == 2) ? gq[2] : gq[3];
       }
       m++;
-      const double Gd = HAS_D ? (d ? P.Fb : -P.Fa) : 0.0;
+      const double Gd = (HAS_D && onD) ? (d ? P.Fb : -P.Fa) : 0.0;
       const double cst = P.c0 + Gd;
       const double dxi = HAS_G ? sqrt(2.0 * P.D * h) * gn : 0.0;
       if (!INERTIAL) {

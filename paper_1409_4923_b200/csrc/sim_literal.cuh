@@ -96,15 +96,18 @@ __global__ void __launch_bounds__(256) bm_paths_literal(const __grid_constant__ 
       wraps = (Count)k;
     }
     T x = (T)x0;
-    int d = HAS_D ? ((u01_f64(wi.z) < bp.mu_a / (bp.mu_a + bp.mu_b)) ? 1 : 0) : 0;
+    // a non-positive rate of leaving -Fa switches the dichotomous source off at this point (as the oracle); a
+    // non-positive rate of leaving +Fb makes that state absorbing (infinite sojourn)
+    const bool onD = HAS_D && bp.mu_a > 0.0;
+    int d = onD ? ((u01_f64(wi.z) < bp.mu_a / (bp.mu_a + bp.mu_b)) ? 1 : 0) : 0;
 
     // countdowns in grid steps (integers: exact in both precisions)
     Count sP = 0, sD = 0;
     T z = (T)0;
     uint32_t kP = 0, kD = 0;
     const T inv_lam = onP ? (T)(1.0 / lam) : (T)0, zeta = (T)zet;
-    const T inv_mua = (HAS_D && bp.mu_a > 0.0) ? (T)(1.0 / bp.mu_a) : (T)0;
-    const T inv_mub = (HAS_D && bp.mu_b > 0.0) ? (T)(1.0 / bp.mu_b) : (T)0;
+    const T inv_mua = onD ? (T)(1.0 / bp.mu_a) : (T)0;
+    const T inv_mub = (onD && bp.mu_b > 0.0) ? (T)(1.0 / bp.mu_b) : (T)HUGE_VAL;
     auto to_steps = [&](T wait) -> Count {  // [wait / dt], Alg. 3 line 5 / Alg. 4
       const T q = M::floor_(F64 ? wait / dt : wait * inv_dt);
       return q < (F64 ? (T)9.0e18 : (T)2.0e9) ? (Count)q : COUNT_MAX;
@@ -114,7 +117,7 @@ __global__ void __launch_bounds__(256) bm_paths_literal(const __grid_constant__ 
       sP = to_steps(M::exp_variate(w.x, inv_lam));
       z = M::exp_variate(w.y, zeta);
     }
-    if (HAS_D) {
+    if (HAS_D && onD) {
       const uint4 w = philox_call(a.keys, g, STREAM_DICH, 0);
       sD = to_steps(M::exp_variate(w.x, d ? inv_mub : inv_mua));
     }
@@ -183,7 +186,7 @@ __global__ void __launch_bounds__(256) bm_paths_literal(const __grid_constant__ 
       }
       // Alg. 4: flip when the countdown has run out; the state's force times dt
       T dGam = (T)0;
-      if (HAS_D) {
+      if (HAS_D && onD) {
         if (sD <= 0) {
           d = 1 - d;
           jumps += 1;

@@ -42,7 +42,7 @@ def test_struct_layouts_match_header(B):
 
 
 def test_version_and_status_strings(B):
-    assert B.bm_version() == 101
+    assert B.bm_version() == 200
     assert B.status_string(B.BM_OK) == "BM_OK" and B.status_string(B.BM_ERR_CUDA) == "BM_ERR_CUDA"
     assert B.status_string(99) == "BM_ERR_UNKNOWN"
 
@@ -67,6 +67,42 @@ def test_invalid_arguments_are_rejected_before_any_cuda_call(B):
     assert L.bm_simulate(C.byref(cfg), p.ctypes.data, 1, 32, 10, 1e-3, 1, st.ctypes.data, None, None, None, 0, None) == B.BM_ERR_WORKSPACE
     assert L.bm_philox_fill(1, 0, 0, 1, 0, 4, None, None) == B.BM_ERR_INVALID_ARG
     assert L.bm_gauss_fill(B.BM_F64, 0, 1, 0, 4, 2, 4, p.ctypes.data, None) == B.BM_ERR_INVALID_ARG   # m0 % 8 != 0
+
+
+def test_host_entry_validates_parameter_values(B):
+    """negative rates / intensities and non-positive amplitudes of a source that is on are
+    BM_ERR_INVALID_ARG.  Only the HOST entry can see the values; it rejects them before any CUDA call."""
+    st = np.zeros((1, 8))
+
+    def rc(noise=7, model=B.BM_OVERDAMPED, **kw):
+        base = dict(A1=1.0, D=0.01, lambda_=2.0, zeta=0.3, Fa=0.5, Fb=0.5, mu_a=1.0, mu_b=1.0, gamma=0.9)
+        base.update(kw)
+        cfg = B.make_config(noise=noise, model=model)
+        try:
+            B.bm_simulate_host(cfg, W.params_table(1, **base), 1, 32, 10, 1e-3, 1, st)
+        except B.BmError as e:
+            return e.status
+        return B.BM_OK
+    for bad in (dict(D=-1e-3), dict(lambda_=-1.0), dict(zeta=0.0), dict(zeta=-0.3), dict(mu_a=-1.0), dict(mu_b=-2.0),
+                dict(Fa=0.0), dict(Fb=-0.5), dict(A1=float("nan")), dict(F=float("inf"))):
+        assert rc(**bad) == B.BM_ERR_INVALID_ARG, bad
+    assert rc(model=B.BM_INERTIAL, gamma=-0.1) == B.BM_ERR_INVALID_ARG
+    assert rc(model=B.BM_INERTIAL, v0_lo=1.0, v0_hi=-1.0) == B.BM_ERR_INVALID_ARG
+    # a source that is switched off ignores its parameters; a rate of zero switches a source off at that point
+    import torch
+    ok = B.BM_OK if torch.cuda.is_available() else B.BM_ERR_CUDA
+    assert rc(noise=B.BM_NOISE_GAUSS, lambda_=-1.0, mu_a=-1.0) == ok
+    assert rc(lambda_=0.0, zeta=0.0, mu_a=0.0, Fa=0.0) == ok
+
+
+def test_step_count_limits(B):
+    """The fp32 kernels count grid cells in 32 bits; the fp64 kernels index the Gaussian stream in a 32-bit counter word."""
+    L = B.lib()
+    p = np.zeros((1, 16)); st = np.zeros((1, 8))
+    for prec, limit in ((B.BM_F32, 0x7FFFFFF0), (B.BM_F64, 1 << 33)):
+        cfg = B.make_config(prec=prec)
+        assert L.bm_simulate(C.byref(cfg), p.ctypes.data, 1, 32, limit + 1, 1e-3, 1, st.ctypes.data, None, None, None, 0, None) == B.BM_ERR_INVALID_ARG
+        assert L.bm_simulate(C.byref(cfg), p.ctypes.data, 1, 32, limit, 1e-3, 1, st.ctypes.data, None, None, None, 0, None) == B.BM_ERR_WORKSPACE
 
 
 def test_no_cpu_fallback_without_a_device(B):

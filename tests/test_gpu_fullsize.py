@@ -68,8 +68,11 @@ def test_c3_full_size_fp32_sampled_points(B, orc):
     stats, _, _ = B.run_workload(w, B.BM_F32)
     assert np.all(stats[:, 0] == w.n_paths)
     for pt in (0, 128, 255):
-        ids = pt * w.n_paths + np.arange(160)
+        ids = pt * w.n_paths + np.arange(1024)       # the whole point: 1024 paths
         check_point(stats[pt], oracle_sample(orc, w, ids), orc, f"C3 full fp32 point {pt}")
+    # flips per path at every point: a Poisson process of rate mu = 1 over T = 2000 periods (5 SE)
+    muT = 1.0 * w.n_steps * w.dt
+    assert np.all(np.abs(stats[:, 5] - muT) < 5 * math.sqrt(muT / w.n_paths))
     # the sweep is antisymmetric up to the ratchet bias: <v> increases with the load f on average
     assert stats[-32:, 1].mean() > stats[:32, 1].mean()
 
