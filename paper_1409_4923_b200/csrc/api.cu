@@ -76,6 +76,7 @@ struct Launch {
   KernelFn fn = nullptr;
   int threads = 0;  // threads per block
   int gauss = 0;    // bm_gauss selected (fp32), 0 for fp64
+  size_t smem = 0;  // dynamic shared memory per block (event rings of the fp32 jump-adapted kernel)
 };
 
 bm_status pick_kernel(const bm_config *c, int32_t n_points, int64_t n_paths, Launch *L, bool chunked = false) {
@@ -97,8 +98,15 @@ bm_status pick_kernel(const bm_config *c, int32_t n_points, int64_t n_paths, Lau
          {pick_f32_in_fma_w32, pick_f32_in_fma_w16, pick_f32_in_fma_w16p}}};
     L->gauss = resolve_gauss(c);
     L->fn = table[c->model == BM_INERTIAL][resolve_sincos(c) == BM_SINCOS_FMA][L->gauss - 1](c->potential, c->noise);
+    L->smem = (size_t)L->threads * sizeof(uint32_t) * (size_t)f32_smem_words_per_thread(c->noise, L->gauss);
   }
   if (!L->fn) return BM_ERR_UNSUPPORTED;
+  // beyond the 48 KB default a kernel has to opt in (per function and device; repeating the call is harmless)
+  if (L->smem > 48 * 1024 &&
+      cudaFuncSetAttribute((const void *)L->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L->smem) != cudaSuccess) {
+    cudaGetLastError();
+    return BM_ERR_CUDA;
+  }
   return BM_OK;
 }
 
@@ -218,7 +226,7 @@ static bm_status simulate_range(const bm_config *cfg, const bm_params *params, i
 
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   const unsigned grid = (unsigned)((long long)a.blocks_per_point * n_points);
-  L.fn<<<grid, L.threads, 0, st>>>(a);  // a1: (point x path) -> grid
+  L.fn<<<grid, L.threads, L.smem, st>>>(a);  // a1: (point x path) -> grid
   if (cudaGetLastError() != cudaSuccess) return BM_ERR_CUDA;
   if (step_end < n_steps) return BM_OK;  // the ensemble reduction belongs to the last chunk
   if (launch_grid_reduce(a.partials, n_points, a.blocks_per_point, out_stats, st) != cudaSuccess) return BM_ERR_CUDA;
@@ -341,7 +349,7 @@ BM_API bm_status bm_kernel_info(const bm_config *cfg, int32_t n_points, int64_t 
   cudaFuncAttributes attr;
   if (cudaFuncGetAttributes(&attr, (const void *)L.fn) != cudaSuccess) { cudaGetLastError(); return BM_ERR_CUDA; }
   int nb = 0, dev = 0, sms = 0;
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, (const void *)L.fn, L.threads, 0) != cudaSuccess) { cudaGetLastError(); return BM_ERR_CUDA; }
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, (const void *)L.fn, L.threads, L.smem) != cudaSuccess) { cudaGetLastError(); return BM_ERR_CUDA; }
   if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
     cudaGetLastError();
     return BM_ERR_CUDA;

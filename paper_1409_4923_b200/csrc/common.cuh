@@ -61,6 +61,17 @@ __device__ __forceinline__ StateIO state_io(const SimArgs &a, unsigned long long
   return StateIO{a.state + g, (long long)a.n_points * a.n_paths};
 }
 
+// fp32 path kernel: event rings in dynamic shared memory (sim_f32.cuh, "event queues"); the host sizes the launch with
+// the same function the kernel lays its arrays out with.
+constexpr int EVQ = 8;  // ring capacity per path and stream (a power of two, <= 16)
+constexpr int EVK = 4;  // refill passes per episode
+constexpr int EV_FIELDS_P = 4, EV_FIELDS_D = 3;  // (cell, off, amplitude, normal), (cell, off, normal)
+
+// 32-bit words of dynamic shared memory per thread of the fp32 path kernel (host and device agree through this)
+__host__ __device__ constexpr int f32_smem_words_per_thread(int noise, int gauss) {
+  return ((noise & BM_NOISE_POISSON) ? EVQ * EV_FIELDS_P : 0) + ((noise & BM_NOISE_DICH) ? EVQ * EV_FIELDS_D : 0) + 0 * gauss;
+}
+
 constexpr uint32_t PHILOX_M0 = 0xD2511F53u, PHILOX_M1 = 0xCD9E8D57u;
 constexpr uint32_t PHILOX_W0 = 0x9E3779B9u, PHILOX_W1 = 0xBB67AE85u;
 

@@ -1,8 +1,8 @@
-// sim_f32.cuh -- fp32 path kernel (the throughput kernel), v5.  One thread = one realization; position, clocks,
+// sim_f32.cuh -- fp32 path kernel (the throughput kernel), v6.  One thread = one realization; position, next events,
 // Gaussian cache and observable snapshot stay in registers for the whole run.
 //
 // Same method as the fp64 kernel (R1-R9), arranged for fp32 accuracy and for the SM's pipes
-// (profiles/r1_c1_f32_v3.md and profiles/r1_f32_v5.md are the measurements this layout answers):
+// (profiles/r1_f32_v5.md and profiles/r2_*.md are the measurements this layout answers):
 //  * the position is carried as theta = 2 pi x / L (radians of the potential's phase), folded to [-pi, pi) with an
 //    int32 wrap counter by a round-to-nearest "magic add" (no F2I/FRND, which share the 16-lane XU
 //    pipe with MUFU).  In these units a force cosine is FMUL.RZ + MUFU.COS with no scaling multiply in front;
@@ -16,12 +16,14 @@
 //  * the Box-Muller pair of cells (2i+2, 2i+3) is formed while cells (2i, 2i+1) run, and the ten Philox rounds of
 //    the next Gaussian call are spread over the pair slots, so the integer and MUFU work of the Gaussians sits in
 //    the stalls of the serial cosine chain of Alg. 1 instead of in a phase of its own;
+//  * kick and flip times do not depend on the motion, so they are drawn AHEAD of time into per-path rings in shared
+//    memory, refilled by the whole warp at once (v6: a slow cell no longer holds a Philox call that one or two lanes
+//    execute while thirty wait; see "event queues" below);
 //  * a lane with events inside the current cell integrates up to each event on its own (a divergent loop:
-//    sub-step of length h, a8, redraw of the clock), then every lane finishes the cell together with its own
+//    sub-step of length h, a8, next event from the ring), then every lane finishes the cell together with its own
 //    remaining length (a5).  The Gaussian of a grid cell comes from the Gaussian stream indexed by the CELL, the
-//    Gaussian of a sub-step that ends at event k from the spare word of call k of that event's stream, drawn one
-//    event earlier (R13), so the normal cache never gets out of phase between lanes and the Philox rounds of a
-//    redraw do not sit in front of the sub-step that needs the normal;
+//    Gaussian of a sub-step that ends at event k from the spare word of call k of that event's stream (R13), so the
+//    normal cache never gets out of phase between lanes;
 //  * a jump clock is (cell index, offset in that cell), so nothing small is ever subtracted from something large;
 //  * the Box-Muller radius carries the noise amplitude (sqrt(-2 ln u) * sqrt(2 D dt) in one MUFU.SQRT);
 //  * uniforms come from Philox words through a mantissa splice (no I2F).  BM_GAUSS_W32: one word per uniform,
@@ -34,6 +36,7 @@
 // fp32 results are judged statistically against the fp64 oracle (3 combined standard errors).
 #pragma once
 #include "common.cuh"
+
 
 namespace bm {
 
@@ -244,12 +247,36 @@ __device__ __forceinline__ void gauss_block_standard_f32(const PhiloxKeys &K, un
   }
 }
 
+// ---- event queues (a5, a8) -----------------------------------------------------------------------------------
+// The kick and flip times of a path do not depend on its motion, so they are drawn AHEAD of time: per path and jump
+// stream the next event sits in registers (cell, offset, amplitude, normal of the sub-step that ends on it) and up to
+// EVQ later ones in a ring in shared memory ([slot][field][thread]: conflict-free whatever the lanes' slots are).
+// The rings are refilled by the whole warp at once, in uniform control flow at the top of a block of cells, EVK
+// events per lane and episode, so one pass of Philox rounds serves up to 32 events instead of the one or two lanes
+// that happen to have an event in a cell.  An episode starts when the last queued event of some lane falls into the
+// block about to run; afterwards every event of the block is known (the block is COVERED) unless a lane has more than
+// EVQ of them, in which case the block runs cell by cell with refills in between (CAREFUL).
+// EVQ (ring capacity), EVK (refill passes per episode) and the shared-memory layout: common.cuh
+
+// covered non-clean blocks: unrolled pair slots (1) or one rolled copy of the slot code (0) -- a measured choice
+#ifndef BM_F32_UNROLLED
+#define BM_F32_UNROLLED(inertial) (!(inertial))
+#endif
+
+// register budget of the path kernel (experiment builds override it with -DBM_F32_MAXNREG=n)
+#ifdef BM_F32_MAXNREG
+#define BM_F32_BOUNDS(model) __maxnreg__(BM_F32_MAXNREG)
+#else
+#define BM_F32_BOUNDS(model) __launch_bounds__((model) == BM_INERTIAL ? 256 : 512, 1)
+#endif
+
 // Per-point constants, fp32, theta units (theta = SCALE x)
 struct PointF32 {
   float kk1, kk2;    // SINE2: SCALE * (-V') = base-part + c (kk1 + kk2 c), c = cos theta.  PWL/QUAD: kk1 = A1
   float base;        // SCALE * (F - lambda zeta (+ 4 pi A2 for SINE2))
   float Ga, Gb;      // SCALE * (-Fa), SCALE * (+Fb)
   float cn;          // -2 ln2 * SCALE^2 * 2 D dt: Box-Muller radius^2 per unit of lg2 u, full grid step
+  float s2;          // SCALE^2 * 2 D: variance of the Gaussian increment per unit time
   float inv_lam_dt;  // 1/(lambda dt): waiting time in cells = -ln u * inv_lam_dt
   float zeta;        // SCALE * zeta
   float inv_mua_dt, inv_mub_dt;
@@ -259,13 +286,20 @@ struct PointF32 {
 };
 
 template <int MODEL, int POT, int NOISE, int SINCOS, int GW>
-__global__ void __launch_bounds__(MODEL == BM_INERTIAL ? 256 : 512) bm_paths_f32(const __grid_constant__ SimArgs a) {
+__global__ void BM_F32_BOUNDS(MODEL) bm_paths_f32(const __grid_constant__ SimArgs a) {
   constexpr bool HAS_G = NOISE & BM_NOISE_GAUSS, HAS_P = NOISE & BM_NOISE_POISSON, HAS_D = NOISE & BM_NOISE_DICH;
+  constexpr bool HAS_EV = HAS_P || HAS_D;
   constexpr bool INERTIAL = MODEL == BM_INERTIAL;
   constexpr int NB = GaussLayout<GW>::NB, NP = GaussLayout<GW>::NP;  // grid cells, pairs per Gaussian call
   constexpr float S = Units<POT>::SCALE;
   constexpr unsigned FULL = 0xffffffffu;
   constexpr int NEVER = 0x7FFFFFFF;
+  constexpr int NFP = HAS_P ? EV_FIELDS_P : 0, NFD = HAS_D ? EV_FIELDS_D : 0;
+
+  extern __shared__ uint32_t smem_words[];
+  const int T = blockDim.x, tid = threadIdx.x;
+  uint32_t *const ringP = smem_words + tid;               // [EVQ][NFP][T]
+  uint32_t *const ringD = ringP + EVQ * NFP * T;          // [EVQ][NFD][T]
 
   const int point = blockIdx.x / a.blocks_per_point;
   const int chunk = blockIdx.x - point * a.blocks_per_point;
@@ -298,6 +332,7 @@ __global__ void __launch_bounds__(MODEL == BM_INERTIAL ? 256 : 512) bm_paths_f32
   P.Ga = onD ? (float)((double)S * (-bp.Fa)) : 0.f;
   P.Gb = onD ? (float)((double)S * bp.Fb) : 0.f;
   P.cn = (float)(-2.0 * M_LN2 * (double)S * (double)S * 2.0 * Dd * dtd);
+  P.s2 = (float)((double)S * (double)S * 2.0 * Dd);
   P.inv_lam_dt = (lam > 0.0) ? (float)(1.0 / (lam * dtd)) : 0.f;
   P.zeta = (float)((double)S * zet);
   P.inv_mua_dt = onD ? (float)(1.0 / (bp.mu_a * dtd)) : 0.f;
@@ -328,23 +363,32 @@ __global__ void __launch_bounds__(MODEL == BM_INERTIAL ? 256 : 512) bm_paths_f32
   int d = 0;
   if (onD) d = ((((double)wi.z + 0.5) * (1.0 / 4294967296.0)) < bp.mu_a / (bp.mu_a + bp.mu_b)) ? 1 : 0;
 
+  // Standard normal of the sub-step that ends on an event, from the third word of the event's Philox call (R13):
+  // radius from its top 23 bits, angle from its low 16 (the W16 assignment).
+  auto event_normal = [&](uint32_t w) -> float {
+    const float r = sqrt_approx(-2.0f * LN2_F * lg2_approx(u01_open0_f32(w)));
+    const float t = __uint_as_float((w & 0xFFFFu) | 0x3F800000u);
+    return r * cos_approx(fmaf(t, 128.0f * TWO_PI_F, -128.0f * TWO_PI_F));
+  };
+
   const int n_discard = (int)a.n_discard;
-  // jump clocks: (cell index, offset inside that cell); NEVER = switched off at this point
+  // next event of each stream: (cell index, offset inside that cell); NEVER = switched off at this point.  kP, kD:
+  // its index in the stream = the Philox call it came from; qP, qD: ring read slot (bits 0-3) and fill (bits 4-).
   int nP = NEVER, nD = NEVER;
-  float fP = 0.f, fD = 0.f, z = 0.f;
+  float fP = 0.f, fD = 0.f, z = 0.f, gP = 0.f, gD = 0.f;
   uint32_t kP = 0, kD = 0;
-  uint32_t gwP = 0, gwD = 0;  // Gaussian word of the sub-step that ends at the next kick / flip (R13)
+  int qP = 0, qD = 0;
   // lanes past a ragged end stay inert: no events, no checkpoint traffic (they must not steer the warp's votes)
   if (HAS_P && lam > 0.0 && valid) {
     const uint4 w = philox_call(K, g, STREAM_POISSON, 0);
-    gwP = w.z;
     schedule_f32(0, 0.f, dt, inv_dt, neg_log_u_f32(w.x) * P.inv_lam_dt, nP, fP);
     z = P.zeta * neg_log_u_f32(w.y);
+    if (HAS_G) gP = event_normal(w.z);
   }
   if (onD && valid) {
     const uint4 w = philox_call(K, g, STREAM_DICH, 0);
-    gwD = w.z;
     schedule_f32(0, 0.f, dt, inv_dt, neg_log_u_f32(w.x) * (d ? P.inv_mub_dt : P.inv_mua_dt), nD, fD);
+    if (HAS_G) gD = event_normal(w.z);
   }
 
   // drive phase in 2^-64 turns per cell (inertial): exact integer accumulation, no float time.  n is the same in
@@ -362,7 +406,8 @@ __global__ void __launch_bounds__(MODEL == BM_INERTIAL ? 256 : 512) bm_paths_f32
   float snap_x = x;
   int snap_w = wraps;
   // row f2: a launch that continues a run reloads everything the lines above initialised (the Philox calls of the
-  // initialisation are wasted then, once per launch)
+  // initialisation are wasted then, once per launch).  The rings are not part of the state: they restart empty and
+  // refill with the same events (an event is a function of its predecessor and its Philox call only).
   const int n_begin = (int)a.step_begin, n_end = (int)a.step_end;
   if (a.state != nullptr && n_begin > 0 && valid) {
     const StateIO io = state_io(a, g);
@@ -371,21 +416,110 @@ __global__ void __launch_bounds__(MODEL == BM_INERTIAL ? 256 : 512) bm_paths_f32
     io.get2(1, lo, hi); v = __uint_as_float(lo); jumps = (int)hi;
     io.get2(2, lo, hi); nP = (int)lo; fP = __uint_as_float(hi);
     io.get2(3, lo, hi); z = __uint_as_float(lo); kP = hi;
-    io.get2(4, gwP, gwD);
+    io.get2(4, lo, hi); gP = __uint_as_float(lo); gD = __uint_as_float(hi);
     io.get2(5, lo, hi); nD = (int)lo; fD = __uint_as_float(hi);
     io.get2(6, lo, hi); kD = lo; d = (int)hi;
     ph = io.get(7);
     io.get2(8, lo, hi); drive0 = __uint_as_float(lo); snap_x = __uint_as_float(hi);
     io.get2(9, lo, hi); snap_w = (int)lo;
   }
+  int cov = min(nP, nD);  // cell of the last event known to this lane, minimum over the streams
   float cst = P.base + (HAS_D ? (d ? P.Gb : P.Ga) : 0.f);
   const float hh_full = 0.5f * dt;
   // full-step constants of Alg. 1 (loop invariant; k0f, k0h follow cst across a flip)
   const float k1f = dt * P.kk1, k2f = dt * P.kk2, k1h = hh_full * P.kk1, k2h = hh_full * P.kk2;
   float k0f = dt * cst, k0h = hh_full * cst;
 
-  // ---- FAST: a full grid step without events in this lane (h = dt) --------------------------------------------
-  auto fast_cell = [&](float gr, float gc, bool do_fold) {  // noise = gr * gc
+  // ---- one refill pass: every lane with room appends one event per stream; returns whether this lane still has a
+  //      stream whose last event lies before `limit` and whose ring has room ------------------------------------
+  auto refill_pass = [&](int limit, bool &did) -> bool {
+    bool more = false;
+    int tailP = NEVER, tailD = NEVER;
+    if (HAS_P) {
+      const int rd = qP & 15, cnt = qP >> 4;
+      int tc = nP;
+      float tf = fP;
+      if (cnt > 0) {
+        const int s = (rd + cnt - 1) & (EVQ - 1);
+        tc = (int)ringP[(s * NFP + 0) * T];
+        tf = __uint_as_float(ringP[(s * NFP + 1) * T]);
+      }
+      tailP = tc;
+      if (cnt < EVQ && tc != NEVER) {
+        const uint4 w = philox_call(K, g, STREAM_POISSON, kP + (uint32_t)cnt + 1u);
+        int c;
+        float f;
+        schedule_f32(tc, tf, dt, inv_dt, neg_log_u_f32(w.x) * P.inv_lam_dt, c, f);
+        const int s = (rd + cnt) & (EVQ - 1);
+        ringP[(s * NFP + 0) * T] = (uint32_t)c;
+        ringP[(s * NFP + 1) * T] = __float_as_uint(f);
+        ringP[(s * NFP + 2) * T] = __float_as_uint(P.zeta * neg_log_u_f32(w.y));
+        if (HAS_G) ringP[(s * NFP + 3) * T] = __float_as_uint(event_normal(w.z));
+        qP += 16;
+        tailP = c;
+        did = true;
+        more |= (c < limit) && (cnt + 1 < EVQ);
+      }
+    }
+    if (HAS_D) {
+      const int rd = qD & 15, cnt = qD >> 4;
+      int tc = nD;
+      float tf = fD;
+      if (cnt > 0) {
+        const int s = (rd + cnt - 1) & (EVQ - 1);
+        tc = (int)ringD[(s * NFD + 0) * T];
+        tf = __uint_as_float(ringD[(s * NFD + 1) * T]);
+      }
+      tailD = tc;
+      if (cnt < EVQ && tc != NEVER) {
+        const uint4 w = philox_call(K, g, STREAM_DICH, kD + (uint32_t)cnt + 1u);
+        const int dn = d ^ ((cnt + 1) & 1);  // the state entered by the last queued flip
+        int c;
+        float f;
+        schedule_f32(tc, tf, dt, inv_dt, neg_log_u_f32(w.x) * (dn ? P.inv_mub_dt : P.inv_mua_dt), c, f);
+        const int s = (rd + cnt) & (EVQ - 1);
+        ringD[(s * NFD + 0) * T] = (uint32_t)c;
+        ringD[(s * NFD + 1) * T] = __float_as_uint(f);
+        if (HAS_G) ringD[(s * NFD + 2) * T] = __float_as_uint(event_normal(w.z));
+        qD += 16;
+        tailD = c;
+        did = true;
+        more |= (c < limit) && (cnt + 1 < EVQ);
+      }
+    }
+    cov = min(tailP, tailD);
+    return more;
+  };
+  // an episode: at least EVK passes (every lane with room takes part, so a pass is shared by the whole warp), then on
+  // until no lane that is still short of `limit` has room
+  auto refill_episode = [&](int limit) {
+    for (int pass = 0;; ++pass) {
+      bool did = false;
+      const bool more = refill_pass(limit, did);
+      if (!__any_sync(FULL, did)) break;
+      if (pass + 1 >= EVK && !__any_sync(FULL, more)) break;
+    }
+  };
+  auto pop_P = [&]() {
+    if ((qP >> 4) == 0) { nP = NEVER; return; }  // not reached: a popped event always has a queued successor
+    const int s = qP & 15;
+    nP = (int)ringP[(s * NFP + 0) * T];
+    fP = __uint_as_float(ringP[(s * NFP + 1) * T]);
+    z = __uint_as_float(ringP[(s * NFP + 2) * T]);
+    if (HAS_G) gP = __uint_as_float(ringP[(s * NFP + 3) * T]);
+    qP = ((qP & ~15) - 16) | ((s + 1) & (EVQ - 1));
+  };
+  auto pop_D = [&]() {
+    if ((qD >> 4) == 0) { nD = NEVER; return; }
+    const int s = qD & 15;
+    nD = (int)ringD[(s * NFD + 0) * T];
+    fD = __uint_as_float(ringD[(s * NFD + 1) * T]);
+    if (HAS_G) gD = __uint_as_float(ringD[(s * NFD + 2) * T]);
+    qD = ((qD & ~15) - 16) | ((s + 1) & (EVQ - 1));
+  };
+
+  // ---- FAST: a full grid step without events in this lane (h = dt); noise = gr * gc ----------------------------
+  auto fast_cell = [&](float gr, float gc, bool do_fold) {
     float xf = x;
     if (do_fold || POT != BM_POT_SINE2) fold_f32<POT>(xf, wraps);
     if (!INERTIAL) {
@@ -400,73 +534,73 @@ __global__ void __launch_bounds__(MODEL == BM_INERTIAL ? 256 : 512) bm_paths_f32
     }
   };
 
-  // ---- a5-a8: a sub-step of length h from the lane's current state; dr0/dr1 = drive at its two ends -----------
-  auto sub_step = [&](float h, float noise, float dr0, float dr1) {
+  // ---- a5-a8: a sub-step of length h from the lane's current state; noise = na * nb; dr0/dr1 = drive at its ends.
+  //      With h = dt, refold = false and (na, nb) = (gr, gc) this is fast_cell operation by operation, so a lane
+  //      without an event gets the same result whichever way its warp takes through a cell. -----------------------
+  auto sub_step = [&](float h, float na, float nb, float dr0, float dr1, bool refold) {
     const float hh = 0.5f * h;
-    fold_f32<POT>(x, wraps);
+    float xf = x;
+    int wf = wraps;
+    fold_f32<POT>(xf, wf);
+    if (refold || POT != BM_POT_SINE2) { wraps = wf; x = xf; } else xf = x;
     if (!INERTIAL) {
-      x = pc_overdamped_f32<POT, SINCOS>(x, x + noise, h * cst, h * P.kk1, h * P.kk2, hh * cst, hh * P.kk1, hh * P.kk2);
+      const float xs = HAS_G ? fmaf(na, nb, xf) : xf;
+      x = pc_overdamped_f32<POT, SINCOS>(xf, xs, h * cst, h * P.kk1, h * P.kk2, hh * cst, hh * P.kk1, hh * P.kk2);
     } else {
-      const float xf = x;
-      pc_inertial_f32<SINCOS>(x, v, xf, v + noise, h, hh, P.gamma, P.kk1, P.kk2, cst + dr0, cst + dr1);
+      const float vs = HAS_G ? fmaf(na, nb, v) : v;
+      pc_inertial_f32<SINCOS>(x, v, xf, vs, h, hh, P.gamma, P.kk1, P.kk2, cst + dr0, cst + dr1);
     }
   };
 
-  // ---- SLOW: a cell in which at least one lane of the warp has a kick or a flip --------------------------------
-  auto slow_cell = [&](int n, float gnoise) {
-    float tau = 0.f;         // the lane's offset inside cell n
-    float dr_tau = drive0;   // drive at that time
-    const float phf = INERTIAL ? __uint_as_float((uint32_t)(ph >> 41) | 0x3F800000u) : 0.f;  // 1 + frac(omega n dt / 2 pi)
-    // event lanes only (divergent): integrate to the event, apply it (a8), redraw its clock
-    while ((HAS_P && nP == n) || (HAS_D && nD == n)) {
-      const bool inP = HAS_P && nP == n, inD = HAS_D && nD == n;
-      const bool isP = inP && (!inD || fP <= fD);  // a tie applies the kick first (R5)
-      const float te = isP ? fP : fD;
-      const float h = fmaxf(te - tau, 0.f);
-      // Philox call k+1 of the event's stream: .x waiting time to event k+1, .y amplitude of kick k+1, .z Gaussian
-      // of the sub-step that will end at event k+1 (R13).  The sub-step that ends now uses the word drawn one event
-      // earlier, so the Philox rounds and the predictor-corrector chain are independent instruction streams.
-      const uint4 w = philox_call(K, g, isP ? STREAM_POISSON : STREAM_DICH, (isP ? kP : kD) + 1u);
-      const uint32_t gw = isP ? gwP : gwD;
-      if (isP) gwP = w.z; else gwD = w.z;
-      float noise = 0.f;
-      if (HAS_G) {
-        const float r = sqrt_approx(P.cn * lg2_approx(u01_open0_f32(gw)) * (h * inv_dt));  // Var ~ h (A9)
-        const float t = __uint_as_float((gw & 0xFFFFu) | 0x3F800000u);
-        noise = r * cos_approx(fmaf(t, 128.0f * TWO_PI_F, -128.0f * TWO_PI_F));
-      }
-      float dr1 = 0.f;
-      if (INERTIAL) dr1 = P.amp * cos_turns<SINCOS>(fmaf(te, P.w_turns, phf));
-      sub_step(h, noise, dr_tau, dr1);
-      dr_tau = dr1;
-      tau = te;
-      jumps++;
-      if (HAS_P && isP) {  // a8: kick
-        if (!INERTIAL) x += z; else v += z;
-        kP++;
-        schedule_f32(n, tau, dt, inv_dt, neg_log_u_f32(w.x) * P.inv_lam_dt, nP, fP);
-        z = P.zeta * neg_log_u_f32(w.y);
-      }
-      if (HAS_D && !isP) {  // a8: flip
-        d ^= 1;
-        kD++;
-        cst = P.base + (d ? P.Gb : P.Ga);
-        k0f = dt * cst;
-        k0h = hh_full * cst;
-        schedule_f32(n, tau, dt, inv_dt, neg_log_u_f32(w.x) * (d ? P.inv_mub_dt : P.inv_mua_dt), nD, fD);
-      }
+  // One event of this lane in cell c (the lane's earliest; a tie applies the kick first, R5): integrate to it, apply
+  // it (a8) and take the next event of that stream from the ring.
+  auto do_event = [&](float &tau, float &dr_tau, float phf) {
+    const bool isP = HAS_P && (!HAS_D || nP < nD || (nP == nD && fP <= fD));
+    const float te = isP ? fP : fD;
+    const float h = fmaxf(te - tau, 0.f);
+    float dr1 = 0.f;
+    if (INERTIAL) dr1 = P.amp * cos_turns<SINCOS>(fmaf(te, P.w_turns, phf));
+    sub_step(h, HAS_G ? (isP ? gP : gD) : 0.f, HAS_G ? sqrt_approx(h * P.s2) : 0.f, dr_tau, dr1, true);  // Var ~ h (A9)
+    dr_tau = dr1;
+    tau = te;
+    jumps++;
+    if (HAS_P && isP) {  // a8: kick
+      if (!INERTIAL) x += z; else v += z;
+      kP++;
+      pop_P();
     }
-    // every lane: the rest of the cell (the whole cell for a lane without events)
+    if (HAS_D && !isP) {  // a8: flip
+      d ^= 1;
+      kD++;
+      cst = P.base + (d ? P.Gb : P.Ga);
+      k0f = dt * cst;
+      k0h = hh_full * cst;
+      pop_D();
+    }
+  };
+
+  // ---- SLOW: a cell in which at least one lane of the warp has a kick or a flip.  Event lanes integrate up to each
+  //      of their events on their own, then every lane finishes the cell with its own remaining length (a5): the
+  //      whole cell, with the fast cell's arithmetic, for a lane without events. ----------------------------------
+  auto finish_cell = [&](float gr, float gc, float tau, float dr_tau) {
+    const bool whole = tau == 0.f;
     const float h = dt - tau;
-    float noise = 0.f;
-    if (HAS_G) noise = gnoise * ((tau == 0.f) ? 1.0f : sqrt_approx(h * inv_dt));
+    float na = gr, nb = gc;
+    if (HAS_G && !whole) { na = gr * gc; nb = sqrt_approx(h * inv_dt); }
     float drive1 = 0.f;
     if (INERTIAL) {
       ph += dph;
       drive1 = P.amp * cos_turns<SINCOS>(__uint_as_float((uint32_t)(ph >> 41) | 0x3F800000u));
     }
-    sub_step(h, noise, dr_tau, drive1);
+    sub_step(h, na, nb, dr_tau, drive1, !whole);
     drive0 = drive1;
+  };
+  auto slow_cell = [&](int c, float gr, float gc) {
+    float tau = 0.f;         // the lane's offset inside cell c
+    float dr_tau = drive0;   // drive at that time
+    const float phf = INERTIAL ? __uint_as_float((uint32_t)(ph >> 41) | 0x3F800000u) : 0.f;  // 1 + frac(omega c dt / 2 pi)
+    while ((HAS_P && nP == c) || (HAS_D && nD == c)) do_event(tau, dr_tau, phf);
+    finish_cell(gr, gc, tau, dr_tau);
   };
 
   // Events of this lane in cells [n, n+32) as a bit mask (bit = cell - n; shl.b32 clamps a shift >= 32 to zero, so
@@ -480,13 +614,12 @@ __global__ void __launch_bounds__(MODEL == BM_INERTIAL ? 256 : 512) bm_paths_f32
 
   // ---- time loop: blocks of NB cells = one Gaussian call -------------------------------------------------------
   // A block is CLEAN when no lane of the warp has an event in it and it holds neither t_i nor the end of the run:
-  // NB fast cells, one vote.  Otherwise the warp builds a uniform control word (bit j: some lane has an event in
-  // cell n+j; bit 8+j: cell n+j is the snapshot cell or lies beyond the end) and tests one bit pair per cell.
-  // The Box-Muller pair of cells (2i+2, 2i+3) is formed while cells (2i, 2i+1) run (its consumer is near, so the
-  // instruction scheduler fills the stalls of the serial predictor-corrector chain with it), and the Philox call of
-  // the next block is issued at the top of the block.
-  constexpr bool ROLLED = INERTIAL;  // non-clean blocks: one rolled copy of the cell code (measured, DESIGN.md s.6)
-  __shared__ float s_noise[ROLLED ? NB : 1][ROLLED ? 256 : 1];
+  // NB fast cells, one vote.  Otherwise the warp makes sure the block's events are queued, builds a uniform control
+  // word (bit j: some lane has an event in cell n+j; bit 8+j: cell n+j is the snapshot cell or lies beyond the end)
+  // and tests one bit pair per cell.  The Box-Muller pair of cells (2i+2, 2i+3) is formed while cells (2i, 2i+1) run
+  // (its consumer is near, so the instruction scheduler fills the stalls of the serial predictor-corrector chain with
+  // it), and the Philox call of the next block is issued at the top of the block.
+  constexpr bool UNROLLED = BM_F32_UNROLLED(INERTIAL);  // covered non-clean blocks: unrolled pair slots or a rolled slot loop
   uint4 w = make_uint4(0u, 0u, 0u, 0u);
   Pair cur = Pair{0.f, 0.f, 0.f};
   if (HAS_G) {
@@ -503,11 +636,31 @@ __global__ void __launch_bounds__(MODEL == BM_INERTIAL ? 256 : 512) bm_paths_f32
       philox_rounds<0, 10>(c, K);
     }
   };
+  // a10: the snapshot at t_i, or nothing at all beyond the end of the run (returns false)
+  auto special_cell = [&](int n, int j, unsigned ctl) -> bool {
+    if ((ctl >> j) & 0x100u) {
+      if (n + j >= n_end) return false;
+      fold_f32<POT>(x, wraps);
+      snap_x = x;
+      snap_w = wraps;
+    }
+    return true;
+  };
+  // pair I of the block's Gaussian call, or the first pair of the next one, with a run-time index (rolled slot loop)
+  auto pair_dyn = [&](const uint4 &w0, const uint4 &w1, int i) -> Pair {
+    if (GW == BM_GAUSS_W32) {
+      const bool last = i + 1 >= NP;
+      return pair_w32(last ? w1.x : w0.z, last ? w1.y : w0.w, P.cn);
+    }
+    const uint32_t ww = i == 0 ? w0.y : i == 1 ? w0.z : i == 2 ? w0.w : w1.x;
+    return GW == BM_GAUSS_W16P ? pair_w16p(ww, P.cn) : pair_w16(ww, P.cn);
+  };
+
   uint32_t blk = (uint32_t)(n_begin / NB);
   for (int n = n_begin; n < n_end; n += NB) {
     blk++;
     const bool special = ((unsigned)(n_discard - n) < (unsigned)NB) || (n + NB > n_end);
-    const bool clean = !special && !((HAS_P || HAS_D) && __any_sync(FULL, min(nP, nD) < n + NB));
+    const bool clean = !special && !(HAS_EV && __any_sync(FULL, min(nP, nD) < n + NB));
     // counter of the next Gaussian call; its ten rounds are spread over the pair slots of this block
     uint4 wn = make_uint4(blk, (uint32_t)STREAM_GAUSS, (uint32_t)g, (uint32_t)(g >> 32));
     if (clean) {
@@ -523,91 +676,97 @@ __global__ void __launch_bounds__(MODEL == BM_INERTIAL ? 256 : 512) bm_paths_f32
         cur = nxt;
       }
     } else {
+      bool careful = false;
+      if (HAS_EV && __any_sync(FULL, cov < n + NB)) {
+        refill_episode(n + NB);
+        careful = __any_sync(FULL, cov < n + NB);  // a lane with more than EVQ events in this block
+      }
       unsigned ctl = 0;
-      if (HAS_P || HAS_D) ctl = __reduce_or_sync(FULL, ev_bits(n)) & 0xFFu;
+      if (HAS_EV) ctl = __reduce_or_sync(FULL, ev_bits(n)) & 0xFFu;
       if (special) {
         if ((unsigned)(n_discard - n) < (unsigned)NB) ctl |= 0x100u << (n_discard - n);
         if (n + NB > n_end) ctl |= (0xFF00u << (n_end - n)) & 0xFF00u;
       }
       fold_f32<POT>(x, wraps);
-      if (!ROLLED) {
-        // pair slot by pair slot: a slot without event or special cell is the clean path's code for two cells
+      if (UNROLLED && !careful) {
+        // COVERED, pair slot by pair slot, unrolled: a slot without event or special cell is the clean path's code
+        // for two cells (with the next block's Philox rounds and Box-Muller pair formed alongside, as there)
 #pragma unroll
         for (int i = 0; i < NP; ++i) {
           Pair nxt = cur;
+          if (HAS_G) {
+            next_rounds(wn, i);
+            nxt = (i + 1 < NP) ? pair_of<GW>(w, i + 1, P.cn) : pair_of<GW>(wn, 0, P.cn);
+          }
           if (((ctl >> (2 * i)) & 0x303u) == 0u) {
-            if (HAS_G) {
-              next_rounds(wn, i);
-              nxt = (i + 1 < NP) ? pair_of<GW>(w, i + 1, P.cn) : pair_of<GW>(wn, 0, P.cn);
-            }
             fast_cell(cur.r, cur.c, false);
             fast_cell(cur.r, cur.s, false);
           } else {
-            if (HAS_G) {
-              next_rounds(wn, i);
-              nxt = (i + 1 < NP) ? pair_of<GW>(w, i + 1, P.cn) : pair_of<GW>(wn, 0, P.cn);
-            }
 #pragma unroll
             for (int jj = 0; jj < 2; ++jj) {
               const int j = 2 * i + jj;
-              const unsigned m = ctl >> j;
-              bool run = true;
-              if (m & 0x100u) {
-                if (n + j >= n_end) {
-                  run = false;
-                } else {  // a10: t_i
-                  fold_f32<POT>(x, wraps);
-                  snap_x = x;
-                  snap_w = wraps;
-                }
+              if (!special_cell(n, j, ctl)) break;
+              const float gc = jj ? cur.s : cur.c;
+              if (HAS_EV && ((ctl >> j) & 1u)) {
+                slow_cell(n + j, cur.r, gc);
+                ctl |= __reduce_or_sync(FULL, ev_bits(n)) & 0xFFu;  // later events of the same lanes in this block
+              } else {
+                fast_cell(cur.r, gc, false);
               }
-              if (run) {
-                const float gc = jj ? cur.s : cur.c;
-                if ((HAS_P || HAS_D) && (m & 1u)) {
-                  slow_cell(n + j, cur.r * gc);
-                  ctl |= __reduce_or_sync(FULL, ev_bits(n)) & 0xFFu;  // events re-scheduled into this block
-                } else {
-                  fast_cell(cur.r, gc, false);
-                }
+            }
+          }
+          cur = nxt;
+        }
+      } else if (!careful) {
+        // COVERED, rolled over the pair slots (one copy of the slow-cell code)
+        if (HAS_G) philox_rounds<0, 10>(wn, K);
+#pragma unroll 1
+        for (int i = 0; i < NP; ++i) {
+          Pair nxt = cur;
+          if (HAS_G) nxt = pair_dyn(w, wn, i);
+          if (((ctl >> (2 * i)) & 0x303u) == 0u) {
+            fast_cell(cur.r, cur.c, false);
+            fast_cell(cur.r, cur.s, false);
+          } else {
+#pragma unroll 1
+            for (int jj = 0; jj < 2; ++jj) {
+              const int j = 2 * i + jj;
+              if (!special_cell(n, j, ctl)) break;
+              const float gc = jj ? cur.s : cur.c;
+              if (HAS_EV && ((ctl >> j) & 1u)) {
+                slow_cell(n + j, cur.r, gc);
+                ctl |= __reduce_or_sync(FULL, ev_bits(n)) & 0xFFu;  // later events of the same lanes in this block
+              } else {
+                fast_cell(cur.r, gc, false);
               }
             }
           }
           cur = nxt;
         }
       } else {
-        // the block's NB noise values go through shared memory (each thread reads back only what it wrote: no
-        // barrier), so the cell loop stays rolled
-        if (HAS_G) {
-          philox_rounds<0, 10>(wn, K);
-#pragma unroll
-          for (int i = 0; i < NP; ++i) {
-            s_noise[2 * i][threadIdx.x] = cur.r * cur.c;
-            s_noise[2 * i + 1][threadIdx.x] = cur.r * cur.s;
-            cur = (i + 1 < NP) ? pair_of<GW>(w, i + 1, P.cn) : pair_of<GW>(wn, 0, P.cn);
-          }
-        }
+        // CAREFUL (some lane has more events in this block than its ring holds): every cell is taken as a slow cell,
+        // in turns of one event per lane with a refill before each turn, so that a lane's next event is always
+        // known before it is needed.  Same arithmetic per lane as the covered path.
+        if (HAS_G) philox_rounds<0, 10>(wn, K);
 #pragma unroll 1
-        for (int j = 0; j < NB; ++j) {
-          const unsigned m = ctl >> j;
-          if ((j & 1) == 0 && (m & 0x303u) == 0u) {  // a pair of cells without event or special cell
-            fast_cell(HAS_G ? s_noise[j][threadIdx.x] : 0.f, 1.0f, false);
-            fast_cell(HAS_G ? s_noise[j + 1][threadIdx.x] : 0.f, 1.0f, false);
-            ++j;
-            continue;
+        for (int i = 0; i < NP; ++i) {
+          Pair nxt = cur;
+          if (HAS_G) nxt = pair_dyn(w, wn, i);
+#pragma unroll 1
+          for (int jj = 0; jj < 2; ++jj) {
+            const int j = 2 * i + jj, c = n + j;
+            if (!special_cell(n, j, ctl)) break;
+            float tau = 0.f, dr_tau = drive0;
+            const float phf = INERTIAL ? __uint_as_float((uint32_t)(ph >> 41) | 0x3F800000u) : 0.f;
+            for (;;) {  // uniform over the warp
+              if (__any_sync(FULL, cov <= c)) refill_episode(c + 1);
+              const bool mine = (HAS_P && nP == c) || (HAS_D && nD == c);
+              if (!__any_sync(FULL, mine)) break;
+              if (mine) do_event(tau, dr_tau, phf);
+            }
+            finish_cell(cur.r, jj ? cur.s : cur.c, tau, dr_tau);
           }
-          if (m & 0x100u) {
-            if (n + j >= n_end) break;
-            fold_f32<POT>(x, wraps);  // a10: t_i
-            snap_x = x;
-            snap_w = wraps;
-          }
-          const float gnoise = HAS_G ? s_noise[j][threadIdx.x] : 0.f;
-          if ((HAS_P || HAS_D) && (m & 1u)) {
-            slow_cell(n + j, gnoise);
-            ctl |= __reduce_or_sync(FULL, ev_bits(n)) & 0xFFu;  // events re-scheduled into this block
-          } else {
-            fast_cell(gnoise, 1.0f, false);
-          }
+          cur = nxt;
         }
       }
     }
@@ -620,7 +779,7 @@ __global__ void __launch_bounds__(MODEL == BM_INERTIAL ? 256 : 512) bm_paths_f32
     io.put2(1, __float_as_uint(v), (uint32_t)jumps);
     io.put2(2, (uint32_t)nP, __float_as_uint(fP));
     io.put2(3, __float_as_uint(z), kP);
-    io.put2(4, gwP, gwD);
+    io.put2(4, __float_as_uint(gP), __float_as_uint(gD));
     io.put2(5, (uint32_t)nD, __float_as_uint(fD));
     io.put2(6, kD, (uint32_t)d);
     io.put(7, ph);

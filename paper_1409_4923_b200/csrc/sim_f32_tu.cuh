@@ -6,6 +6,7 @@
 
 namespace bm {
 
+#if !defined(BM_MINIMAL) || (BM_TU_SINCOS == 1 && BM_TU_GAUSS == 2)
 template <int POT>
 static KernelFn pick_noise_tu(int noise) {
   switch (noise & 7) {
@@ -20,15 +21,21 @@ static KernelFn pick_noise_tu(int noise) {
   }
 }
 
+#endif
+
 KernelFn BM_TU_PICKER(int potential, int noise) {
+#if defined(BM_MINIMAL) && (BM_TU_SINCOS != 1 || BM_TU_GAUSS != 2)
+  return nullptr; /* experiment builds (make EXTRA=-DBM_MINIMAL): the AUTO variants on the smooth potential only */
+#else
   switch (potential) {
     case BM_POT_SINE2: return pick_noise_tu<BM_POT_SINE2>(noise);
-#if BM_TU_MODEL == 0 /* BM_OVERDAMPED: the other potentials exist for the over-damped model only */
+#if BM_TU_MODEL == 0 && !defined(BM_MINIMAL) /* BM_OVERDAMPED: the other potentials exist for the over-damped model only */
     case BM_POT_PWL: return pick_noise_tu<BM_POT_PWL>(noise);
     case BM_POT_QUAD: return pick_noise_tu<BM_POT_QUAD>(noise);
 #endif
     default: return nullptr;
   }
+#endif
 }
 
 }  // namespace bm
