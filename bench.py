@@ -52,6 +52,8 @@ def parse():
     ap.add_argument("--block-threads", type=int, default=0)
     ap.add_argument("--gauss", default="auto", choices=["auto", "w32", "w16", "w16p"],
                     help="fp32: Philox words per Box-Muller pair (bm_gauss)")
+    ap.add_argument("--paths-per-thread", type=int, default=0, choices=[0, 1, 2],
+                    help="fp64: realizations per thread (bm_config.paths_per_thread; 0 = library default)")
     ap.add_argument("--scale-steps", type=float, default=1.0, help="shrink n_steps (profiling runs only; flagged)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-fp64", action="store_true")
@@ -208,9 +210,10 @@ def sincos_of(B, name):
 class Runner:
     """Device buffers of one workload + the event-timed bm_simulate call (marshalling only)."""
 
-    def __init__(self, B, torch, w, prec, sincos, block_threads, seed, dev, stream, gauss=0):
+    def __init__(self, B, torch, w, prec, sincos, block_threads, seed, dev, stream, gauss=0, paths_per_thread=0):
         self.B, self.torch, self.w, self.seed, self.stream, self.dev = B, torch, w, seed, stream, dev
-        self.cfg = B.config_for(w, prec, sincos, block_threads, gauss=gauss)
+        self.cfg = B.config_for(w, prec, sincos, block_threads, gauss=gauss,
+                                paths_per_thread=paths_per_thread if (prec == B.BM_F64 and w.scheme == 0 and w.potential == 0) else 0)
         self.params = torch.from_numpy(np.ascontiguousarray(w.params)).to(dev)
         self.stats = torch.zeros((w.n_points, 8), dtype=torch.float64, device=dev)
         self.ws = torch.empty(max(16, B.bm_workspace_bytes(self.cfg, w.n_points, w.n_paths)), dtype=torch.uint8,
@@ -268,7 +271,8 @@ def run_ours(args):
     from paper_1409_4923_b200 import replicas
     seed = replicas.replica_seed(w.seed, rank)          # replicas only: independent ensembles, no collective
     run = Runner(B, torch, w, prec, sc, args.block_threads, seed, dev, stream,
-                 {"auto": B.BM_GAUSS_AUTO, "w32": B.BM_GAUSS_W32, "w16": B.BM_GAUSS_W16, "w16p": B.BM_GAUSS_W16P}[args.gauss])
+                 {"auto": B.BM_GAUSS_AUTO, "w32": B.BM_GAUSS_W32, "w16": B.BM_GAUSS_W16, "w16p": B.BM_GAUSS_W16P}[args.gauss],
+                 args.paths_per_thread)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
     info = B.bm_kernel_info(run.cfg, w.n_points, w.n_paths)
 

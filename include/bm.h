@@ -107,6 +107,12 @@ typedef struct {
   int64_t n_discard;   /* grid steps before t_i, 0 <= n_discard < n_steps (PAPER.md:423 uses n_steps/10) */
   int64_t trace_steps; /* with out_trace: record the first trace_steps grid steps ... */
   int64_t trace_paths; /* ... of global paths 0..trace_paths-1 (BM_F64 only) */
+  int32_t paths_per_thread; /* BM_F64 jump-adapted kernels: realizations carried by one thread.  0 = library default
+                            (1: the measured-faster form); 1; 2
+                            (BM_POT_SINE2 only, else BM_ERR_UNSUPPORTED).  A path's result does not depend on it; it
+                            enters the determinism contract through the reduction tree of out_stats only.  Must be 0
+                            for BM_F32 and the paper-literal scheme. */
+  int32_t rsv;         /* 0 */
 } bm_config;
 
 /* per-path record written to out_paths: 6 doubles */

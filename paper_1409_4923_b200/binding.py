@@ -34,7 +34,8 @@ STATS_FIELDS = ("n", "mean_v", "var_v", "mean_xT", "var_xT", "mean_jumps", "mean
 class BmConfig(C.Structure):
     _fields_ = [("model", C.c_int32), ("prec", C.c_int32), ("sincos", C.c_int32), ("potential", C.c_int32),
                 ("scheme", C.c_int32), ("noise", C.c_int32), ("block_threads", C.c_int32), ("gauss", C.c_int32),
-                ("n_discard", C.c_int64), ("trace_steps", C.c_int64), ("trace_paths", C.c_int64)]
+                ("n_discard", C.c_int64), ("trace_steps", C.c_int64), ("trace_paths", C.c_int64),
+                ("paths_per_thread", C.c_int32), ("rsv", C.c_int32)]
 
 
 class BmError(RuntimeError):
@@ -109,9 +110,9 @@ def noise_mask(params):
 
 def make_config(model=BM_OVERDAMPED, prec=BM_F32, sincos=BM_SINCOS_AUTO, potential=BM_POT_SINE2,
                 scheme=BM_SCHEME_JUMP_ADAPTED, noise=BM_NOISE_GAUSS, block_threads=0, n_discard=0, trace_steps=0,
-                trace_paths=0, gauss=BM_GAUSS_AUTO):
+                trace_paths=0, gauss=BM_GAUSS_AUTO, paths_per_thread=0):
     return BmConfig(model, prec, sincos, potential, scheme, noise, block_threads, gauss, n_discard, trace_steps,
-                    trace_paths)
+                    trace_paths, paths_per_thread, 0)
 
 
 def _stream_ptr(stream):
@@ -256,18 +257,19 @@ def bm_pipe_probe(op, iters, blocks, threads, sink, stream=None):
 
 # ---- conveniences used by tests and bench.py (marshalling only) -------------------------------------------
 
-def config_for(w, prec, sincos=BM_SINCOS_AUTO, block_threads=0, trace_steps=0, trace_paths=0, gauss=BM_GAUSS_AUTO):
+def config_for(w, prec, sincos=BM_SINCOS_AUTO, block_threads=0, trace_steps=0, trace_paths=0, gauss=BM_GAUSS_AUTO,
+               paths_per_thread=0):
     """bm_config of a workloads.Workload."""
     return make_config(model=w.model, prec=prec, sincos=sincos, potential=w.potential, scheme=w.scheme,
                        noise=noise_mask(w.params), block_threads=block_threads, n_discard=w.n_discard,
-                       trace_steps=trace_steps, trace_paths=trace_paths, gauss=gauss)
+                       trace_steps=trace_steps, trace_paths=trace_paths, gauss=gauss, paths_per_thread=paths_per_thread)
 
 
 def run_workload(w, prec, want_paths=False, sincos=BM_SINCOS_AUTO, block_threads=0, trace_steps=0, trace_paths=0,
-                 device="cuda:0", gauss=BM_GAUSS_AUTO):
+                 device="cuda:0", gauss=BM_GAUSS_AUTO, paths_per_thread=0):
     """Run a Workload through bm_simulate; returns (stats[n_points,8], paths or None, trace or None) as numpy."""
     import torch
-    cfg = config_for(w, prec, sincos, block_threads, trace_steps, trace_paths, gauss)
+    cfg = config_for(w, prec, sincos, block_threads, trace_steps, trace_paths, gauss, paths_per_thread)
     dev = torch.device(device)
     params = torch.from_numpy(np.ascontiguousarray(w.params)).to(dev)
     stats = torch.zeros((w.n_points, 8), dtype=torch.float64, device=dev)

@@ -35,6 +35,7 @@ bool valid_cfg(const bm_config *c) {
   if (c->block_threads != 0 && (c->block_threads < 32 || c->block_threads > 512 || (c->block_threads & 31))) return false;
   if (c->block_threads > 256 && !(c->prec == BM_F32 && c->model == BM_OVERDAMPED && c->scheme == BM_SCHEME_JUMP_ADAPTED)) return false;
   if (c->gauss < BM_GAUSS_AUTO || c->gauss > BM_GAUSS_W16P) return false;
+  if (c->paths_per_thread < 0 || c->paths_per_thread > 2) return false;
   if (c->n_discard < 0 || c->trace_steps < 0 || c->trace_paths < 0) return false;
   return true;
 }
@@ -49,16 +50,30 @@ constexpr int DESIGN_SMS = 148;
 int max_block_threads(const bm_config *c) {
   return (c->prec == BM_F32 && c->model == BM_OVERDAMPED && c->scheme == BM_SCHEME_JUMP_ADAPTED) ? 512 : 256;
 }
+int paths_per_thread_of(const bm_config *c, int32_t n_points, int64_t n_paths);
 int block_threads_of(const bm_config *c, int32_t n_points, int64_t n_paths) {
   if (c->block_threads) return c->block_threads;
   int best = DEFAULT_BLOCK_F32;
   long long best_cost = -1;
+  const int ppt = paths_per_thread_of(c, n_points, n_paths);
   for (int bt = 128; bt <= max_block_threads(c); bt *= 2) {
-    const long long blocks = (long long)n_points * ((n_paths + bt - 1) / bt);
+    const long long blocks = (long long)n_points * ((n_paths + (long long)bt * ppt - 1) / ((long long)bt * ppt));
     const long long cost = ((blocks + DESIGN_SMS - 1) / DESIGN_SMS) * (bt / 128);  // warps on the busiest scheduler
     if (best_cost < 0 || cost <= best_cost) { best = bt; best_cost = cost; }
   }
   return best_cost > 8 ? DEFAULT_BLOCK_F32 : best;
+}
+
+// Realizations per thread of the fp64 jump-adapted kernels (sim_f64.cuh).  Two per thread exist for the smooth
+// potential as a measured choice; AUTO is one: with a fixed ensemble two chains per thread only trade warps for
+// chains (C1 131.8 ms against 103.5, C2 404.8 against 283.9).
+bool has_two_paths(const bm_config *c) {
+  return c->prec == BM_F64 && c->scheme == BM_SCHEME_JUMP_ADAPTED && c->potential == BM_POT_SINE2;
+}
+int paths_per_thread_of(const bm_config *c, int32_t n_points, int64_t n_paths) {
+  if (!has_two_paths(c)) return 1;
+  (void)n_points; (void)n_paths;
+  return c->paths_per_thread ? c->paths_per_thread : 1;
 }
 
 int resolve_sincos(const bm_config *c) {
@@ -76,6 +91,7 @@ struct Launch {
   KernelFn fn = nullptr;
   int threads = 0;  // threads per block
   int gauss = 0;    // bm_gauss selected (fp32), 0 for fp64
+  int ppt = 1;      // realizations per thread (fp64 jump-adapted kernels)
   size_t smem = 0;  // dynamic shared memory per block (event rings of the fp32 jump-adapted kernel)
 };
 
@@ -83,26 +99,32 @@ bm_status pick_kernel(const bm_config *c, int32_t n_points, int64_t n_paths, Lau
   *L = Launch();
   if (c->scheme == BM_SCHEME_PAPER_LITERAL && c->model != BM_OVERDAMPED) return BM_ERR_UNSUPPORTED;
   if (c->model == BM_INERTIAL && c->potential != BM_POT_SINE2) return BM_ERR_UNSUPPORTED;
+  if (c->paths_per_thread == 2 && !has_two_paths(c)) return BM_ERR_UNSUPPORTED;
   L->threads = block_threads_of(c, n_points, n_paths);
+  L->ppt = paths_per_thread_of(c, n_points, n_paths);
   if (c->scheme == BM_SCHEME_PAPER_LITERAL) {
     L->fn = pick_literal(c->prec, c->potential, c->noise);
   } else if (c->prec == BM_F64) {
-    L->fn = c->model == BM_OVERDAMPED ? pick_f64_overdamped(c->potential, c->noise, chunked)
-                                      : pick_f64_inertial(c->potential, c->noise, chunked);
+    L->fn = c->model == BM_OVERDAMPED ? pick_f64_overdamped(c->potential, c->noise, chunked, L->ppt)
+                                      : pick_f64_inertial(c->potential, c->noise, chunked, L->ppt);
   } else {
-    typedef KernelFn (*Picker)(int, int);
+    typedef KernelFn (*Picker)(int, int, int);
     static const Picker table[2][2][3] = {  // [model][sincos fma][gauss - 1]
         {{pick_f32_od_sfu_w32, pick_f32_od_sfu_w16, pick_f32_od_sfu_w16p},
          {pick_f32_od_fma_w32, pick_f32_od_fma_w16, pick_f32_od_fma_w16p}},
         {{pick_f32_in_sfu_w32, pick_f32_in_sfu_w16, pick_f32_in_sfu_w16p},
          {pick_f32_in_fma_w32, pick_f32_in_fma_w16, pick_f32_in_fma_w16p}}};
     L->gauss = resolve_gauss(c);
-    L->fn = table[c->model == BM_INERTIAL][resolve_sincos(c) == BM_SINCOS_FMA][L->gauss - 1](c->potential, c->noise);
+    // register class of the over-damped kernel: 64 registers once the grid is more than the ~95-register form can
+    // keep resident (5 blocks of 128 threads per SM); a function of the arguments only
+    const long long threads_total = (long long)n_points * ((n_paths + L->threads - 1) / L->threads) * L->threads;
+    const int occ = threads_total > (long long)DESIGN_SMS * 640 ? 1 : 0;
+    L->fn = table[c->model == BM_INERTIAL][resolve_sincos(c) == BM_SINCOS_FMA][L->gauss - 1](c->potential, c->noise, occ);
     L->smem = (size_t)L->threads * sizeof(uint32_t) * (size_t)f32_smem_words_per_thread(c->noise, L->gauss);
   }
   if (!L->fn) return BM_ERR_UNSUPPORTED;
   // beyond the 48 KB default a kernel has to opt in (per function and device; repeating the call is harmless)
-  if (L->smem > 48 * 1024 &&
+  if (L->smem > 44 * 1024 &&  /* the kernels also hold 1792 B of static shared memory (block reduction) */
       cudaFuncSetAttribute((const void *)L->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L->smem) != cudaSuccess) {
     cudaGetLastError();
     return BM_ERR_CUDA;
@@ -153,8 +175,8 @@ bool valid_params_host(const bm_config *c, const bm_params *p, int32_t n_points)
 }
 
 long long blocks_per_point_of(const bm_config *c, int32_t n_points, int64_t n_paths) {
-  const int bt = block_threads_of(c, n_points, n_paths);
-  return (n_paths + bt - 1) / bt;
+  const long long per_block = (long long)block_threads_of(c, n_points, n_paths) * paths_per_thread_of(c, n_points, n_paths);
+  return (n_paths + per_block - 1) / per_block;
 }
 
 }  // namespace

@@ -264,10 +264,13 @@ __device__ __forceinline__ void gauss_block_standard_f32(const PhiloxKeys &K, un
 #endif
 
 // register budget of the path kernel (experiment builds override it with -DBM_F32_MAXNREG=n)
+// OCC = 1: the over-damped kernel within 64 registers, for grids of many blocks per SM (C4: 8 instead of 5 resident
+// 128-thread blocks); OCC = 0: what the code asks for (~95 registers; no re-materialised constants), for ensembles
+// that fit the device in one wave anyway (C1).  A measured choice.
 #ifdef BM_F32_MAXNREG
-#define BM_F32_BOUNDS(model) __maxnreg__(BM_F32_MAXNREG)
+#define BM_F32_BOUNDS(model, occ) __maxnreg__(BM_F32_MAXNREG)
 #else
-#define BM_F32_BOUNDS(model) __launch_bounds__((model) == BM_INERTIAL ? 256 : 512, 1)
+#define BM_F32_BOUNDS(model, occ) __launch_bounds__((model) == BM_INERTIAL ? 256 : 512, ((model) != BM_INERTIAL && (occ)) ? 2 : 1)
 #endif
 
 // Per-point constants, fp32, theta units (theta = SCALE x)
@@ -285,8 +288,8 @@ struct PointF32 {
   float w_turns;     // omega/(2 pi): drive turns per unit time
 };
 
-template <int MODEL, int POT, int NOISE, int SINCOS, int GW>
-__global__ void BM_F32_BOUNDS(MODEL) bm_paths_f32(const __grid_constant__ SimArgs a) {
+template <int MODEL, int POT, int NOISE, int SINCOS, int GW, int OCC>
+__global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ SimArgs a) {
   constexpr bool HAS_G = NOISE & BM_NOISE_GAUSS, HAS_P = NOISE & BM_NOISE_POISSON, HAS_D = NOISE & BM_NOISE_DICH;
   constexpr bool HAS_EV = HAS_P || HAS_D;
   constexpr bool INERTIAL = MODEL == BM_INERTIAL;

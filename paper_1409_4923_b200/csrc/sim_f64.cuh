@@ -62,11 +62,35 @@ struct PointF64 {
   double A1, A2, c0, D, lambda, zeta, Fa, Fb, mu_a, mu_b, gamma, amp, omega;
 };
 
+// cos(2 pi x) for the force evaluations, branch-free (so that the chains of a thread's paths interleave) and without the
+// generality of cospi: 2x is rounded to the nearest integer k with a magic addition (|x| < 2^50), r = x - k/2 lies in
+// [-1/4, 1/4], cos 2 pi x = (-1)^k cos 2 pi r, and cos 2 pi r is a degree-12 polynomial in r^2 (interpolant at the
+// Chebyshev nodes of [0, 1/16]; approximation error 9.5e-17, evaluated in two interleaved Horner chains; absolute
+// error of the result below 3e-16, where the oracle's cos(2 pi xi) itself carries 7e-16 from rounding 2 pi xi).
+__device__ __forceinline__ double cos2pi_f64(double x) {
+  const double MAGIC = 6755399441055744.0;  // 1.5 * 2^52: (y + MAGIC) has ulp 1
+  const double t = fma(x, 2.0, MAGIC);
+  const double k = t - MAGIC;
+  const double r = fma(k, -0.5, x);
+  const double u = r * r, w = u * u;
+  double e = 2.253668089082175e-05, o = -0.00032289025049633054;
+  e = fma(e, w, 0.0037798236737849045);   o = fma(o, w, -0.03638284043309509);
+  e = fma(e, w, 0.28200596842351006);     o = fma(o, w, -1.7143907110876637);
+  e = fma(e, w, 7.903536371318447);       o = fma(o, w, -26.4262567833744);
+  e = fma(e, w, 60.24464137187666);       o = fma(o, w, -85.45681720669373);
+  e = fma(e, w, 64.9393940226683);        o = fma(o, w, -19.739208802178716);
+  e = fma(e, w, 1.0);
+  const double c = fma(o, u, e);
+  // (-1)^k: the parity of k is the lowest mantissa bit of t
+  const int hi = __double2hiint(c) ^ (__double2loint(t) << 31);
+  return __hiloint2double(hi, __double2loint(c));
+}
+
 // -V'(x) on the (nearly) folded coordinate
 template <int POT>
 __device__ __forceinline__ double minus_dV_f64(const PointF64 &P, double x) {
   if (POT == BM_POT_SINE2) {
-    const double c = cospi(2.0 * x);
+    const double c = cos2pi_f64(x);
     const double c2 = fma(2.0 * c, c, -1.0);  // cos 4 pi x = 2 cos^2 2 pi x - 1: one cosine per force evaluation
     return -(2.0 * M_PI * P.A1 * c + 4.0 * M_PI * P.A2 * c2);
   } else if (POT == BM_POT_PWL) {
@@ -102,168 +126,217 @@ __device__ __forceinline__ double unfolded_f64(const StateF64 &s) {
 }
 
 // CHUNKED: the launch may be one chunk of a run (row f2).  A separate instantiation, because the checkpoint code in
-// the same kernel changes the register allocation of the time loop (111 -> 102 registers, 6 % slower on C1).
-template <int MODEL, int POT, int NOISE, bool CHUNKED>
+// the same kernel changes the register allocation of the time loop (6 % slower on C1).
+// NPATH realizations per thread (path q of thread t in block-chunk c of a point is p = (c * NPATH + q) * blockDim + t):
+// one fp64 sub-step is a dependent chain of ~700 cycles (three software cosines behind each other), so a small
+// ensemble (C1, C2: 3.5 warps per scheduler) leaves the FP64 pipe idle most of the time; two independent chains per
+// thread fill it.  A path's arithmetic does not depend on NPATH (same operations in the same order per path).
+template <int MODEL, int POT, int NOISE, bool CHUNKED, int NPATH>
 __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimArgs a) {
   constexpr bool HAS_G = NOISE & BM_NOISE_GAUSS, HAS_P = NOISE & BM_NOISE_POISSON, HAS_D = NOISE & BM_NOISE_DICH;
   constexpr bool INERTIAL = MODEL == BM_INERTIAL;
+  constexpr int N = NPATH;
   const int point = blockIdx.x / a.blocks_per_point;
   const int chunk = blockIdx.x - point * a.blocks_per_point;
-  const long long p = (long long)chunk * blockDim.x + threadIdx.x;
-  Partial mine = partial_zero();
 
-  if (p < a.n_paths) {
-    const unsigned long long g = (unsigned long long)point * (unsigned long long)a.n_paths + (unsigned long long)p;
-    const bm_params bp = a.params[point];
-    PointF64 P;
-    P.A1 = bp.A1; P.A2 = bp.A2; P.D = HAS_G ? bp.D : 0.0;
-    P.lambda = HAS_P ? bp.lambda : 0.0; P.zeta = HAS_P ? bp.zeta : 0.0;
-    P.Fa = bp.Fa; P.Fb = bp.Fb; P.mu_a = bp.mu_a; P.mu_b = bp.mu_b;
-    P.gamma = bp.gamma; P.amp = bp.amp; P.omega = bp.omega;
-    P.c0 = bp.F - P.lambda * P.zeta;  // constant part of the drift a(x), all three stages (R6)
-    const double dt = step_length(a, point);
-    const double L0 = (POT == BM_POT_QUAD) ? 1.0 : period_f64<POT>();
+  const bm_params bp = a.params[point];
+  PointF64 P;
+  P.A1 = bp.A1; P.A2 = bp.A2; P.D = HAS_G ? bp.D : 0.0;
+  P.lambda = HAS_P ? bp.lambda : 0.0; P.zeta = HAS_P ? bp.zeta : 0.0;
+  P.Fa = bp.Fa; P.Fb = bp.Fb; P.mu_a = bp.mu_a; P.mu_b = bp.mu_b;
+  P.gamma = bp.gamma; P.amp = bp.amp; P.omega = bp.omega;
+  P.c0 = bp.F - P.lambda * P.zeta;  // constant part of the drift a(x), all three stages (R6)
+  const double dt = step_length(a, point);
+  const double L0 = (POT == BM_POT_QUAD) ? 1.0 : period_f64<POT>();
+  // a non-positive rate switches its source off at this point (lambda; mu_a: Gamma = 0, as the oracle)
+  const bool onP = HAS_P && P.lambda > 0.0;
+  const bool onD = HAS_D && P.mu_a > 0.0;
+  const long long n_end = CHUNKED ? a.step_end : a.n_steps;
+  const double amp_dt = sqrt(2.0 * P.D * dt);  // noise amplitude of an unsplit grid step (the same expression as below)
 
+  bool valid[N], tracing[N];
+  unsigned long long g[N], m[N];
+  StateF64 s[N], snap[N];
+  int d[N];
+  uint32_t kP[N], kD[N];
+  double rP[N], rD[N], z[N], rem[N], jumps[N], gq[N][4];
+  double *trace[N];
+  long long n[N];
+#pragma unroll
+  for (int q = 0; q < N; ++q) {
+    const long long p = ((long long)chunk * N + q) * blockDim.x + threadIdx.x;
+    valid[q] = p < a.n_paths;
+    g[q] = (unsigned long long)point * (unsigned long long)a.n_paths + (unsigned long long)(valid[q] ? p : 0);
     // R4: initial condition from init-stream call 0
-    const uint4 wi = philox_call(a.keys, g, STREAM_INIT, 0);
-    StateF64 s;
-    s.xi = (bp.x0_fixed >= 0.0) ? bp.x0_fixed : L0 * ((double)wi.x * (1.0 / 4294967296.0));
-    s.wraps = 0;
-    s.v = INERTIAL ? bp.v0_lo + (bp.v0_hi - bp.v0_lo) * u01_f64(wi.y) : 0.0;
-    fold_f64<POT>(s);
-    // a non-positive rate of leaving -Fa switches the dichotomous source off at this point (Gamma = 0, as the oracle)
-    const bool onD = HAS_D && P.mu_a > 0.0;
-    int d = onD ? ((u01_f64(wi.z) < P.mu_a / (P.mu_a + P.mu_b)) ? 1 : 0) : -1;
-
-    uint32_t kP = 0, kD = 0;
-    double rP = 0.0, rD = 0.0, z = 0.0;
-    bool onP = false;
-    if (HAS_P) {
-      onP = P.lambda > 0.0;  // lambda == 0 at a point of a sweep: the clock never fires
-      if (onP) {
-        const uint4 w = philox_call(a.keys, g, STREAM_POISSON, 0);
-        rP = -log(u01_f64(w.x)) / P.lambda;
-        z = -P.zeta * log(u01_f64(w.y));
-      }
+    const uint4 wi = philox_call(a.keys, g[q], STREAM_INIT, 0);
+    s[q].xi = (bp.x0_fixed >= 0.0) ? bp.x0_fixed : L0 * ((double)wi.x * (1.0 / 4294967296.0));
+    s[q].wraps = 0;
+    s[q].v = INERTIAL ? bp.v0_lo + (bp.v0_hi - bp.v0_lo) * u01_f64(wi.y) : 0.0;
+    fold_f64<POT>(s[q]);
+    d[q] = onD ? ((u01_f64(wi.z) < P.mu_a / (P.mu_a + P.mu_b)) ? 1 : 0) : -1;
+    kP[q] = 0; kD[q] = 0; rP[q] = 0.0; rD[q] = 0.0; z[q] = 0.0;
+    if (onP) {
+      const uint4 w = philox_call(a.keys, g[q], STREAM_POISSON, 0);
+      rP[q] = -log(u01_f64(w.x)) / P.lambda;
+      z[q] = -P.zeta * log(u01_f64(w.y));
     }
-    if (HAS_D && onD) {
-      const uint4 w = philox_call(a.keys, g, STREAM_DICH, 0);
-      rD = -log(u01_f64(w.x)) / (d ? P.mu_b : P.mu_a);
+    if (onD) {
+      const uint4 w = philox_call(a.keys, g[q], STREAM_DICH, 0);
+      rD[q] = -log(u01_f64(w.x)) / (d[q] ? P.mu_b : P.mu_a);
     }
-
-    const bool tracing = a.out_trace != nullptr && (long long)g < a.trace_paths;
-    double *trace = tracing ? a.out_trace + (long long)g * a.trace_steps * 2 : nullptr;
-
-    long long n = CHUNKED ? a.step_begin : 0;
-    unsigned long long m = 0;
-    double rem = dt, jumps = 0.0;
-    double gq[4] = {0.0, 0.0, 0.0, 0.0};
-    StateF64 snap = s;
-    if (CHUNKED && a.state != nullptr && a.step_begin > 0) {  // row f2: continue a run from its checkpoint
+    tracing[q] = valid[q] && a.out_trace != nullptr && (long long)g[q] < a.trace_paths;
+    trace[q] = tracing[q] ? a.out_trace + (long long)g[q] * a.trace_steps * 2 : nullptr;
+    n[q] = CHUNKED ? a.step_begin : 0;
+    m[q] = 0;
+    rem[q] = dt;
+    jumps[q] = 0.0;
+    gq[q][0] = gq[q][1] = gq[q][2] = gq[q][3] = 0.0;
+    snap[q] = s[q];
+    if (CHUNKED && a.state != nullptr && a.step_begin > 0 && valid[q]) {  // row f2: continue a run from its checkpoint
       CkptF64 c;
-      ckpt_load_f64(a, g, c);
-      s.xi = c.xi; s.wraps = c.wraps; s.v = c.v; rP = c.rP; rD = c.rD; z = c.z; kP = c.kP; kD = c.kD; d = c.d;
-      m = c.m; jumps = c.jumps; snap.xi = c.sxi; snap.wraps = c.swraps; snap.v = c.sv;
-      if (HAS_G && (m & 3ull) != 0) {
+      ckpt_load_f64(a, g[q], c);
+      s[q].xi = c.xi; s[q].wraps = c.wraps; s[q].v = c.v; rP[q] = c.rP; rD[q] = c.rD; z[q] = c.z; kP[q] = c.kP; kD[q] = c.kD;
+      d[q] = c.d; m[q] = c.m; jumps[q] = c.jumps; snap[q].xi = c.sxi; snap[q].wraps = c.swraps; snap[q].v = c.sv;
+      if (HAS_G && (m[q] & 3ull) != 0) {
         double t[4];
-        regen_gauss_block_f64(a.keys, g, (uint32_t)(m >> 2), t);
-        gq[0] = t[0]; gq[1] = t[1]; gq[2] = t[2]; gq[3] = t[3];
+        regen_gauss_block_f64(a.keys, g[q], (uint32_t)(m[q] >> 2), t);
+        gq[q][0] = t[0]; gq[q][1] = t[1]; gq[q][2] = t[2]; gq[q][3] = t[3];
       }
     }
-    const long long n_end = CHUNKED ? a.step_end : a.n_steps;
-    while (n < n_end) {
-      double h = rem;
-      if (HAS_P && onP && rP < h) h = rP;
-      if (HAS_D && onD && rD < h) h = rD;
-      double gn = 0.0;
-      if (HAS_G) {
-        if ((m & 3ull) == 0) {
-          const uint4 w = philox_call(a.keys, g, STREAM_GAUSS, (uint32_t)(m >> 2));
-          box_muller_f64(w.x, w.y, gq[0], gq[1]);
-          box_muller_f64(w.z, w.w, gq[2], gq[3]);
+    if (!valid[q]) n[q] = n_end;  // a path past the ragged end does nothing
+  }
+
+  for (;;) {
+    bool act[N], any = false;
+#pragma unroll
+    for (int q = 0; q < N; ++q) { act[q] = n[q] < n_end; any |= act[q]; }
+    if (!any) break;
+    // a5: sub-step length; a3/a4: the sub-step's Gaussian
+    double h[N], gn[N], cst[N], dxi[N];
+#pragma unroll
+    for (int q = 0; q < N; ++q) {
+      h[q] = rem[q];
+      if (onP && rP[q] < h[q]) h[q] = rP[q];
+      if (onD && rD[q] < h[q]) h[q] = rD[q];
+      gn[q] = 0.0;
+      if (HAS_G && act[q]) {
+        if ((m[q] & 3ull) == 0) {
+          const uint4 w = philox_call(a.keys, g[q], STREAM_GAUSS, (uint32_t)(m[q] >> 2));
+          box_muller_f64(w.x, w.y, gq[q][0], gq[q][1]);
+          box_muller_f64(w.z, w.w, gq[q][2], gq[q][3]);
         }
-        const int j = (int)(m & 3ull);
-        gn = (j == 0) ? gq[0] : (j == 1) ? gq[1] : (j == 2) ? gq[2] : gq[3];
+        const int j = (int)(m[q] & 3ull);
+        gn[q] = (j == 0) ? gq[q][0] : (j == 1) ? gq[q][1] : (j == 2) ? gq[q][2] : gq[q][3];
       }
-      m++;
-      const double Gd = (HAS_D && onD) ? (d ? P.Fb : -P.Fa) : 0.0;
-      const double cst = P.c0 + Gd;
-      const double dxi = HAS_G ? sqrt(2.0 * P.D * h) * gn : 0.0;
-      if (!INERTIAL) {
-        // Alg. 1
-        const double x = s.xi;
-        const double F1 = minus_dV_f64<POT>(P, x) + cst;
-        double xb = x + F1 * h + dxi;
-        double F2 = minus_dV_f64<POT>(P, xb) + cst;
-        xb = x + 0.5 * (F1 + F2) * h + dxi;
-        F2 = minus_dV_f64<POT>(P, xb) + cst;
-        s.xi = x + 0.5 * (F1 + F2) * h + dxi;
-      } else {
-        // R7: two-component version, additive noise in v only, drive evaluated at t and t+h
-        const double t = __dadd_rn(__dmul_rn((double)n, dt), __dsub_rn(dt, rem));
-        const double x = s.xi, v = s.v;
-        const double A1x = v;
-        const double A1v = -P.gamma * v + minus_dV_f64<POT>(P, x) + P.amp * cos(P.omega * t) + cst;
-        double xb = x + A1x * h, vb = v + A1v * h + dxi;
-        const double drive = P.amp * cos(P.omega * __dadd_rn(t, h));
-        double A2x = vb;
-        double A2v = -P.gamma * vb + minus_dV_f64<POT>(P, xb) + drive + cst;
-        xb = x + 0.5 * (A1x + A2x) * h;
-        vb = v + 0.5 * (A1v + A2v) * h + dxi;
-        A2x = vb;
-        A2v = -P.gamma * vb + minus_dV_f64<POT>(P, xb) + drive + cst;
-        s.xi = x + 0.5 * (A1x + A2x) * h;
-        s.v = v + 0.5 * (A1v + A2v) * h + dxi;
+      const double Gd = onD ? (d[q] ? P.Fb : -P.Fa) : 0.0;
+      cst[q] = P.c0 + Gd;
+      dxi[q] = HAS_G ? ((h[q] == dt) ? amp_dt : sqrt(2.0 * P.D * h[q])) * gn[q] : 0.0;
+    }
+    // a6 / a7: the predictor-corrector sub-step, stage by stage over the thread's paths (independent chains)
+    double xn[N], vn[N];
+    if (!INERTIAL) {
+      // Alg. 1
+      double F1[N], xb[N], F2[N];
+#pragma unroll
+      for (int q = 0; q < N; ++q) F1[q] = minus_dV_f64<POT>(P, s[q].xi) + cst[q];
+#pragma unroll
+      for (int q = 0; q < N; ++q) xb[q] = s[q].xi + F1[q] * h[q] + dxi[q];
+#pragma unroll
+      for (int q = 0; q < N; ++q) F2[q] = minus_dV_f64<POT>(P, xb[q]) + cst[q];
+#pragma unroll
+      for (int q = 0; q < N; ++q) xb[q] = s[q].xi + 0.5 * (F1[q] + F2[q]) * h[q] + dxi[q];
+#pragma unroll
+      for (int q = 0; q < N; ++q) F2[q] = minus_dV_f64<POT>(P, xb[q]) + cst[q];
+#pragma unroll
+      for (int q = 0; q < N; ++q) { xn[q] = s[q].xi + 0.5 * (F1[q] + F2[q]) * h[q] + dxi[q]; vn[q] = s[q].v; }
+    } else {
+      // R7: two-component version, additive noise in v only, drive evaluated at t and t+h
+      double A1v[N], xb[N], vb[N], drive[N], A2x[N], A2v[N];
+#pragma unroll
+      for (int q = 0; q < N; ++q) {
+        const double t = __dadd_rn(__dmul_rn((double)n[q], dt), __dsub_rn(dt, rem[q]));
+        A1v[q] = -P.gamma * s[q].v + minus_dV_f64<POT>(P, s[q].xi) + P.amp * cos(P.omega * t) + cst[q];
+        drive[q] = P.amp * cos(P.omega * __dadd_rn(t, h[q]));
       }
-      rem -= h;
-      if (HAS_P && onP) {
-        rP -= h;
-        if (rP <= 0.0) {  // kick kP (a8)
-          if (!INERTIAL) s.xi += z; else s.v += z;
-          jumps += 1.0;
-          kP++;
-          const uint4 w = philox_call(a.keys, g, STREAM_POISSON, kP);
-          rP = -log(u01_f64(w.x)) / P.lambda;
-          z = -P.zeta * log(u01_f64(w.y));
-        }
+#pragma unroll
+      for (int q = 0; q < N; ++q) { xb[q] = s[q].xi + s[q].v * h[q]; vb[q] = s[q].v + A1v[q] * h[q] + dxi[q]; }
+#pragma unroll
+      for (int q = 0; q < N; ++q) { A2x[q] = vb[q]; A2v[q] = -P.gamma * vb[q] + minus_dV_f64<POT>(P, xb[q]) + drive[q] + cst[q]; }
+#pragma unroll
+      for (int q = 0; q < N; ++q) {
+        xb[q] = s[q].xi + 0.5 * (s[q].v + A2x[q]) * h[q];
+        vb[q] = s[q].v + 0.5 * (A1v[q] + A2v[q]) * h[q] + dxi[q];
       }
-      if (HAS_D && onD) {
-        rD -= h;
-        if (rD <= 0.0) {  // flip
-          d = 1 - d;
-          jumps += 1.0;
-          kD++;
-          const uint4 w = philox_call(a.keys, g, STREAM_DICH, kD);
-          rD = -log(u01_f64(w.x)) / (d ? P.mu_b : P.mu_a);
-        }
-      }
-      fold_f64<POT>(s);
-      if (rem <= 0.0) {
-        n++;
-        rem = dt;
-        if (tracing && n <= a.trace_steps) {
-          trace[2 * (n - 1)] = unfolded_f64<POT>(s);
-          trace[2 * (n - 1) + 1] = s.v;
-        }
-        if (n == a.n_discard) snap = s;
+#pragma unroll
+      for (int q = 0; q < N; ++q) { A2x[q] = vb[q]; A2v[q] = -P.gamma * vb[q] + minus_dV_f64<POT>(P, xb[q]) + drive[q] + cst[q]; }
+#pragma unroll
+      for (int q = 0; q < N; ++q) {
+        xn[q] = s[q].xi + 0.5 * (s[q].v + A2x[q]) * h[q];
+        vn[q] = s[q].v + 0.5 * (A1v[q] + A2v[q]) * h[q] + dxi[q];
       }
     }
+    // a8, a9 and the bookkeeping of the grid step, path by path
+#pragma unroll
+    for (int q = 0; q < N; ++q) {
+      if (!act[q]) continue;
+      s[q].xi = xn[q];
+      s[q].v = vn[q];
+      m[q]++;
+      rem[q] -= h[q];
+      if (onP) {
+        rP[q] -= h[q];
+        if (rP[q] <= 0.0) {  // kick kP (a8)
+          if (!INERTIAL) s[q].xi += z[q]; else s[q].v += z[q];
+          jumps[q] += 1.0;
+          kP[q]++;
+          const uint4 w = philox_call(a.keys, g[q], STREAM_POISSON, kP[q]);
+          rP[q] = -log(u01_f64(w.x)) / P.lambda;
+          z[q] = -P.zeta * log(u01_f64(w.y));
+        }
+      }
+      if (onD) {
+        rD[q] -= h[q];
+        if (rD[q] <= 0.0) {  // flip
+          d[q] = 1 - d[q];
+          jumps[q] += 1.0;
+          kD[q]++;
+          const uint4 w = philox_call(a.keys, g[q], STREAM_DICH, kD[q]);
+          rD[q] = -log(u01_f64(w.x)) / (d[q] ? P.mu_b : P.mu_a);
+        }
+      }
+      fold_f64<POT>(s[q]);
+      if (rem[q] <= 0.0) {
+        n[q]++;
+        rem[q] = dt;
+        if (tracing[q] && n[q] <= a.trace_steps) {
+          trace[q][2 * (n[q] - 1)] = unfolded_f64<POT>(s[q]);
+          trace[q][2 * (n[q] - 1) + 1] = s[q].v;
+        }
+        if (n[q] == a.n_discard) snap[q] = s[q];
+      }
+    }
+  }
+
+  Partial mine = partial_zero();
+#pragma unroll
+  for (int q = 0; q < N; ++q) {
+    if (!valid[q]) continue;
     if (CHUNKED && a.state != nullptr) {  // row f2: checkpoint (chunks end on completed grid steps, so rem = dt)
       CkptF64 c;
-      c.xi = s.xi; c.wraps = s.wraps; c.v = s.v; c.rP = rP; c.rD = rD; c.z = z; c.kP = kP; c.kD = kD; c.d = d;
-      c.m = m; c.jumps = jumps; c.sxi = snap.xi; c.swraps = snap.wraps; c.sv = snap.v;
-      ckpt_store_f64(a, g, c);
+      c.xi = s[q].xi; c.wraps = s[q].wraps; c.v = s[q].v; c.rP = rP[q]; c.rD = rD[q]; c.z = z[q]; c.kP = kP[q]; c.kD = kD[q];
+      c.d = d[q]; c.m = m[q]; c.jumps = jumps[q]; c.sxi = snap[q].xi; c.swraps = snap[q].wraps; c.sv = snap[q].v;
+      ckpt_store_f64(a, g[q], c);
     }
     // a10: eq. (30)
     const double span = (double)(a.n_steps - a.n_discard) * dt;
-    const double xT = unfolded_f64<POT>(s);
-    const double vbar = ((double)(s.wraps - snap.wraps) * period_f64<POT>() + (s.xi - snap.xi)) / span;
+    const double xT = unfolded_f64<POT>(s[q]);
+    const double vbar = ((double)(s[q].wraps - snap[q].wraps) * period_f64<POT>() + (s[q].xi - snap[q].xi)) / span;
     if (a.out_paths && (!CHUNKED || a.step_end >= a.n_steps)) {
-      double *o = a.out_paths + g * BM_OUT_STRIDE;
-      o[BM_OUT_XT] = xT; o[BM_OUT_VT] = s.v; o[BM_OUT_VBAR] = vbar; o[BM_OUT_JUMPS] = jumps;
-      o[BM_OUT_SUBSTEPS] = (double)m; o[BM_OUT_XTI] = unfolded_f64<POT>(snap);
+      double *o = a.out_paths + g[q] * BM_OUT_STRIDE;
+      o[BM_OUT_XT] = xT; o[BM_OUT_VT] = s[q].v; o[BM_OUT_VBAR] = vbar; o[BM_OUT_JUMPS] = jumps[q];
+      o[BM_OUT_SUBSTEPS] = (double)m[q]; o[BM_OUT_XTI] = unfolded_f64<POT>(snap[q]);
     }
-    mine = leaf(vbar, xT, jumps, (double)m);
+    mine = merge(mine, leaf(vbar, xT, jumps[q], (double)m[q]));
   }
   if (CHUNKED && a.step_end < a.n_steps) return;  // not the last chunk: the partials are not used (uniform over the grid)
   block_reduce_store(mine, a.partials + (long long)blockIdx.x * PARTIAL_STRIDE);

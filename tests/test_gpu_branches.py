@@ -162,3 +162,41 @@ def test_chunked_ragged_ensemble_of_several_waves(B, prec):
         assert np.array_equal(paths.cpu().numpy(), p0), f"{prec}: chunked run differs from the single launch (rep {rep})"
         assert np.array_equal(stats.cpu().numpy(), s0)
     assert p0[:, B.BM_OUT_JUMPS].mean() > 2.5
+
+
+@pytest.mark.parametrize("name", ["C1", "C2", "od-all", "in-all-dense"])
+def test_fp64_two_paths_per_thread_give_the_same_paths(B, name):
+    """bm_config.paths_per_thread = 2 (fp64 kernels: two independent chains per thread) is the same computation per path
+    as one per thread; only the reduction tree of the statistics changes.  Also for a chunked run and a ragged end."""
+    import torch
+    w = {"C1": lambda: W.c1().scaled(n_paths=777, n_steps=3000), "C2": lambda: W.c2().scaled(n_paths=333, n_steps=2400),
+         "od-all": lambda: od_case(7, True, n_paths=300, n_steps=800), "in-all-dense": lambda: inertial_case(7, 300, 800, True)}[name]()
+    s1, p1, _ = B.run_workload(w, B.BM_F64, want_paths=True, paths_per_thread=1)
+    s2, p2, _ = B.run_workload(w, B.BM_F64, want_paths=True, paths_per_thread=2)
+    assert np.array_equal(p1[:, [B.BM_OUT_JUMPS, B.BM_OUT_SUBSTEPS]], p2[:, [B.BM_OUT_JUMPS, B.BM_OUT_SUBSTEPS]])
+    assert np.abs(p1 - p2).max() <= 1e-13 * (1 + np.abs(p1).max()), np.abs(p1 - p2).max()
+    assert np.allclose(s1, s2, rtol=1e-12, atol=1e-13)
+    _, p3, _ = B.run_workload(w, B.BM_F64, want_paths=True, paths_per_thread=2, block_threads=64)
+    assert np.array_equal(p2, p3)
+    cfg = B.config_for(w, B.BM_F64, paths_per_thread=2)
+    dev = torch.device("cuda:0")
+    params = torch.from_numpy(np.ascontiguousarray(w.params)).to(dev)
+    stats = torch.zeros((1, 8), dtype=torch.float64, device=dev)
+    paths = torch.zeros((w.n_paths, B.BM_OUT_STRIDE), dtype=torch.float64, device=dev)
+    state = torch.zeros(B.bm_state_bytes(cfg, 1, w.n_paths), dtype=torch.uint8, device=dev)
+    for b in range(0, w.n_steps, 800):
+        B.bm_simulate_chunk(cfg, params, 1, w.n_paths, w.n_steps, w.dt, w.seed, b, min(800, w.n_steps - b), state, stats, paths)
+    torch.cuda.synchronize()
+    assert np.array_equal(paths.cpu().numpy(), p2) and np.array_equal(stats.cpu().numpy(), s2)
+
+
+def test_paths_per_thread_is_an_fp64_option(B):
+    import torch
+    w = W.c1().scaled(n_paths=64, n_steps=16)
+    params = torch.from_numpy(np.ascontiguousarray(w.params)).cuda()
+    stats = torch.zeros((1, 8), dtype=torch.float64, device="cuda")
+    for kw in (dict(prec=B.BM_F32), dict(prec=B.BM_F64, potential=B.BM_POT_PWL), dict(prec=B.BM_F64, scheme=B.BM_SCHEME_PAPER_LITERAL)):
+        c = B.make_config(**{**dict(noise=3, paths_per_thread=2), **kw})
+        with pytest.raises(B.BmError) as e:
+            B.bm_simulate(c, params, 1, w.n_paths, w.n_steps, w.dt, w.seed, stats)
+        assert e.value.status == B.BM_ERR_UNSUPPORTED
