@@ -37,7 +37,7 @@ XU_OPS_PER_SUBSTEP = {0: 5.0, 1: 6.0}
 XU_LANES_PER_SM = 16          # MUFU lanes per SM per clock (4 per SM sub-partition); confirmed by bm_pipe_probe
 # dram__bytes_read.sum + dram__bytes_write.sum of one path-kernel launch from the committed `ncu --set full` captures
 # (profiles/r1_f32_v5.md): parameters and per-block partials only, the path is register-resident.  Bytes per launch.
-NCU_DRAM_BYTES = {("C1", "f32"): 58880, ("C2", "f32"): 37376}
+NCU_DRAM_BYTES = {("C1", "f32"): 68864, ("C2", "f32"): 56064}
 
 
 def parse():
@@ -57,6 +57,9 @@ def parse():
     ap.add_argument("--scale-steps", type=float, default=1.0, help="shrink n_steps (profiling runs only; flagged)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-fp64", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config block of the default run")
+    ap.add_argument("--probe-pipes", action="store_true",
+                    help="measure the SM's pipe throughputs with bm_pipe_probe and print them as one JSON object")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
     return ap.parse_args()
 
@@ -137,13 +140,13 @@ class ClockSampler:
 
 # ---- the oracle, timed as it stands (cpu_baseline leg and --impl reference) -----------------------------------
 
-def oracle_time_sample(w, n_sample_paths):
+def oracle_time_sample(w, n_sample_paths, threads=0):
     """Oracle on the first n_sample_paths global paths of w at full length; returns seconds."""
     from oracle import bm_oracle as orc
     ids = np.arange(n_sample_paths, dtype=np.int64)
     t0 = time.perf_counter()
     orc.simulate(w.params, w.n_paths, w.n_steps, w.dt, w.seed, model=w.model, potential=w.potential,
-                 scheme=w.scheme, n_discard=w.n_discard, ids=ids)
+                 scheme=w.scheme, n_discard=w.n_discard, ids=ids, threads=threads)
     return time.perf_counter() - t0
 
 
@@ -170,9 +173,16 @@ def cpu_baseline(w, target_seconds):
     if t < 0.7 * target_seconds and n < total:      # the two-paths-per-core calibration overestimates the cost
         n = min(total, max(cores, int(n * target_seconds / max(t, 1e-3)) // cores * cores))
         t = oracle_time_sample(w, n)
-    return {"value": n * w.n_steps / t, "unit": UNIT, "cores": int(orc.threads_used() or cores), "kind": "oracle",
+    used = int(orc.threads_used() or cores)
+    # one core, as the paper's own comparison: a sample of about a third of the time
+    n1 = max(1, int(n / max(used, 1) / 3))
+    t1 = oracle_time_sample(w, n1, threads=1)
+    return {"value": n * w.n_steps / t, "unit": UNIT, "cores": used, "kind": "oracle",
             "sample": f"first {n} of {total} paths of {w.name} at full length "
-                      f"({w.n_steps} grid steps), fp64, gcc -O2 + OpenMP, {t:.1f} s"}
+                      f"({w.n_steps} grid steps), fp64, gcc -O2 + OpenMP, {t:.1f} s",
+            "value_1core": n1 * w.n_steps / t1,
+            "sample_1core": f"first {n1} paths of {w.name} at full length on one thread, {t1:.1f} s (PAPER.md:437 compares "
+                            "with one CPU core)"}
 
 
 def run_reference(args):
@@ -247,9 +257,77 @@ class Runner:
         return max(e0.elapsed_time(e1), 1e3 * (time.perf_counter() - t0))
 
 
+# FP64-pipe instructions per sub-step of the fp64 kernels as built (sm__inst_executed_pipe_fp64 of the committed
+# `ncu --set full` captures / warp sub-steps, profiles/r2_f64.md): the count the fp64 roofline fraction is formed with.
+FP64_OPS_PER_SUBSTEP = {0: 136.0, 1: 190.0}
+FP64_LANES_PER_SM = 64        # DFMA lanes per SM per clock (bm_pipe_probe: 63)
+
+
+def roofline_of(B, w, prec_name, stats, ms_per_step, clocks, info):
+    """Roofline of the path kernel (the grid pass is < 0.1 % of a step).  fp32: bound by the XU (MUFU) pipe, algorithmic
+    operation count; fp64: the FP64 pipe, instruction count of the kernel as built.  Peak = lanes x SMs x the SM clock
+    SAMPLED during the timed region (falls back to the maximum clock when nvidia-smi gave nothing)."""
+    substeps = float(stats[:, 6].mean())                # counted by the kernel
+    jumps = float(stats[:, 5].mean())
+    sm_mhz = clocks.get("sm_mhz") or clocks.get("sm_max_mhz") or 1965.0
+    if prec_name == "f32":
+        per_path = XU_OPS_PER_SUBSTEP[w.model] * substeps + 2.0 * jumps
+        if w.scheme == 1:   # the paper's scheme as printed: no Gaussian transcendental; 3 force cosines only for SINE2
+            per_path = (3.0 if w.potential == 0 else 0.0) * substeps + 2.0 * jumps
+        lanes, pipe = XU_LANES_PER_SM, "xu (MUFU)"
+        what = "algorithmic MUFU-class operations (DESIGN.md section 6)"
+    else:
+        per_path = FP64_OPS_PER_SUBSTEP[w.model] * substeps
+        lanes, pipe = FP64_LANES_PER_SM, "fp64"
+        what = "FP64-pipe instructions of the kernel as built (profiles/r2_f64.md)"
+    ops = per_path * w.n_points * w.n_paths
+    peak = lanes * info["sm_count"] * sm_mhz * 1e6 / 1e9
+    achieved = ops / (ms_per_step * 1e-3) / 1e9
+    return {"bound": "alu", "pipe": pipe, "achieved": achieved, "peak": peak, "unit": "Gop/s", "frac": achieved / peak,
+            "ops_per_path_step": per_path / w.n_steps, "ops_counted": what,
+            "peak_source": f"derived: {lanes} lanes/SM/clk x {info['sm_count']} SMs x {sm_mhz:.0f} MHz (SM clock sampled "
+                           "during the timed region; lane counts confirmed by bm_pipe_probe, profiles/pipes_r2.json)",
+            "kernel_ms": ms_per_step, "regs_per_thread": info["regs_per_thread"],
+            "launch_threads": info["launch_threads"], "blocks_per_sm": info["blocks_per_sm"],
+            "substeps_per_step": substeps / w.n_steps}
+
+
+def measure(B, torch, w, prec_name, args, seed, dev, stream, flush, steps, warmup, barrier, sampler_index, sincos=0, gauss=0,
+            block_threads=0, paths_per_thread=0):
+    """W warm-up steps, then K timed steps of one workload (CUDA events on the launching stream, L2 flush between
+    steps outside the event pairs, clocks sampled during the timed region).  Returns (Runner, ms list, clocks, stats)."""
+    prec = B.BM_F32 if prec_name == "f32" else B.BM_F64
+    run = Runner(B, torch, w, prec, sincos, block_threads, seed, dev, stream, gauss, paths_per_thread)
+    for _ in range(max(warmup, 0)):
+        run.device_step()
+    sampler = ClockSampler(sampler_index)
+    sampler.start()
+    time.sleep(0.25)
+    barrier()
+    t0 = time.time()
+    ms = []
+    for _ in range(steps):
+        flush.zero_()                                   # L2 flush, outside the event pair
+        torch.cuda.synchronize(dev)
+        ms.append(run.device_step())
+    barrier()
+    t1 = time.time()
+    if t1 - t0 < 0.3:                                   # give nvidia-smi (20 ms period) something to sample under load
+        t_hold = time.time()
+        while time.time() - t_hold < 0.3:
+            run.device_step()
+        torch.cuda.synchronize(dev)
+        t1 = time.time()
+    clocks = sampler.stop(t0, t1)
+    return run, ms, clocks, run.stats.cpu().numpy().copy()
+
+
+PER_CONFIG = (("C0", "f32"), ("C2", "f32"), ("C3", "f32"), ("C4", "f32"), ("C1", "f64"), ("C2", "f64"))
+
+
 def run_ours(args):
     import torch
-    from paper_1409_4923_b200 import binding as B
+    from paper_1409_4923_b200 import binding as B, workloads as W
     B.lib()                                             # raises when libbm.so is missing: there is no fallback
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the product has no CPU path)")
@@ -266,15 +344,11 @@ def run_ours(args):
     torch.cuda.set_device(dev)
     stream = torch.cuda.Stream(device=dev)
     w = workload_of(args)
-    prec = B.BM_F32 if args.prec == "f32" else B.BM_F64
     sc = sincos_of(B, args.sincos)
+    gs = {"auto": B.BM_GAUSS_AUTO, "w32": B.BM_GAUSS_W32, "w16": B.BM_GAUSS_W16, "w16p": B.BM_GAUSS_W16P}[args.gauss]
     from paper_1409_4923_b200 import replicas
     seed = replicas.replica_seed(w.seed, rank)          # replicas only: independent ensembles, no collective
-    run = Runner(B, torch, w, prec, sc, args.block_threads, seed, dev, stream,
-                 {"auto": B.BM_GAUSS_AUTO, "w32": B.BM_GAUSS_W32, "w16": B.BM_GAUSS_W16, "w16p": B.BM_GAUSS_W16P}[args.gauss],
-                 args.paths_per_thread)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-    info = B.bm_kernel_info(run.cfg, w.n_points, w.n_paths)
 
     def barrier():
         torch.cuda.synchronize(dev)
@@ -282,22 +356,9 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize(dev)
 
-    for _ in range(max(args.warmup, 0)):
-        run.device_step()
-    sampler = ClockSampler(local_rank)
-    sampler.start()
-    time.sleep(0.25)
-    barrier()
-    t_wall0 = time.time()
-    ms = []
-    for _ in range(args.steps):
-        flush.zero_()                                   # L2 flush, outside the event pair
-        torch.cuda.synchronize(dev)
-        ms.append(run.device_step())
-    barrier()
-    t_wall1 = time.time()
-    clocks = sampler.stop(t_wall0, t_wall1)
-    stats = run.stats.cpu().numpy().copy()
+    run, ms, clocks, stats = measure(B, torch, w, args.prec, args, seed, dev, stream, flush, args.steps, args.warmup, barrier,
+                                     local_rank, sc, gs, args.block_threads, args.paths_per_thread)
+    info = B.bm_kernel_info(run.cfg, w.n_points, w.n_paths)
     total_ms = replicas.max_over_ranks(float(sum(ms)), dist, dev)   # timing plumbing only (max over ranks)
     ms_per_step = total_ms / args.steps
     value = replicas.whole_job_value(w.path_steps, world, ms_per_step)
@@ -318,13 +379,7 @@ def run_ours(args):
             dist.destroy_process_group()
         return 0
 
-    # roofline of the dominant kernel (the path kernel; the grid pass is < 0.1 % of the step): "alu" bound, XU pipe
-    substeps = float(stats[:, 6].mean())                # counted by the kernel
-    jumps = float(stats[:, 5].mean())
-    xu_per_path = XU_OPS_PER_SUBSTEP[w.model] * substeps + 2.0 * jumps
-    if w.scheme == 1:   # the paper's scheme as printed: no Gaussian transcendental; 3 force cosines only for SINE2
-        xu_per_path = (3.0 if w.potential == 0 else 0.0) * substeps + 2.0 * jumps
-    xu_ops = xu_per_path * w.n_points * w.n_paths       # algorithmic MUFU-class ops per launch (fp32 accounting)
+    roof = roofline_of(B, w, args.prec, stats, ms_per_step, clocks, info)
     # the XU peak measured live with the library's probe kernel (8 independent MUFU chains per thread), beside the
     # derived one: lane-operations per second of MUFU.COS on this device at its current clocks
     sink = torch.zeros(info["sm_count"] * 4 * 256, dtype=torch.float32, device=dev)
@@ -332,40 +387,56 @@ def run_ours(args):
     for r in range(3):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
-        B.bm_pipe_probe(B.BM_PROBE_MUFU_COS, 1000, info["sm_count"] * 4, 256, sink)
+        B.bm_pipe_probe(B.BM_PROBE_MUFU_COS if args.prec == "f32" else B.BM_PROBE_DFMA, 1000, info["sm_count"] * 4, 256, sink)
         e1.record()
         e1.synchronize()
         probe_ms.append(e0.elapsed_time(e1))
-    peak_probe = info["sm_count"] * 4 * 256 * 1000 * 64 / (min(probe_ms) * 1e-3) / 1e9
-    sm_mhz = clocks.get("sm_max_mhz") or 1965.0
-    peak = XU_LANES_PER_SM * info["sm_count"] * sm_mhz * 1e6 / 1e9
-    achieved = xu_ops / (ms_per_step * 1e-3) / 1e9
-    roof = {"bound": "alu", "pipe": "xu (MUFU) for fp32; fp64 runs the same algorithm on the FP64 pipe",
-            "achieved": achieved, "peak": peak, "unit": "Gop/s", "frac": achieved / peak,
-            "peak_probe": peak_probe, "frac_of_probe": achieved / peak_probe,
-            "traffic": NCU_DRAM_BYTES.get((w.name, args.prec)) if args.scale_steps == 1.0 else None,
-            "traffic_source": "profiles/r1_f32_v5.md (ncu --set full, dram bytes of one launch; independent of n_steps)",
-            "peak_source": f"derived: {XU_LANES_PER_SM} MUFU lanes/SM/clk x {info['sm_count']} SMs x {sm_mhz:.0f} MHz "
-                           "(max SM clock; lane count confirmed by bm_pipe_probe, DESIGN.md section 6)",
-            "ops_per_path_step": xu_per_path / w.n_steps, "kernel": "bm_paths_literal" if w.scheme == 1 else ("bm_paths_f32" if prec == B.BM_F32 else "bm_paths_f64"),
-            "kernel_ms": ms_per_step, "regs_per_thread": info["regs_per_thread"],
-            "launch_threads": info["launch_threads"], "gauss": {1: "w32", 2: "w16", 3: "w16p"}.get(info["gauss"], "n/a"),
-            "blocks_per_sm": info["blocks_per_sm"]}
+    roof["peak_probe"] = info["sm_count"] * 4 * 256 * 1000 * 64 / (min(probe_ms) * 1e-3) / 1e9
+    roof["frac_of_probe"] = roof["achieved"] / roof["peak_probe"]
+    roof["traffic"] = NCU_DRAM_BYTES.get((w.name, args.prec)) if args.scale_steps == 1.0 else None
+    roof["traffic_source"] = ("a constant from the committed ncu --set full capture of this kernel (profiles/, dram bytes of "
+                              "one launch: parameters and per-block partials; independent of n_steps), not read in this run")
+    roof["kernel"] = "bm_paths_literal" if w.scheme == 1 else ("bm_paths_f32" if args.prec == "f32" else "bm_paths_f64")
+    roof["gauss"] = {1: "w32", 2: "w16", 3: "w16p"}.get(info["gauss"], "n/a")
+    jumps = float(stats[:, 5].mean())
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": args.prec, "data": "synthetic",
             "config": workload_config(w, args, {"parallelism": "replicas only" if world > 1 else "single GPU",
-                                                "sincos": args.sincos, "substeps_per_step": substeps / w.n_steps}),
+                                                "sincos": args.sincos, "substeps_per_step": roof["substeps_per_step"]}),
             "ms_median": float(np.median(ms)), "ms_best": float(min(ms)),
-            "substeps_per_s": world * substeps * w.n_points * w.n_paths / (ms_per_step * 1e-3),
+            "substeps_per_s": world * roof["substeps_per_step"] * w.path_steps / (ms_per_step * 1e-3),
             "clocks": clocks, "e2e": e2e, "gpu_launches": 2 * args.steps, "roofline": roof,
             "result": {"mean_v": float(stats[0, 1]), "var_v": float(stats[0, 2]), "mean_jumps": jumps}}
 
-    if world == 1 and not args.no_fp64 and args.prec == "f32":
+    # every BASELINE.json config and both precisions beside the headline (3 warm-up + 3 timed full-size steps each)
+    if world == 1 and not args.no_per_config and args.scale_steps == 1.0 and args.workload == "C1" and args.prec == "f32":
+        per = {}
+        launches = 0
+        for name, pn in PER_CONFIG:
+            wc = W.CONFIGS[name]()
+            r2, ms2, ck2, st2 = measure(B, torch, wc, pn, args, wc.seed, dev, stream, flush, 3, 3, barrier, local_rank)
+            i2 = B.bm_kernel_info(r2.cfg, wc.n_points, wc.n_paths)
+            mps = float(np.mean(ms2))
+            rf = roofline_of(B, wc, pn, st2, mps, ck2, i2)
+            per[f"{name}_{pn}"] = {"workload": name, "dtype": pn, "n_points": int(wc.n_points), "n_paths_per_point": int(wc.n_paths),
+                                   "n_steps": int(wc.n_steps), "steps": 3, "warmup": 3, "ms_per_step": mps,
+                                   "ms_best": float(min(ms2)), "value": wc.path_steps / (mps * 1e-3), "unit": UNIT,
+                                   "roofline": {k: rf[k] for k in ("pipe", "achieved", "peak", "unit", "frac", "ops_per_path_step",
+                                                                   "regs_per_thread", "launch_threads", "blocks_per_sm",
+                                                                   "substeps_per_step")},
+                                   "clocks": ck2, "mean_v_point0": float(st2[0, 1])}
+            launches += 2 * 6
+            del r2
+        line["per_config"] = per
+        line["gpu_launches"] += launches
+        line["fp64"] = {"value": per["C1_f64"]["value"], "unit": UNIT, "ms_per_step": per["C1_f64"]["ms_per_step"],
+                        "frac_fp64_pipe": per["C1_f64"]["roofline"]["frac"]}
+    elif world == 1 and not args.no_fp64 and args.prec == "f32":
         r64 = Runner(B, torch, w, B.BM_F64, sc, args.block_threads, seed, dev, stream)
         r64.device_step()
-        m64 = [r64.device_step() for _ in range(2)]
-        line["fp64"] = {"value": w.path_steps / (min(m64) * 1e-3), "unit": UNIT, "ms_per_step": float(min(m64)),
+        m64 = [r64.device_step() for _ in range(3)]
+        line["fp64"] = {"value": w.path_steps / (float(np.mean(m64)) * 1e-3), "unit": UNIT, "ms_per_step": float(np.mean(m64)),
                         "mean_v": float(r64.stats.cpu().numpy()[0, 1])}
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(w, args.cpu_seconds)
@@ -375,8 +446,51 @@ def run_ours(args):
     return 0
 
 
+def probe_pipes():
+    """Throughput of the SM's arithmetic pipes measured with the library's probe kernels (bm_pipe_probe): warp
+    instructions of one kind, 8 independent chains per thread, 4 blocks of 256 threads per SM.  Printed as
+    lane-operations per SM and clock at the SM clock sampled during the probes (profiles/pipes_r2.json)."""
+    import torch
+    from paper_1409_4923_b200 import binding as B
+    dev = torch.device("cuda", 0)
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    names = {B.BM_PROBE_FFMA: "FFMA", B.BM_PROBE_MUFU_COS: "MUFU.COS", B.BM_PROBE_MUFU_LG2: "MUFU.LG2",
+             B.BM_PROBE_MUFU_SQRT: "MUFU.SQRT", B.BM_PROBE_IMAD_WIDE: "IMAD.WIDE.U32", B.BM_PROBE_LOP3: "LOP3",
+             B.BM_PROBE_DFMA: "DFMA", B.BM_PROBE_I2F: "I2F", B.BM_PROBE_FADD: "FADD", B.BM_PROBE_MIX: "MUFU+IMAD.WIDE mix"}
+    sink = torch.zeros(sms * 4 * 256, dtype=torch.float32, device=dev)
+    iters = 2000
+    sampler = ClockSampler(0)
+    sampler.start()
+    time.sleep(0.25)
+    t0 = time.time()
+    best = {}
+    for op, nm in names.items():
+        for rep in range(4):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            B.bm_pipe_probe(op, iters, sms * 4, 256, sink)
+            e1.record()
+            e1.synchronize()
+            if rep:
+                best[nm] = min(best.get(nm, 1e30), e0.elapsed_time(e1))
+    t1 = time.time()
+    clocks = sampler.stop(t0, t1)
+    mhz = clocks.get("sm_mhz") or 1965.0
+    ops = sms * 4 * 256 * iters * 64
+    table = {nm: {"ms": ms, "Gop_per_s": ops / (ms * 1e-3) / 1e9,
+                  "lane_ops_per_sm_per_clk": ops / (ms * 1e-3) / (sms * mhz * 1e6),
+                  "cycles_per_warp_instr_per_subpartition": 32.0 / (ops / (ms * 1e-3) / (sms * mhz * 1e6) / 4.0)}
+             for nm, ms in best.items()}
+    print(json.dumps({"what": "bm_pipe_probe throughputs", "gpu": torch.cuda.get_device_name(dev), "sm_count": sms,
+                      "launch": f"{sms * 4} blocks x 256 threads x {iters} x 64 operations per thread", "clocks": clocks,
+                      "pipes": table}, indent=1))
+    return 0
+
+
 def main():
     args = parse()
+    if args.probe_pipes:
+        return probe_pipes()
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

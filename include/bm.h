@@ -187,6 +187,24 @@ BM_API bm_status bm_state_histogram(const bm_config *cfg, int32_t n_points, int6
                              size_t state_bytes, int32_t n_bins, uint64_t *counts, void *stream);
 
 /*
+ * Effective diffusion and velocity autocorrelation (the stationary state of eq. 18-19,
+ * PAPER.md:176-183): per-point ensemble moments of the checkpoint `state` (as bm_simulate_chunk left it at time t),
+ * optionally against `ref_state`, a copy of the checkpoint of the SAME run at an earlier time t0 (NULL: the entries
+ * that need it are 0).  out [n_points][BM_MOM_STRIDE] doubles, device:
+ *   N, MEAN_X, VAR_X (unfolded x(t)), MEAN_V, VAR_V (v(t); 0 for the over-damped model),
+ *   MEAN_DX, VAR_DX of x(t) - x(t0):  D_eff(t - t0) = VAR_DX / (2 (t - t0)),
+ *   COV_V0V = <v(t0) v(t)> - <v(t0)><v(t)>,  VAR_V0 = Var v(t0).            Variances divide by n-1.
+ * One block per point, two passes in a fixed order: bit-reproducible.  Called between the chunks of a chunked run it
+ * gives D_eff(t) and the velocity autocorrelation function without touching the path kernels (whose state stays in
+ * registers); DESIGN.md section 6 has the measured cost of a chunk boundary.
+ * Errors: BM_ERR_INVALID_ARG (null / misaligned pointers), BM_ERR_WORKSPACE (state smaller than bm_state_bytes(...)).
+ */
+enum { BM_MOM_N = 0, BM_MOM_MEAN_X = 1, BM_MOM_VAR_X = 2, BM_MOM_MEAN_V = 3, BM_MOM_VAR_V = 4, BM_MOM_MEAN_DX = 5,
+       BM_MOM_VAR_DX = 6, BM_MOM_COV_V0V = 7, BM_MOM_VAR_V0 = 8, BM_MOM_STRIDE = 10 };
+BM_API bm_status bm_state_moments(const bm_config *cfg, int32_t n_points, int64_t n_paths, const void *state, size_t state_bytes,
+                           const void *ref_state, double *out, void *stream);
+
+/*
  * HOST-pointer convenience entry (the end-to-end path): params, out_stats and out_paths (optional) are HOST
  * buffers.  Takes device scratch from a private stream-ordered pool (one per device, kept between calls: an
  * allocation cache with no influence on results), copies params in, runs bm_simulate on `stream`, copies the

@@ -202,3 +202,20 @@ def reduce(paths):
 
 def threads_used():
     return lib().orc_threads_used()
+
+
+# ---- observables of the stationary state beyond <v> -------------------------
+# Plain definitions written out on the oracle's per-path traces (x unfolded, v after every grid step; grid step index
+# i = 1, 2, ... is time i*dt).  Test infrastructure like the rest of this module.
+
+def deff_from_trace(trace, i0, i, dt):
+    """Effective diffusion coefficient over [t_i0, t_i]: D_eff = Var_p[x_p(t_i) - x_p(t_i0)] / (2 (t_i - t_i0)), unbiased
+    variance over the paths p (the spread of the ensemble grows as 2 D_eff t in the stationary state)."""
+    dx = trace[:, i - 1, 0] - trace[:, i0 - 1, 0]
+    return dx.var(ddof=1) / (2.0 * (i - i0) * dt)
+
+
+def vacf_from_trace(trace, i0, i):
+    """Velocity autocovariance C(t_i - t_i0) = <v(t_i0) v(t_i)> - <v(t_i0)><v(t_i)> over the paths (unbiased, n - 1)."""
+    a, b = trace[:, i0 - 1, 1], trace[:, i - 1, 1]
+    return ((a - a.mean()) * (b - b.mean())).sum() / (a.size - 1)

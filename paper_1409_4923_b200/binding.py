@@ -26,7 +26,11 @@ BM_OUT_XT, BM_OUT_VT, BM_OUT_VBAR, BM_OUT_JUMPS, BM_OUT_SUBSTEPS, BM_OUT_XTI, BM
  BM_PROBE_DFMA, BM_PROBE_I2F, BM_PROBE_FADD, BM_PROBE_MIX, BM_PROBE_COUNT) = range(11)
 
 BM_STATE_SLOTS, BM_CHUNK_ALIGN = 16, 8
-EXPORTS = ("bm_workspace_bytes", "bm_simulate", "bm_simulate_dt", "bm_state_bytes", "bm_simulate_chunk", "bm_state_histogram", "bm_simulate_host", "bm_philox_fill", "bm_gauss_fill",
+(BM_MOM_N, BM_MOM_MEAN_X, BM_MOM_VAR_X, BM_MOM_MEAN_V, BM_MOM_VAR_V, BM_MOM_MEAN_DX, BM_MOM_VAR_DX, BM_MOM_COV_V0V,
+ BM_MOM_VAR_V0) = range(9)
+BM_MOM_STRIDE = 10
+EXPORTS = ("bm_workspace_bytes", "bm_simulate", "bm_simulate_dt", "bm_state_bytes", "bm_simulate_chunk", "bm_state_histogram",
+           "bm_state_moments", "bm_simulate_host", "bm_philox_fill", "bm_gauss_fill",
            "bm_kernel_info", "bm_pipe_probe", "bm_status_string", "bm_version")
 STATS_FIELDS = ("n", "mean_v", "var_v", "mean_xT", "var_xT", "mean_jumps", "mean_substeps", "rsv")
 
@@ -69,6 +73,8 @@ def lib():
         L.bm_simulate_chunk.restype = C.c_int
         L.bm_state_histogram.argtypes = [cfgp, i32, i64, vp, C.c_size_t, i32, vp, vp]
         L.bm_state_histogram.restype = C.c_int
+        L.bm_state_moments.argtypes = [cfgp, i32, i64, vp, C.c_size_t, vp, vp, vp]
+        L.bm_state_moments.restype = C.c_int
         L.bm_simulate_host.argtypes = [cfgp, vp, i32, i64, i64, dbl, u64, vp, vp, vp]
         L.bm_simulate_host.restype = C.c_int
         L.bm_philox_fill.argtypes = [u64, u64, i32, u32, u32, i32, vp, vp]
@@ -203,6 +209,22 @@ def bm_state_histogram(cfg, n_points, n_paths, state, n_bins, counts, stream=Non
                                   C.c_void_p(counts.data_ptr()), _stream_ptr(stream))
     if rc != BM_OK:
         raise BmError(rc, "bm_state_histogram")
+
+
+def bm_state_moments(cfg, n_points, n_paths, state, out, ref_state=None, stream=None):
+    """out (CUDA float64 tensor [n_points, BM_MOM_STRIDE]) = ensemble moments of the checkpoint `state`, optionally
+    against the earlier checkpoint `ref_state` of the same run (D_eff, velocity autocovariance)."""
+    import torch
+    assert state.is_cuda and state.dtype == torch.uint8 and state.is_contiguous()
+    assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == n_points * BM_MOM_STRIDE
+    rp = None
+    if ref_state is not None:
+        assert ref_state.is_cuda and ref_state.dtype == torch.uint8 and ref_state.numel() >= state.numel()
+        rp = C.c_void_p(ref_state.data_ptr())
+    rc = lib().bm_state_moments(C.byref(cfg), n_points, n_paths, C.c_void_p(state.data_ptr()), state.numel(), rp,
+                                C.c_void_p(out.data_ptr()), _stream_ptr(stream))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_state_moments")
 
 
 def bm_simulate_host(cfg, params, n_points, n_paths, n_steps, dt, seed, out_stats, out_paths=None, stream=None):

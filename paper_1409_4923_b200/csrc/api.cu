@@ -306,6 +306,22 @@ BM_API bm_status bm_state_histogram(const bm_config *cfg, int32_t n_points, int6
                            reinterpret_cast<cudaStream_t>(stream)) == cudaSuccess ? BM_OK : BM_ERR_CUDA;
 }
 
+BM_API bm_status bm_state_moments(const bm_config *cfg, int32_t n_points, int64_t n_paths, const void *state, size_t state_bytes,
+                           const void *ref_state, double *out, void *stream) {
+  if (!valid_cfg(cfg) || n_points <= 0 || n_paths <= 0 || !state || !out) return BM_ERR_INVALID_ARG;
+  if (((uintptr_t)state & 15) || ((uintptr_t)ref_state & 15) || ((uintptr_t)out & 7)) return BM_ERR_INVALID_ARG;
+  const size_t need = bm_state_bytes(cfg, n_points, n_paths);
+  if (need == 0 || state_bytes < need) return BM_ERR_WORKSPACE;
+  const double period = cfg->potential == BM_POT_SINE2 ? 1.0 : (cfg->potential == BM_POT_PWL ? 2.0 : 0.0);
+  const bool literal = cfg->scheme == BM_SCHEME_PAPER_LITERAL;
+  const bool theta = cfg->prec == BM_F32 && !literal;  // position and velocity kept as scale * x
+  const double scale = (theta && cfg->potential == BM_POT_SINE2) ? 6.283185307179586 : 1.0;
+  return launch_state_moments(reinterpret_cast<const unsigned long long *>(state),
+                              reinterpret_cast<const unsigned long long *>(ref_state), n_points, n_paths,
+                              theta ? 0 : (literal ? 2 : 1), period, 1.0 / scale, out,
+                              reinterpret_cast<cudaStream_t>(stream)) == cudaSuccess ? BM_OK : BM_ERR_CUDA;
+}
+
 BM_API bm_status bm_simulate_host(const bm_config *cfg, const bm_params *params, int32_t n_points, int64_t n_paths,
                            int64_t n_steps, double dt, uint64_t seed, bm_stats *out_stats, double *out_paths,
                            void *stream) {

@@ -34,6 +34,8 @@ cudaError_t launch_grid_reduce(const double *partials, int n_points, int blocks_
                                cudaStream_t st);
 cudaError_t launch_state_hist(const unsigned long long *state, int n_points, long long n_paths, int kind, double inv_period,
                               int n_bins, unsigned long long *counts, cudaStream_t st);
+cudaError_t launch_state_moments(const unsigned long long *state, const unsigned long long *ref, int n_points, long long n_paths,
+                                 int kind, double period, double inv_scale, double *out, cudaStream_t st);
 cudaError_t launch_probe(int op, int iters, int blocks, int threads, float *sink, cudaStream_t st);
 
 }  // namespace bm

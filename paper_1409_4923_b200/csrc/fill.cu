@@ -133,6 +133,94 @@ cudaError_t launch_state_hist(const unsigned long long *state, int n_points, lon
   return cudaGetLastError();
 }
 
+// Row f3: ensemble moments of a checkpoint, per parameter point, optionally against a reference checkpoint of the same
+// run taken at an earlier time t0: D_eff(t) = Var[x(t) - x(t0)] / (2 (t - t0)) and the velocity autocovariance
+// <v(t0) v(t)> - <v(t0)><v(t)> (the stationary state).  One block per point; thread t
+// takes paths t, t + T, ... in order, then a fixed shuffle / shared-memory tree: bit-reproducible.  Two passes (means,
+// then central moments), fp64 throughout.  kind 0: fp32 jump-adapted kernel (slot 0 = (theta, wraps), slot 1 low word
+// = velocity in theta units, theta = scale * x);  kind 1: fp64 jump-adapted kernel (slots 0, 1, 2 = xi, wraps, v);
+// kind 2: paper-literal kernels (slots 0, 1 = x, wraps; no velocity).
+struct PathXV { double x, v; };
+__device__ __forceinline__ PathXV load_xv(const unsigned long long *st, long long stride, long long i, int kind, double period,
+                                          double inv_scale) {
+  PathXV r;
+  if (kind == 0) {
+    const unsigned long long a = __ldcg(st + i), b = __ldcg(st + stride + i);
+    r.x = (double)(int)(uint32_t)(a >> 32) * period + (double)__uint_as_float((uint32_t)a) * inv_scale;
+    r.v = (double)__uint_as_float((uint32_t)b) * inv_scale;
+  } else {
+    r.x = (double)(long long)__ldcg(st + stride + i) * period + __longlong_as_double((long long)__ldcg(st + i));
+    r.v = kind == 1 ? __longlong_as_double((long long)__ldcg(st + 2 * stride + i)) : 0.0;
+  }
+  return r;
+}
+
+template <int K>
+__device__ __forceinline__ void block_sum(double (&acc)[K], double (*sm)[K]) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+#pragma unroll
+  for (int k = 0; k < K; ++k)
+#pragma unroll
+    for (int d = 16; d >= 1; d >>= 1) acc[k] += __shfl_down_sync(0xffffffffu, acc[k], d);
+  __syncthreads();
+  if (lane == 0)
+#pragma unroll
+    for (int k = 0; k < K; ++k) sm[warp][k] = acc[k];
+  __syncthreads();
+#pragma unroll
+  for (int k = 0; k < K; ++k) {
+    double t = 0.0;
+    for (int w = 0; w < nwarps; ++w) t += sm[w][k];  // every thread adds the warps' sums in the same order
+    acc[k] = t;
+  }
+}
+
+__global__ void __launch_bounds__(256) state_moments_kernel(const unsigned long long *__restrict__ state,
+                                                           const unsigned long long *__restrict__ ref, long long n_paths,
+                                                           long long stride, int kind, double period, double inv_scale,
+                                                           double *__restrict__ out) {
+  __shared__ double sm[8][6];
+  const int point = blockIdx.x;
+  const long long base = (long long)point * n_paths;
+  double a1[6] = {0, 0, 0, 0, 0, 0};  // sums of x, v, dx, v0 (and two spare)
+  for (long long p = threadIdx.x; p < n_paths; p += blockDim.x) {
+    const PathXV c = load_xv(state, stride, base + p, kind, period, inv_scale);
+    a1[0] += c.x; a1[1] += c.v;
+    if (ref) {
+      const PathXV r = load_xv(ref, stride, base + p, kind, period, inv_scale);
+      a1[2] += c.x - r.x; a1[3] += r.v;
+    }
+  }
+  block_sum<6>(a1, sm);
+  const double n = (double)n_paths;
+  const double mx = a1[0] / n, mv = a1[1] / n, md = a1[2] / n, mv0 = a1[3] / n;
+  double a2[6] = {0, 0, 0, 0, 0, 0};  // sums of (x-mx)^2, (v-mv)^2, (dx-md)^2, (v0-mv0)(v-mv), (v0-mv0)^2
+  for (long long p = threadIdx.x; p < n_paths; p += blockDim.x) {
+    const PathXV c = load_xv(state, stride, base + p, kind, period, inv_scale);
+    a2[0] += (c.x - mx) * (c.x - mx); a2[1] += (c.v - mv) * (c.v - mv);
+    if (ref) {
+      const PathXV r = load_xv(ref, stride, base + p, kind, period, inv_scale);
+      const double dx = c.x - r.x;
+      a2[2] += (dx - md) * (dx - md); a2[3] += (r.v - mv0) * (c.v - mv); a2[4] += (r.v - mv0) * (r.v - mv0);
+    }
+  }
+  block_sum<6>(a2, sm);
+  if (threadIdx.x == 0) {
+    const double nm1 = n > 1.0 ? n - 1.0 : 1.0;
+    double *o = out + (long long)point * BM_MOM_STRIDE;
+    o[BM_MOM_N] = n; o[BM_MOM_MEAN_X] = mx; o[BM_MOM_VAR_X] = a2[0] / nm1; o[BM_MOM_MEAN_V] = mv; o[BM_MOM_VAR_V] = a2[1] / nm1;
+    o[BM_MOM_MEAN_DX] = ref ? md : 0.0; o[BM_MOM_VAR_DX] = ref ? a2[2] / nm1 : 0.0; o[BM_MOM_COV_V0V] = ref ? a2[3] / nm1 : 0.0;
+    o[BM_MOM_VAR_V0] = ref ? a2[4] / nm1 : 0.0; o[9] = 0.0;
+  }
+}
+
+cudaError_t launch_state_moments(const unsigned long long *state, const unsigned long long *ref, int n_points, long long n_paths,
+                                 int kind, double period, double inv_scale, double *out, cudaStream_t st) {
+  state_moments_kernel<<<(unsigned)n_points, 256, 0, st>>>(state, ref, n_paths, (long long)n_points * n_paths, kind, period,
+                                                          inv_scale, out);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_grid_reduce(const double *partials, int n_points, int blocks_per_point, bm_stats *out,
                                cudaStream_t st) {
   const int threads = 128;  // 4 points per block
