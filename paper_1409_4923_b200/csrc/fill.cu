@@ -175,11 +175,11 @@ __device__ __forceinline__ void block_sum(double (&acc)[K], double (*sm)[K]) {
   }
 }
 
-__global__ void __launch_bounds__(256) state_moments_kernel(const unsigned long long *__restrict__ state,
+__global__ void __launch_bounds__(1024) state_moments_kernel(const unsigned long long *__restrict__ state,
                                                            const unsigned long long *__restrict__ ref, long long n_paths,
                                                            long long stride, int kind, double period, double inv_scale,
                                                            double *__restrict__ out) {
-  __shared__ double sm[8][6];
+  __shared__ double sm[32][6];
   const int point = blockIdx.x;
   const long long base = (long long)point * n_paths;
   double a1[6] = {0, 0, 0, 0, 0, 0};  // sums of x, v, dx, v0 (and two spare)
@@ -216,7 +216,8 @@ __global__ void __launch_bounds__(256) state_moments_kernel(const unsigned long 
 
 cudaError_t launch_state_moments(const unsigned long long *state, const unsigned long long *ref, int n_points, long long n_paths,
                                  int kind, double period, double inv_scale, double *out, cudaStream_t st) {
-  state_moments_kernel<<<(unsigned)n_points, 256, 0, st>>>(state, ref, n_paths, (long long)n_points * n_paths, kind, period,
+  // one block per point: 1024 threads for the large single-point ensembles, 256 for sweeps of many points
+  state_moments_kernel<<<(unsigned)n_points, n_paths >= 8192 ? 1024 : 256, 0, st>>>(state, ref, n_paths, (long long)n_points * n_paths, kind, period,
                                                           inv_scale, out);
   return cudaGetLastError();
 }

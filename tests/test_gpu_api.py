@@ -169,3 +169,51 @@ def test_kernel_info_and_probe(B):
     for op in range(B.BM_PROBE_COUNT):
         B.bm_pipe_probe(op, 4, 148, 256, sink)
     torch.cuda.synchronize()
+
+
+@pytest.mark.parametrize("kind", ["f32", "f64", "literal-f32", "f32-inertial"])
+def test_guard_bands_around_every_buffer_stay_intact(B, kind):
+    """compute-sanitizer is closed on this GPU pool, so out-of-bounds writes are looked for with guard bands of our
+    own: every device buffer a call may write (stats, per-path outputs, checkpoint state, workspace, histogram, moments)
+    is carved out of one arena with 4 KiB of a canary pattern on both sides; ragged ensemble sizes, a multi-point sweep,
+    single-launch and chunked runs; afterwards every canary byte must be untouched."""
+    import torch
+    dev = torch.device("cuda:0")
+    n_points, n_paths, n_steps = 3, 333, 160
+    if kind == "f32-inertial":
+        w = W.Workload("g", W.INERTIAL, np.repeat(W.c2().params, n_points, axis=0), n_paths, n_steps, W.DT_INERTIAL, 16)
+    else:
+        w = W.c4().scaled(n_paths=n_paths, n_steps=n_steps, points=[5, 64 * 128 + 64, 127 * 128 + 127])
+        if kind.startswith("literal"):
+            w = W.Workload("g", W.OVERDAMPED, w.params, n_paths, n_steps, w.dt, 16, scheme=W.SCHEME_PAPER_LITERAL)
+    prec = B.BM_F64 if kind == "f64" else B.BM_F32
+    cfg = B.config_for(w, prec)
+    GUARD, CANARY = 4096, 0xA5
+    sizes = {"stats": n_points * 64, "paths": n_points * n_paths * B.BM_OUT_STRIDE * 8,
+             "state": B.bm_state_bytes(cfg, n_points, n_paths), "ws": max(16, B.bm_workspace_bytes(cfg, n_points, n_paths)),
+             "hist": n_points * 24 * 8, "mom": n_points * B.BM_MOM_STRIDE * 8}
+    offs, total = {}, GUARD
+    for k, sz in sizes.items():
+        offs[k] = total
+        total += (sz + 255) // 256 * 256 + GUARD
+    arena = torch.full((total,), CANARY, dtype=torch.uint8, device=dev)
+    view = {k: arena[offs[k]:offs[k] + sizes[k]] for k in sizes}
+    for v in view.values():
+        v.zero_()
+    stats = view["stats"].view(torch.float64).view(n_points, 8)
+    paths = view["paths"].view(torch.float64).view(n_points * n_paths, B.BM_OUT_STRIDE)
+    hist = view["hist"].view(torch.int64).view(n_points, 24)
+    mom = view["mom"].view(torch.float64).view(n_points, B.BM_MOM_STRIDE)
+    params = torch.from_numpy(np.ascontiguousarray(w.params)).to(dev)
+    B.bm_simulate(cfg, params, n_points, n_paths, n_steps, w.dt, w.seed, stats, paths, workspace=view["ws"])
+    for b in range(0, n_steps, 40):
+        B.bm_simulate_chunk(cfg, params, n_points, n_paths, n_steps, w.dt, w.seed, b, 40, view["state"], stats, paths, workspace=view["ws"])
+        B.bm_state_histogram(cfg, n_points, n_paths, view["state"], 24, hist)
+        B.bm_state_moments(cfg, n_points, n_paths, view["state"], mom)
+    torch.cuda.synchronize()
+    host = arena.cpu().numpy()
+    mask = np.ones(total, dtype=bool)
+    for k in sizes:
+        mask[offs[k]:offs[k] + sizes[k]] = False
+    assert np.all(host[mask] == CANARY), f"{int((host[mask] != CANARY).sum())} guard bytes overwritten"
+    assert float(stats[0, 0]) == n_paths and int(hist.sum()) == n_points * n_paths * (n_steps // 40)
