@@ -357,6 +357,97 @@ static void path_paper_literal(const orc_config *cfg, const orc_params *p, uint6
   out[ORC_OUT_XTI] = unfolded(&snap, L);
 }
 
+/* ------------------------------------------------------------------------------------------------
+ * Dynamic step size control from chi (NEXT row f4).  PAPER.md:237: "The difference chi = xbar_{n+1} - x_{n+1} between
+ * these values provides information about the local approximation error.  This quantity can be utilized to introduce a
+ * dynamic time step size control".  The paper gives no controller; reading R14:
+ *   - a grid step dt is covered by intervals of length dt 2^-k, k = 0..K (K = adapt_levels), each aligned to a multiple
+ *     of its own length, so every grid point n dt is hit exactly and t_i, t_f, the trace stay where they were;
+ *   - an interval is integrated as in the jump-adapted scheme (sub-steps end on the kicks and flips inside it; one
+ *     Gaussian, number m = running sub-step count, per sub-step); chi of a sub-step is Alg. 1's predictor (line 4)
+ *     minus its corrector (line 6);
+ *   - no step is ever rejected (its noise has been drawn; redoing it with a finer step would need a Brownian bridge
+ *     to keep the law): the largest |chi| of an interval sets the length of the NEXT one: halve (k+1) if it
+ *     exceeds tol, double (k-1) if it is below tol/8 and the next interval would still be aligned, else keep.
+ * Every path starts at k = 0.  tol = +inf reproduces the jump-adapted scheme; tol = 0 the same scheme at dt 2^-K.
+ * Over-damped only (Alg. 1 is the over-damped scheme).
+ * ---------------------------------------------------------------------------------------------- */
+static void path_adaptive(const orc_config *cfg, const orc_params *p, uint64_t g, int64_t n_steps, double dt,
+                          uint64_t seed, double *out, double *trace, int64_t trace_steps) {
+  const double L = orc_period(cfg->potential);
+  const int has_P = p->lambda > 0.0, has_D = p->mu_a > 0.0;
+  const int K = cfg->adapt_levels;
+  const int64_t TPC = (int64_t)1 << K; /* ticks per grid step */
+  pos_t s; int d;
+  init_path(cfg, p, seed, g, L, &s, &d);
+  uint32_t w[4];
+  uint32_t kP = 0, kD = 0;
+  double rP = INFINITY, rD = INFINITY, z = 0.0;
+  if (has_P) {
+    orc_philox_call(seed, g, STREAM_POISSON, kP, w);
+    rP = -log(orc_u01(w[0])) / p->lambda;
+    z = -p->zeta * log(orc_u01(w[1]));
+  }
+  if (has_D) {
+    orc_philox_call(seed, g, STREAM_DICH, kD, w);
+    rD = -log(orc_u01(w[0])) / mu_leave(p, d);
+  }
+  uint64_t m = 0; double jumps = 0.0;
+  double gblk[4] = {0, 0, 0, 0};
+  pos_t snap = s;
+  int k = 0;
+  for (int64_t n = 0; n < n_steps; ++n) {
+    int64_t tick = 0;
+    while (tick < TPC) {
+      const int64_t wd = TPC >> k;           /* interval width in ticks */
+      const double H = ldexp(dt, -k);        /* its length, exactly dt 2^-k */
+      double rem = H, chi_max = 0.0;
+      while (rem > 0.0) {
+        double h = rem;
+        if (has_P && rP < h) h = rP;
+        if (has_D && rD < h) h = rD;
+        if ((m & 3u) == 0) orc_gauss_block(seed, g, (uint32_t)(m >> 2), gblk);
+        double gn = gblk[m & 3u];
+        m++;
+        double st[5];
+        double xn = orc_substep_overdamped(p, cfg->potential, d, s.xi, h, gn, st);
+        double chi = fabs(st[3] - xn);       /* predictor (line 4) minus corrector (line 6) */
+        if (chi > chi_max) chi_max = chi;
+        s.xi = xn;
+        rem -= h;
+        if (has_P) rP -= h;
+        if (has_D) rD -= h;
+        if (has_P && rP <= 0.0) {
+          s.xi += z;
+          jumps += 1.0; kP++;
+          orc_philox_call(seed, g, STREAM_POISSON, kP, w);
+          rP = -log(orc_u01(w[0])) / p->lambda;
+          z = -p->zeta * log(orc_u01(w[1]));
+        }
+        if (has_D && rD <= 0.0) {
+          d = 1 - d;
+          jumps += 1.0; kD++;
+          orc_philox_call(seed, g, STREAM_DICH, kD, w);
+          rD = -log(orc_u01(w[0])) / mu_leave(p, d);
+        }
+        fold(&s, L);
+      }
+      tick += wd;
+      if (chi_max > cfg->adapt_tol && k < K) k += 1;
+      else if (chi_max < 0.125 * cfg->adapt_tol && k > 0 && (tick % (2 * wd)) == 0) k -= 1;
+    }
+    if (trace && n + 1 <= trace_steps) { trace[2 * n] = unfolded(&s, L); trace[2 * n + 1] = 0.0; }
+    if (n + 1 == cfg->n_discard) snap = s;
+  }
+  double span = (double)(n_steps - cfg->n_discard) * dt;
+  out[ORC_OUT_XT] = unfolded(&s, L);
+  out[ORC_OUT_VT] = 0.0;
+  out[ORC_OUT_VBAR] = ((double)(s.wraps - snap.wraps) * L + (s.xi - snap.xi)) / span;
+  out[ORC_OUT_JUMPS] = jumps;
+  out[ORC_OUT_SUBSTEPS] = (double)m;
+  out[ORC_OUT_XTI] = unfolded(&snap, L);
+}
+
 /* ------------------------------------------------------------------------------------------------ */
 static int g_threads_used = 1;
 int orc_threads_used(void) { return g_threads_used; }
@@ -367,6 +458,8 @@ int orc_simulate(const orc_config *cfg, const orc_params *params, int32_t n_poin
   if (!cfg || !params || !out_paths || n_points <= 0 || n_paths <= 0 || n_steps <= 0 || !(dt > 0.0)) return -1;
   if (cfg->n_discard < 0 || cfg->n_discard >= n_steps) return -1;
   if (cfg->scheme == ORC_SCHEME_PAPER_LITERAL && cfg->model != ORC_OVERDAMPED) return -2;
+  if (cfg->scheme == ORC_SCHEME_ADAPTIVE && cfg->model != ORC_OVERDAMPED) return -2;
+  if (cfg->scheme == ORC_SCHEME_ADAPTIVE && (cfg->adapt_levels < 0 || cfg->adapt_levels > 20 || !(cfg->adapt_tol >= 0.0))) return -1;
   if (cfg->potential < 0 || cfg->potential > ORC_POT_QUAD) return -1;
   int64_t total = ids ? n_ids : (int64_t)n_points * n_paths;
   if (total <= 0) return -1;
@@ -388,6 +481,8 @@ int orc_simulate(const orc_config *cfg, const orc_params *params, int32_t n_poin
     double *tr = (trace && i < trace_paths) ? trace + i * trace_steps * 2 : NULL;
     if (cfg->scheme == ORC_SCHEME_PAPER_LITERAL)
       path_paper_literal(cfg, p, g, n_steps, dt, seed, out_paths + i * ORC_OUT_STRIDE, tr, trace_steps);
+    else if (cfg->scheme == ORC_SCHEME_ADAPTIVE)
+      path_adaptive(cfg, p, g, n_steps, dt, seed, out_paths + i * ORC_OUT_STRIDE, tr, trace_steps);
     else
       path_jump_adapted(cfg, p, g, n_steps, dt, seed, out_paths + i * ORC_OUT_STRIDE, tr, trace_steps);
   }

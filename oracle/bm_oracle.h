@@ -39,7 +39,7 @@ typedef struct {
 
 enum { ORC_OVERDAMPED = 0, ORC_INERTIAL = 1 };
 enum { ORC_POT_SINE2 = 0, ORC_POT_PWL = 1, ORC_POT_QUAD = 2 };
-enum { ORC_SCHEME_JUMP_ADAPTED = 0, ORC_SCHEME_PAPER_LITERAL = 1 };
+enum { ORC_SCHEME_JUMP_ADAPTED = 0, ORC_SCHEME_PAPER_LITERAL = 1, ORC_SCHEME_ADAPTIVE = 2 };
 
 typedef struct {
   int32_t model;      /* ORC_OVERDAMPED / ORC_INERTIAL */
@@ -47,6 +47,11 @@ typedef struct {
   int32_t scheme;     /* ORC_SCHEME_* */
   int32_t reserved;
   int64_t n_discard;  /* grid steps before t_i (eq. 30) */
+  /* ORC_SCHEME_ADAPTIVE only (reading R14): tolerance on |chi| = |xbar_{n+1} - x_{n+1}| and the number
+   * of times the step dt may be halved */
+  double adapt_tol;
+  int32_t adapt_levels;
+  int32_t reserved2;
 } orc_config;
 
 /* per-path record: 6 doubles */

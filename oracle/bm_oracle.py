@@ -17,7 +17,7 @@ _LIB = os.path.join(_HERE, "libbm_oracle.so")
 
 OVERDAMPED, INERTIAL = 0, 1
 POT_SINE2, POT_PWL, POT_QUAD = 0, 1, 2
-SCHEME_JUMP_ADAPTED, SCHEME_PAPER_LITERAL = 0, 1
+SCHEME_JUMP_ADAPTED, SCHEME_PAPER_LITERAL, SCHEME_ADAPTIVE = 0, 1, 2
 OUT_XT, OUT_VT, OUT_VBAR, OUT_JUMPS, OUT_SUBSTEPS, OUT_XTI, OUT_STRIDE = 0, 1, 2, 3, 4, 5, 6
 
 PARAM_FIELDS = ("A1", "A2", "F", "D", "lambda_", "zeta", "Fa", "Fb", "mu_a", "mu_b", "gamma", "amp", "omega",
@@ -30,7 +30,7 @@ class OrcParams(C.Structure):
 
 class OrcConfig(C.Structure):
     _fields_ = [("model", C.c_int32), ("potential", C.c_int32), ("scheme", C.c_int32), ("reserved", C.c_int32),
-                ("n_discard", C.c_int64)]
+                ("n_discard", C.c_int64), ("adapt_tol", C.c_double), ("adapt_levels", C.c_int32), ("reserved2", C.c_int32)]
 
 
 class OrcStats(C.Structure):
@@ -167,11 +167,12 @@ def substep_inertial(p, potential, d, t, h, g, x, v):
 
 
 def simulate(params, n_paths, n_steps, dt, seed, *, model=OVERDAMPED, potential=POT_SINE2,
-             scheme=SCHEME_JUMP_ADAPTED, n_discard=0, ids=None, trace_paths=0, trace_steps=0, threads=0):
+             scheme=SCHEME_JUMP_ADAPTED, n_discard=0, ids=None, trace_paths=0, trace_steps=0, threads=0,
+             adapt_tol=float("inf"), adapt_levels=0):
     """Run the oracle.  Returns (paths[n][6] float64, trace or None).  ids: global path ids to run (default all)."""
     arr = params if isinstance(params, C.Array) else params_array(params)
     n_points = len(arr)
-    cfg = OrcConfig(model, potential, scheme, 0, n_discard)
+    cfg = OrcConfig(model, potential, scheme, 0, n_discard, adapt_tol, adapt_levels, 0)
     if ids is not None:
         ids = np.ascontiguousarray(ids, dtype=np.int64)
         n = ids.size
