@@ -54,8 +54,13 @@ typedef enum { BM_SINCOS_AUTO = 0, BM_SINCOS_SFU = 1, BM_SINCOS_FMA = 2 } bm_sin
 typedef enum { BM_POT_SINE2 = 0, BM_POT_PWL = 1, BM_POT_QUAD = 2 } bm_potential;
 /* JUMP_ADAPTED: exact kick/flip times, Box-Muller Gaussians (the hot path).
  * PAPER_LITERAL: Alg. 2/3/4 exactly as printed (three-point increments, grid-quantised countdowns,
- * constant forces in the corrector line only); over-damped only. */
-typedef enum { BM_SCHEME_JUMP_ADAPTED = 0, BM_SCHEME_PAPER_LITERAL = 1 } bm_scheme;
+ * constant forces in the corrector line only); over-damped only.
+ * ADAPTIVE: the jump-adapted scheme with dynamic step size control from chi = xbar_{n+1} - x_{n+1}, the difference of
+ * Alg. 1's predictor and corrector (reading R14): a grid step dt is
+ * covered by aligned intervals dt 2^-k, k = 0..adapt_levels; no step is rejected; the largest |chi| of an interval
+ * halves the next one if above adapt_tol and doubles it if below adapt_tol/8.  BM_F64, over-damped only (else
+ * BM_ERR_UNSUPPORTED); no chunked runs. */
+typedef enum { BM_SCHEME_JUMP_ADAPTED = 0, BM_SCHEME_PAPER_LITERAL = 1, BM_SCHEME_ADAPTIVE = 2 } bm_scheme;
 /* fp32 only: how Philox words of the Gaussian stream become Box-Muller pairs (R3, R13).
  * W32: one word per uniform (radius from w0, angle from w1, ...): four normals per call -- the oracle's assignment,
  *      so a jump-free fp32 path follows the fp64 oracle's path (common random numbers).
@@ -112,7 +117,8 @@ typedef struct {
                             (BM_POT_SINE2 only, else BM_ERR_UNSUPPORTED).  A path's result does not depend on it; it
                             enters the determinism contract through the reduction tree of out_stats only.  Must be 0
                             for BM_F32 and the paper-literal scheme. */
-  int32_t rsv;         /* 0 */
+  int32_t adapt_levels; /* BM_SCHEME_ADAPTIVE: how often dt may be halved, 0..20 */
+  double adapt_tol;    /* BM_SCHEME_ADAPTIVE: tolerance on |chi| (in units of x), >= 0; +inf = never refine */
 } bm_config;
 
 /* per-path record written to out_paths: 6 doubles */

@@ -18,7 +18,7 @@ BM_OVERDAMPED, BM_INERTIAL = 0, 1
 BM_F32, BM_F64 = 0, 1
 BM_SINCOS_AUTO, BM_SINCOS_SFU, BM_SINCOS_FMA = 0, 1, 2
 BM_POT_SINE2, BM_POT_PWL, BM_POT_QUAD = 0, 1, 2
-BM_SCHEME_JUMP_ADAPTED, BM_SCHEME_PAPER_LITERAL = 0, 1
+BM_SCHEME_JUMP_ADAPTED, BM_SCHEME_PAPER_LITERAL, BM_SCHEME_ADAPTIVE = 0, 1, 2
 BM_NOISE_GAUSS, BM_NOISE_POISSON, BM_NOISE_DICH = 1, 2, 4
 BM_GAUSS_AUTO, BM_GAUSS_W32, BM_GAUSS_W16, BM_GAUSS_W16P = 0, 1, 2, 3
 BM_OUT_XT, BM_OUT_VT, BM_OUT_VBAR, BM_OUT_JUMPS, BM_OUT_SUBSTEPS, BM_OUT_XTI, BM_OUT_STRIDE = 0, 1, 2, 3, 4, 5, 6
@@ -39,7 +39,7 @@ class BmConfig(C.Structure):
     _fields_ = [("model", C.c_int32), ("prec", C.c_int32), ("sincos", C.c_int32), ("potential", C.c_int32),
                 ("scheme", C.c_int32), ("noise", C.c_int32), ("block_threads", C.c_int32), ("gauss", C.c_int32),
                 ("n_discard", C.c_int64), ("trace_steps", C.c_int64), ("trace_paths", C.c_int64),
-                ("paths_per_thread", C.c_int32), ("rsv", C.c_int32)]
+                ("paths_per_thread", C.c_int32), ("adapt_levels", C.c_int32), ("adapt_tol", C.c_double)]
 
 
 class BmError(RuntimeError):
@@ -116,9 +116,9 @@ def noise_mask(params):
 
 def make_config(model=BM_OVERDAMPED, prec=BM_F32, sincos=BM_SINCOS_AUTO, potential=BM_POT_SINE2,
                 scheme=BM_SCHEME_JUMP_ADAPTED, noise=BM_NOISE_GAUSS, block_threads=0, n_discard=0, trace_steps=0,
-                trace_paths=0, gauss=BM_GAUSS_AUTO, paths_per_thread=0):
+                trace_paths=0, gauss=BM_GAUSS_AUTO, paths_per_thread=0, adapt_tol=float("inf"), adapt_levels=0):
     return BmConfig(model, prec, sincos, potential, scheme, noise, block_threads, gauss, n_discard, trace_steps,
-                    trace_paths, paths_per_thread, 0)
+                    trace_paths, paths_per_thread, adapt_levels, adapt_tol)
 
 
 def _stream_ptr(stream):
@@ -281,10 +281,11 @@ def bm_pipe_probe(op, iters, blocks, threads, sink, stream=None):
 
 def config_for(w, prec, sincos=BM_SINCOS_AUTO, block_threads=0, trace_steps=0, trace_paths=0, gauss=BM_GAUSS_AUTO,
                paths_per_thread=0):
-    """bm_config of a workloads.Workload."""
+    """bm_config of a workloads.Workload (extra: adapt_tol, adapt_levels for the adaptive scheme)."""
     return make_config(model=w.model, prec=prec, sincos=sincos, potential=w.potential, scheme=w.scheme,
                        noise=noise_mask(w.params), block_threads=block_threads, n_discard=w.n_discard,
-                       trace_steps=trace_steps, trace_paths=trace_paths, gauss=gauss, paths_per_thread=paths_per_thread)
+                       trace_steps=trace_steps, trace_paths=trace_paths, gauss=gauss, paths_per_thread=paths_per_thread,
+                       adapt_tol=w.extra.get("adapt_tol", float("inf")), adapt_levels=w.extra.get("adapt_levels", 0))
 
 
 def run_workload(w, prec, want_paths=False, sincos=BM_SINCOS_AUTO, block_threads=0, trace_steps=0, trace_paths=0,

@@ -30,7 +30,8 @@ bool valid_cfg(const bm_config *c) {
   if (c->prec != BM_F32 && c->prec != BM_F64) return false;
   if (c->sincos < BM_SINCOS_AUTO || c->sincos > BM_SINCOS_FMA) return false;
   if (c->potential < BM_POT_SINE2 || c->potential > BM_POT_QUAD) return false;
-  if (c->scheme != BM_SCHEME_JUMP_ADAPTED && c->scheme != BM_SCHEME_PAPER_LITERAL) return false;
+  if (c->scheme != BM_SCHEME_JUMP_ADAPTED && c->scheme != BM_SCHEME_PAPER_LITERAL && c->scheme != BM_SCHEME_ADAPTIVE) return false;
+  if (c->scheme == BM_SCHEME_ADAPTIVE && (c->adapt_levels < 0 || c->adapt_levels > 20 || !(c->adapt_tol >= 0.0))) return false;
   if (c->noise < 0 || c->noise > 7) return false;
   if (c->block_threads != 0 && (c->block_threads < 32 || c->block_threads > 512 || (c->block_threads & 31))) return false;
   if (c->block_threads > 256 && !(c->prec == BM_F32 && c->model == BM_OVERDAMPED && c->scheme == BM_SCHEME_JUMP_ADAPTED)) return false;
@@ -98,12 +99,15 @@ struct Launch {
 bm_status pick_kernel(const bm_config *c, int32_t n_points, int64_t n_paths, Launch *L, bool chunked = false) {
   *L = Launch();
   if (c->scheme == BM_SCHEME_PAPER_LITERAL && c->model != BM_OVERDAMPED) return BM_ERR_UNSUPPORTED;
+  if (c->scheme == BM_SCHEME_ADAPTIVE && (c->model != BM_OVERDAMPED || c->prec != BM_F64 || chunked)) return BM_ERR_UNSUPPORTED;
   if (c->model == BM_INERTIAL && c->potential != BM_POT_SINE2) return BM_ERR_UNSUPPORTED;
   if (c->paths_per_thread == 2 && !has_two_paths(c)) return BM_ERR_UNSUPPORTED;
   L->threads = block_threads_of(c, n_points, n_paths);
   L->ppt = paths_per_thread_of(c, n_points, n_paths);
   if (c->scheme == BM_SCHEME_PAPER_LITERAL) {
     L->fn = pick_literal(c->prec, c->potential, c->noise);
+  } else if (c->scheme == BM_SCHEME_ADAPTIVE) {
+    L->fn = pick_adaptive_f64(c->potential, c->noise);
   } else if (c->prec == BM_F64) {
     L->fn = c->model == BM_OVERDAMPED ? pick_f64_overdamped(c->potential, c->noise, chunked, L->ppt)
                                       : pick_f64_inertial(c->potential, c->noise, chunked, L->ppt);
@@ -244,6 +248,8 @@ static bm_status simulate_range(const bm_config *cfg, const bm_params *params, i
   a.state = reinterpret_cast<unsigned long long *>(state);
   a.step_begin = step_begin;
   a.step_end = step_end;
+  a.adapt_tol = cfg->adapt_tol;
+  a.adapt_levels = cfg->adapt_levels;
   a.keys = make_keys(seed);
 
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);

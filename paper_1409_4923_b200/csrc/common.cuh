@@ -36,6 +36,8 @@ struct SimArgs {
   // a whole run in one launch (step_begin = 0, step_end = n_steps).
   unsigned long long *state;  // [STATE_SLOTS][n_points * n_paths], 8-byte slots, slot-major (coalesced)
   long long step_begin, step_end;
+  double adapt_tol;  // BM_SCHEME_ADAPTIVE (row f4): tolerance on |chi| and number of halvings of dt
+  int adapt_levels;
   PhiloxKeys keys;
 };
 

@@ -24,6 +24,8 @@ KernelFn pick_f32_in_fma_w16p(int potential, int noise, int occ);
 
 // the paper's own scheme as printed (sim_literal.cu); over-damped only
 KernelFn pick_literal(int prec, int potential, int noise);
+// dynamic step size control from chi (sim_adaptive.cu); fp64, over-damped only
+KernelFn pick_adaptive_f64(int potential, int noise);
 
 // fills (fill.cu)
 cudaError_t launch_philox_fill(const PhiloxKeys &K, unsigned long long path0, int n_paths, uint32_t stream_id,

@@ -20,7 +20,7 @@ COL = {n: i for i, n in enumerate(FIELDS)}
 
 OVERDAMPED, INERTIAL = 0, 1
 POT_SINE2, POT_PWL, POT_QUAD = 0, 1, 2
-SCHEME_JUMP_ADAPTED, SCHEME_PAPER_LITERAL = 0, 1
+SCHEME_JUMP_ADAPTED, SCHEME_PAPER_LITERAL, SCHEME_ADAPTIVE = 0, 1, 2
 
 
 def params_table(n_points=1, **kw):

@@ -33,7 +33,7 @@ def test_header_symbols_are_exported(B):
 
 
 def test_struct_layouts_match_header(B):
-    assert C.sizeof(B.BmConfig) == 64
+    assert C.sizeof(B.BmConfig) == 72
     assert len(W.FIELDS) == 16 and len(B.STATS_FIELDS) == 8
     hdr = open(os.path.join(ROOT, "include", "bm.h")).read()
     body = hdr[hdr.index("typedef struct {", hdr.index("One parameter point")):hdr.index("} bm_params;")]
