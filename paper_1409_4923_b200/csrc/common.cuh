@@ -71,7 +71,7 @@ constexpr int EV_FIELDS_P = 4, EV_FIELDS_D = 3;  // (cell, off, amplitude, norma
 
 // 32-bit words of dynamic shared memory per thread of the fp32 path kernel (host and device agree through this)
 __host__ __device__ constexpr int f32_smem_words_per_thread(int noise, int gauss) {
-  return ((noise & BM_NOISE_POISSON) ? EVQ * EV_FIELDS_P : 0) + ((noise & BM_NOISE_DICH) ? EVQ * EV_FIELDS_D : 0) + 0 * gauss;
+  return ((noise & BM_NOISE_POISSON) ? EVQ * EV_FIELDS_P : 0) + ((noise & BM_NOISE_DICH) ? EVQ * EV_FIELDS_D : 0) + 4 + 0 * gauss;
 }
 
 constexpr uint32_t PHILOX_M0 = 0xD2511F53u, PHILOX_M1 = 0xCD9E8D57u;

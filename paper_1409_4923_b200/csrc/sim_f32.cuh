@@ -303,6 +303,11 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
   const int T = blockDim.x, tid = threadIdx.x;
   uint32_t *const ringP = smem_words + tid;               // [EVQ][NFP][T]
   uint32_t *const ringD = ringP + EVQ * NFP * T;          // [EVQ][NFD][T]
+  // state that is touched a few times per run lives in shared memory, not in registers (the 64-register class of the
+  // over-damped kernel re-materialises loop constants otherwise): the snapshot at t_i and, per stream, the number of
+  // events drawn so far.  The index of a stream's next event = events drawn - events queued - 1 = events applied, so
+  // no counter has to follow the events themselves.
+  uint32_t *const cold = ringD + EVQ * NFD * T;           // [4][T]: snap_x, snap_w, drawnP, drawnD
 
   const int point = blockIdx.x / a.blocks_per_point;
   const int chunk = blockIdx.x - point * a.blocks_per_point;
@@ -375,11 +380,11 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
   };
 
   const int n_discard = (int)a.n_discard;
-  // next event of each stream: (cell index, offset inside that cell); NEVER = switched off at this point.  kP, kD:
-  // its index in the stream = the Philox call it came from; qP, qD: ring read slot (bits 0-3) and fill (bits 4-).
+  // next event of each stream: (cell index, offset inside that cell); NEVER = switched off at this point.  qP, qD:
+  // ring read slot (bits 0-3) and fill (bits 4-); the index of the event in its stream follows from the draw count.
   int nP = NEVER, nD = NEVER;
   float fP = 0.f, fD = 0.f, z = 0.f, gP = 0.f, gD = 0.f;
-  uint32_t kP = 0, kD = 0;
+  uint32_t drawnP = 0, drawnD = 0;  // stored to `cold` below; registers only during the set-up
   int qP = 0, qD = 0;
   // lanes past a ragged end stay inert: no events, no checkpoint traffic (they must not steer the warp's votes)
   if (HAS_P && lam > 0.0 && valid) {
@@ -387,11 +392,13 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
     schedule_f32(0, 0.f, dt, inv_dt, neg_log_u_f32(w.x) * P.inv_lam_dt, nP, fP);
     z = P.zeta * neg_log_u_f32(w.y);
     if (HAS_G) gP = event_normal(w.z);
+    drawnP = 1;
   }
   if (onD && valid) {
     const uint4 w = philox_call(K, g, STREAM_DICH, 0);
     schedule_f32(0, 0.f, dt, inv_dt, neg_log_u_f32(w.x) * (d ? P.inv_mub_dt : P.inv_mua_dt), nD, fD);
     if (HAS_G) gD = event_normal(w.z);
+    drawnD = 1;
   }
 
   // drive phase in 2^-64 turns per cell (inertial): exact integer accumulation, no float time.  n is the same in
@@ -405,8 +412,7 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
     drive0 = P.amp;  // cos(0)
   }
 
-  int jumps = 0;  // events applied = sub-steps that ended inside a cell
-  float snap_x = x;
+  float snap_x = x;  // stored to `cold` below
   int snap_w = wraps;
   // row f2: a launch that continues a run reloads everything the lines above initialised (the Philox calls of the
   // initialisation are wasted then, once per launch).  The rings are not part of the state: they restart empty and
@@ -416,16 +422,20 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
     const StateIO io = state_io(a, g);
     uint32_t lo, hi;
     io.get2(0, lo, hi); x = __uint_as_float(lo); wraps = (int)hi;
-    io.get2(1, lo, hi); v = __uint_as_float(lo); jumps = (int)hi;
+    io.get2(1, lo, hi); v = __uint_as_float(lo);  // (hi: events applied = the two stream indices below)
     io.get2(2, lo, hi); nP = (int)lo; fP = __uint_as_float(hi);
-    io.get2(3, lo, hi); z = __uint_as_float(lo); kP = hi;
+    io.get2(3, lo, hi); z = __uint_as_float(lo); drawnP = (nP != NEVER || hi != 0u) ? hi + 1u : 0u;
     io.get2(4, lo, hi); gP = __uint_as_float(lo); gD = __uint_as_float(hi);
     io.get2(5, lo, hi); nD = (int)lo; fD = __uint_as_float(hi);
-    io.get2(6, lo, hi); kD = lo; d = (int)hi;
+    io.get2(6, lo, hi); drawnD = (nD != NEVER || lo != 0u) ? lo + 1u : 0u; d = (int)hi;
     ph = io.get(7);
     io.get2(8, lo, hi); drive0 = __uint_as_float(lo); snap_x = __uint_as_float(hi);
     io.get2(9, lo, hi); snap_w = (int)lo;
   }
+  cold[0 * T] = __float_as_uint(snap_x);
+  cold[1 * T] = (uint32_t)snap_w;
+  cold[2 * T] = drawnP;
+  cold[3 * T] = drawnD;
   int cov = min(nP, nD);  // cell of the last event known to this lane, minimum over the streams
   float cst = P.base + (HAS_D ? (d ? P.Gb : P.Ga) : 0.f);
   const float hh_full = 0.5f * dt;
@@ -449,7 +459,9 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
       }
       tailP = tc;
       if (cnt < EVQ && tc != NEVER) {
-        const uint4 w = philox_call(K, g, STREAM_POISSON, kP + (uint32_t)cnt + 1u);
+        const uint32_t drawn = cold[2 * T];
+        cold[2 * T] = drawn + 1u;
+        const uint4 w = philox_call(K, g, STREAM_POISSON, drawn);
         int c;
         float f;
         schedule_f32(tc, tf, dt, inv_dt, neg_log_u_f32(w.x) * P.inv_lam_dt, c, f);
@@ -475,7 +487,9 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
       }
       tailD = tc;
       if (cnt < EVQ && tc != NEVER) {
-        const uint4 w = philox_call(K, g, STREAM_DICH, kD + (uint32_t)cnt + 1u);
+        const uint32_t drawn = cold[3 * T];
+        cold[3 * T] = drawn + 1u;
+        const uint4 w = philox_call(K, g, STREAM_DICH, drawn);
         const int dn = d ^ ((cnt + 1) & 1);  // the state entered by the last queued flip
         int c;
         float f;
@@ -566,15 +580,12 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
     sub_step(h, HAS_G ? (isP ? gP : gD) : 0.f, HAS_G ? sqrt_approx(h * P.s2) : 0.f, dr_tau, dr1, true);  // Var ~ h (A9)
     dr_tau = dr1;
     tau = te;
-    jumps++;
     if (HAS_P && isP) {  // a8: kick
       if (!INERTIAL) x += z; else v += z;
-      kP++;
       pop_P();
     }
     if (HAS_D && !isP) {  // a8: flip
       d ^= 1;
-      kD++;
       cst = P.base + (d ? P.Gb : P.Ga);
       k0f = dt * cst;
       k0h = hh_full * cst;
@@ -644,8 +655,8 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
     if ((ctl >> j) & 0x100u) {
       if (n + j >= n_end) return false;
       fold_f32<POT>(x, wraps);
-      snap_x = x;
-      snap_w = wraps;
+      cold[0 * T] = __float_as_uint(x);
+      cold[1 * T] = (uint32_t)wraps;
     }
     return true;
   };
@@ -776,6 +787,13 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
     w = wn;
   }
 
+  // events applied per stream = events drawn - events still queued (the ring and the head); it is also the index of
+  // the stream's next event, i.e. of the Philox call it came from
+  const uint32_t kP = (HAS_P && cold[2 * T] > 0u) ? cold[2 * T] - (uint32_t)(qP >> 4) - 1u : 0u;
+  const uint32_t kD = (HAS_D && cold[3 * T] > 0u) ? cold[3 * T] - (uint32_t)(qD >> 4) - 1u : 0u;
+  const int jumps = (int)(kP + kD);
+  snap_x = __uint_as_float(cold[0 * T]);
+  snap_w = (int)cold[1 * T];
   if (a.state != nullptr && valid) {  // row f2: checkpoint
     const StateIO io = state_io(a, g);
     io.put2(0, __float_as_uint(x), (uint32_t)wraps);
