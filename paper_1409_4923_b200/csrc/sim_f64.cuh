@@ -159,7 +159,10 @@ __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimA
   StateF64 s[N], snap[N];
   int d[N];
   uint32_t kP[N], kD[N];
-  double rP[N], rD[N], z[N], rem[N], jumps[N], gq[N][4];
+  // normals in flight: one Philox block of four (a single launch), two blocks (CHUNKED, see the time loop)
+  constexpr int GQ = CHUNKED ? 8 : 4;
+  double rP[N], rD[N], z[N], rem[N], jumps[N], gq[N][GQ];
+  unsigned long long blk0[N];  // CHUNKED: Gaussian block the path was in when the launch started
   double *trace[N];
   long long n[N];
 #pragma unroll
@@ -190,23 +193,34 @@ __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimA
     m[q] = 0;
     rem[q] = dt;
     jumps[q] = 0.0;
-    gq[q][0] = gq[q][1] = gq[q][2] = gq[q][3] = 0.0;
+#pragma unroll
+    for (int j = 0; j < GQ; ++j) gq[q][j] = 0.0;
     snap[q] = s[q];
     if (CHUNKED && a.state != nullptr && a.step_begin > 0 && valid[q]) {  // row f2: continue a run from its checkpoint
       CkptF64 c;
       ckpt_load_f64(a, g[q], c);
       s[q].xi = c.xi; s[q].wraps = c.wraps; s[q].v = c.v; rP[q] = c.rP; rD[q] = c.rD; z[q] = c.z; kP[q] = c.kP; kD[q] = c.kD;
       d[q] = c.d; m[q] = c.m; jumps[q] = c.jumps; snap[q].xi = c.sxi; snap[q].wraps = c.swraps; snap[q].v = c.sv;
-      if (HAS_G && (m[q] & 3ull) != 0) {
-        double t[4];
-        regen_gauss_block_f64(a.keys, g[q], (uint32_t)(m[q] >> 2), t);
-        gq[q][0] = t[0]; gq[q][1] = t[1]; gq[q][2] = t[2]; gq[q][3] = t[3];
-      }
+    }
+    blk0[q] = m[q] >> 2;
+    if (CHUNKED && HAS_G) {  // the block the path is in (the next one is drawn in iteration 0 of the loop)
+      double t[4];
+      regen_gauss_block_f64(a.keys, g[q], (uint32_t)blk0[q], t);
+      const int o = (int)(blk0[q] & 1ull) * 4;
+#pragma unroll
+      for (int j = 0; j < 8; ++j)
+        if ((j & 4) == o) gq[q][j % GQ] = t[j & 3];
     }
     if (!valid[q]) n[q] = n_end;  // a path past the ragged end does nothing
   }
 
-  for (;;) {
+  // CHUNKED: a launch that resumes a run finds its paths at the same grid step but, after kicks or flips, at different
+  // sub-step counts m, i.e. at different places inside their Philox blocks of four normals; drawing a block whenever
+  // a lane runs out would then happen in every iteration for a quarter of the lanes.  Every iteration is one sub-step
+  // of every active lane, so instead each lane keeps TWO blocks and the whole warp draws the next one every fourth
+  // iteration: by then the older block is used up whatever the lane's phase.  (A single launch starts all lanes at
+  // m = 0; they stay in phase and one block is enough.)
+  for (unsigned long long it = 0;; ++it) {
     bool act[N], any = false;
 #pragma unroll
     for (int q = 0; q < N; ++q) { act[q] = n[q] < n_end; any |= act[q]; }
@@ -220,13 +234,32 @@ __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimA
       if (onD && rD[q] < h[q]) h[q] = rD[q];
       gn[q] = 0.0;
       if (HAS_G && act[q]) {
-        if ((m[q] & 3ull) == 0) {
-          const uint4 w = philox_call(a.keys, g[q], STREAM_GAUSS, (uint32_t)(m[q] >> 2));
-          box_muller_f64(w.x, w.y, gq[q][0], gq[q][1]);
-          box_muller_f64(w.z, w.w, gq[q][2], gq[q][3]);
+        if (!CHUNKED) {
+          if ((m[q] & 3ull) == 0) {
+            const uint4 w = philox_call(a.keys, g[q], STREAM_GAUSS, (uint32_t)(m[q] >> 2));
+            box_muller_f64(w.x, w.y, gq[q][0], gq[q][1]);
+            box_muller_f64(w.z, w.w, gq[q][2], gq[q][3]);
+          }
+          const int j = (int)(m[q] & 3ull);
+          gn[q] = (j == 0) ? gq[q][0] : (j == 1) ? gq[q][1] : (j == 2) ? gq[q][2] : gq[q][3];
+        } else {
+          if ((it & 3ull) == 0) {  // warp-uniform: the block after the one this iteration's normal comes from
+            const unsigned long long b = blk0[q] + (it >> 2) + 1ull;
+            const uint4 w = philox_call(a.keys, g[q], STREAM_GAUSS, (uint32_t)b);
+            double t0, t1, t2, t3;
+            box_muller_f64(w.x, w.y, t0, t1);
+            box_muller_f64(w.z, w.w, t2, t3);
+            const bool hi = (b & 1ull) != 0;
+            gq[q][0 % GQ] = hi ? gq[q][0 % GQ] : t0; gq[q][1 % GQ] = hi ? gq[q][1 % GQ] : t1;
+            gq[q][2 % GQ] = hi ? gq[q][2 % GQ] : t2; gq[q][3 % GQ] = hi ? gq[q][3 % GQ] : t3;
+            gq[q][4 % GQ] = hi ? t0 : gq[q][4 % GQ]; gq[q][5 % GQ] = hi ? t1 : gq[q][5 % GQ];
+            gq[q][6 % GQ] = hi ? t2 : gq[q][6 % GQ]; gq[q][7 % GQ] = hi ? t3 : gq[q][7 % GQ];
+          }
+          const int j = (int)(m[q] & 7ull);
+          const double lo = (j & 2) ? ((j & 1) ? gq[q][3 % GQ] : gq[q][2 % GQ]) : ((j & 1) ? gq[q][1 % GQ] : gq[q][0 % GQ]);
+          const double hi = (j & 2) ? ((j & 1) ? gq[q][7 % GQ] : gq[q][6 % GQ]) : ((j & 1) ? gq[q][5 % GQ] : gq[q][4 % GQ]);
+          gn[q] = (j & 4) ? hi : lo;
         }
-        const int j = (int)(m[q] & 3ull);
-        gn[q] = (j == 0) ? gq[q][0] : (j == 1) ? gq[q][1] : (j == 2) ? gq[q][2] : gq[q][3];
       }
       const double Gd = onD ? (d[q] ? P.Fb : -P.Fa) : 0.0;
       cst[q] = P.c0 + Gd;
