@@ -70,6 +70,15 @@ typedef enum { BM_SCHEME_JUMP_ADAPTED = 0, BM_SCHEME_PAPER_LITERAL = 1, BM_SCHEM
  *      Box-Muller pair instead of four).  AUTO = W16 (the variant measured fastest).
  * Ignored for BM_F64. */
 typedef enum { BM_GAUSS_AUTO = 0, BM_GAUSS_W32 = 1, BM_GAUSS_W16 = 2, BM_GAUSS_W16P = 3 } bm_gauss;
+/* BM_F32 over-damped jump-adapted kernels: how a warp steps onto the kick and flip times of its 32 paths (
+ * the divergence PAPER.md:412 leaves open).  CELLS: all lanes stay in the same grid cell; a cell in which some lane has
+ * an event is taken in two phases (event lanes integrate up to their events, then every lane finishes the cell).
+ * LANES: per-lane clocks -- inside a block of 8 grid cells every lane advances from its own (cell, offset) to its own
+ * next event or cell boundary, one sub-step per lane and pass, until every lane has reached the end of the block.
+ * AUTO: per PARAMETER POINT, LANES where the expected number of events per path and grid cell exceeds 0.02 (there
+ * nearly every cell of a warp holds an event), else CELLS -- the measured break-even.  The two
+ * forms perform the same operations per path: results are bit-identical whatever the mode. */
+typedef enum { BM_EVENTS_AUTO = 0, BM_EVENTS_CELLS = 1, BM_EVENTS_LANES = 2 } bm_event_mode;
 /* noise sources that are switched on; a source that is off ignores its parameters */
 enum { BM_NOISE_GAUSS = 1, BM_NOISE_POISSON = 2, BM_NOISE_DICH = 4 };
 
@@ -119,6 +128,8 @@ typedef struct {
                             for BM_F32 and the paper-literal scheme. */
   int32_t adapt_levels; /* BM_SCHEME_ADAPTIVE: how often dt may be halved, 0..20 */
   double adapt_tol;    /* BM_SCHEME_ADAPTIVE: tolerance on |chi| (in units of x), >= 0; +inf = never refine */
+  int32_t event_mode;  /* bm_event_mode; must be AUTO unless BM_F32, BM_OVERDAMPED, JUMP_ADAPTED (else BM_ERR_UNSUPPORTED) */
+  int32_t rsv;         /* 0 */
 } bm_config;
 
 /* per-path record written to out_paths: 6 doubles */

@@ -21,6 +21,7 @@ BM_POT_SINE2, BM_POT_PWL, BM_POT_QUAD = 0, 1, 2
 BM_SCHEME_JUMP_ADAPTED, BM_SCHEME_PAPER_LITERAL, BM_SCHEME_ADAPTIVE = 0, 1, 2
 BM_NOISE_GAUSS, BM_NOISE_POISSON, BM_NOISE_DICH = 1, 2, 4
 BM_GAUSS_AUTO, BM_GAUSS_W32, BM_GAUSS_W16, BM_GAUSS_W16P = 0, 1, 2, 3
+BM_EVENTS_AUTO, BM_EVENTS_CELLS, BM_EVENTS_LANES = 0, 1, 2
 BM_OUT_XT, BM_OUT_VT, BM_OUT_VBAR, BM_OUT_JUMPS, BM_OUT_SUBSTEPS, BM_OUT_XTI, BM_OUT_STRIDE = 0, 1, 2, 3, 4, 5, 6
 (BM_PROBE_FFMA, BM_PROBE_MUFU_COS, BM_PROBE_MUFU_LG2, BM_PROBE_MUFU_SQRT, BM_PROBE_IMAD_WIDE, BM_PROBE_LOP3,
  BM_PROBE_DFMA, BM_PROBE_I2F, BM_PROBE_FADD, BM_PROBE_MIX, BM_PROBE_COUNT) = range(11)
@@ -39,7 +40,8 @@ class BmConfig(C.Structure):
     _fields_ = [("model", C.c_int32), ("prec", C.c_int32), ("sincos", C.c_int32), ("potential", C.c_int32),
                 ("scheme", C.c_int32), ("noise", C.c_int32), ("block_threads", C.c_int32), ("gauss", C.c_int32),
                 ("n_discard", C.c_int64), ("trace_steps", C.c_int64), ("trace_paths", C.c_int64),
-                ("paths_per_thread", C.c_int32), ("adapt_levels", C.c_int32), ("adapt_tol", C.c_double)]
+                ("paths_per_thread", C.c_int32), ("adapt_levels", C.c_int32), ("adapt_tol", C.c_double),
+                ("event_mode", C.c_int32), ("rsv", C.c_int32)]
 
 
 class BmError(RuntimeError):
@@ -116,9 +118,10 @@ def noise_mask(params):
 
 def make_config(model=BM_OVERDAMPED, prec=BM_F32, sincos=BM_SINCOS_AUTO, potential=BM_POT_SINE2,
                 scheme=BM_SCHEME_JUMP_ADAPTED, noise=BM_NOISE_GAUSS, block_threads=0, n_discard=0, trace_steps=0,
-                trace_paths=0, gauss=BM_GAUSS_AUTO, paths_per_thread=0, adapt_tol=float("inf"), adapt_levels=0):
+                trace_paths=0, gauss=BM_GAUSS_AUTO, paths_per_thread=0, adapt_tol=float("inf"), adapt_levels=0,
+                event_mode=BM_EVENTS_AUTO):
     return BmConfig(model, prec, sincos, potential, scheme, noise, block_threads, gauss, n_discard, trace_steps,
-                    trace_paths, paths_per_thread, adapt_levels, adapt_tol)
+                    trace_paths, paths_per_thread, adapt_levels, adapt_tol, event_mode, 0)
 
 
 def _stream_ptr(stream):
@@ -280,19 +283,20 @@ def bm_pipe_probe(op, iters, blocks, threads, sink, stream=None):
 # ---- conveniences used by tests and bench.py (marshalling only) -------------------------------------------
 
 def config_for(w, prec, sincos=BM_SINCOS_AUTO, block_threads=0, trace_steps=0, trace_paths=0, gauss=BM_GAUSS_AUTO,
-               paths_per_thread=0):
+               paths_per_thread=0, event_mode=BM_EVENTS_AUTO):
     """bm_config of a workloads.Workload (extra: adapt_tol, adapt_levels for the adaptive scheme)."""
     return make_config(model=w.model, prec=prec, sincos=sincos, potential=w.potential, scheme=w.scheme,
                        noise=noise_mask(w.params), block_threads=block_threads, n_discard=w.n_discard,
                        trace_steps=trace_steps, trace_paths=trace_paths, gauss=gauss, paths_per_thread=paths_per_thread,
-                       adapt_tol=w.extra.get("adapt_tol", float("inf")), adapt_levels=w.extra.get("adapt_levels", 0))
+                       adapt_tol=w.extra.get("adapt_tol", float("inf")), adapt_levels=w.extra.get("adapt_levels", 0),
+                       event_mode=event_mode)
 
 
 def run_workload(w, prec, want_paths=False, sincos=BM_SINCOS_AUTO, block_threads=0, trace_steps=0, trace_paths=0,
-                 device="cuda:0", gauss=BM_GAUSS_AUTO, paths_per_thread=0):
+                 device="cuda:0", gauss=BM_GAUSS_AUTO, paths_per_thread=0, event_mode=BM_EVENTS_AUTO):
     """Run a Workload through bm_simulate; returns (stats[n_points,8], paths or None, trace or None) as numpy."""
     import torch
-    cfg = config_for(w, prec, sincos, block_threads, trace_steps, trace_paths, gauss, paths_per_thread)
+    cfg = config_for(w, prec, sincos, block_threads, trace_steps, trace_paths, gauss, paths_per_thread, event_mode)
     dev = torch.device(device)
     params = torch.from_numpy(np.ascontiguousarray(w.params)).to(dev)
     stats = torch.zeros((w.n_points, 8), dtype=torch.float64, device=dev)

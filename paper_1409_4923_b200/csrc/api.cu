@@ -38,6 +38,7 @@ bool valid_cfg(const bm_config *c) {
   if (c->gauss < BM_GAUSS_AUTO || c->gauss > BM_GAUSS_W16P) return false;
   if (c->paths_per_thread < 0 || c->paths_per_thread > 2) return false;
   if (c->n_discard < 0 || c->trace_steps < 0 || c->trace_paths < 0) return false;
+  if (c->event_mode < BM_EVENTS_AUTO || c->event_mode > BM_EVENTS_LANES) return false;
   return true;
 }
 
@@ -94,7 +95,26 @@ struct Launch {
   int gauss = 0;    // bm_gauss selected (fp32), 0 for fp64
   int ppt = 1;      // realizations per thread (fp64 jump-adapted kernels)
   size_t smem = 0;  // dynamic shared memory per block (event rings of the fp32 jump-adapted kernel)
+  // fp32 over-damped kernels with a jump source: the per-lane-clock form, launched on the same grid (every block is
+  // taken by exactly one of the two, by the event mode of its parameter point); fn is null when LANES is forced
+  KernelFn fn_lanes = nullptr;
+  size_t smem_lanes = 0;
 };
+
+bool has_event_modes(const bm_config *c) {
+  return c->prec == BM_F32 && c->model == BM_OVERDAMPED && c->scheme == BM_SCHEME_JUMP_ADAPTED &&
+         (c->noise & (BM_NOISE_POISSON | BM_NOISE_DICH));
+}
+
+bm_status opt_in_smem(KernelFn fn, size_t smem) {
+  // beyond the 48 KB default a kernel has to opt in (per function and device; repeating the call is harmless)
+  if (smem > 44 * 1024 &&  /* the kernels also hold 1792 B of static shared memory (block reduction) */
+      cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
+    cudaGetLastError();
+    return BM_ERR_CUDA;
+  }
+  return BM_OK;
+}
 
 bm_status pick_kernel(const bm_config *c, int32_t n_points, int64_t n_paths, Launch *L, bool chunked = false) {
   *L = Launch();
@@ -102,6 +122,7 @@ bm_status pick_kernel(const bm_config *c, int32_t n_points, int64_t n_paths, Lau
   if (c->scheme == BM_SCHEME_ADAPTIVE && (c->model != BM_OVERDAMPED || c->prec != BM_F64 || chunked)) return BM_ERR_UNSUPPORTED;
   if (c->model == BM_INERTIAL && c->potential != BM_POT_SINE2) return BM_ERR_UNSUPPORTED;
   if (c->paths_per_thread == 2 && !has_two_paths(c)) return BM_ERR_UNSUPPORTED;
+  if (c->event_mode != BM_EVENTS_AUTO && !has_event_modes(c)) return BM_ERR_UNSUPPORTED;
   L->threads = block_threads_of(c, n_points, n_paths);
   L->ppt = paths_per_thread_of(c, n_points, n_paths);
   if (c->scheme == BM_SCHEME_PAPER_LITERAL) {
@@ -112,7 +133,7 @@ bm_status pick_kernel(const bm_config *c, int32_t n_points, int64_t n_paths, Lau
     L->fn = c->model == BM_OVERDAMPED ? pick_f64_overdamped(c->potential, c->noise, chunked, L->ppt)
                                       : pick_f64_inertial(c->potential, c->noise, chunked, L->ppt);
   } else {
-    typedef KernelFn (*Picker)(int, int, int);
+    typedef KernelFn (*Picker)(int, int, int, int);
     static const Picker table[2][2][3] = {  // [model][sincos fma][gauss - 1]
         {{pick_f32_od_sfu_w32, pick_f32_od_sfu_w16, pick_f32_od_sfu_w16p},
          {pick_f32_od_fma_w32, pick_f32_od_fma_w16, pick_f32_od_fma_w16p}},
@@ -123,16 +144,21 @@ bm_status pick_kernel(const bm_config *c, int32_t n_points, int64_t n_paths, Lau
     // keep resident (5 blocks of 128 threads per SM); a function of the arguments only
     const long long threads_total = (long long)n_points * ((n_paths + L->threads - 1) / L->threads) * L->threads;
     const int occ = threads_total > (long long)DESIGN_SMS * 640 ? 1 : 0;
-    L->fn = table[c->model == BM_INERTIAL][resolve_sincos(c) == BM_SINCOS_FMA][L->gauss - 1](c->potential, c->noise, occ);
-    L->smem = (size_t)L->threads * sizeof(uint32_t) * (size_t)f32_smem_words_per_thread(c->noise, L->gauss);
+    const Picker pick = table[c->model == BM_INERTIAL][resolve_sincos(c) == BM_SINCOS_FMA][L->gauss - 1];
+    if (!has_event_modes(c) || c->event_mode != BM_EVENTS_LANES) {
+      L->fn = pick(c->potential, c->noise, occ, 0);
+      L->smem = (size_t)L->threads * sizeof(uint32_t) * (size_t)f32_smem_words_per_thread(c->noise, L->gauss);
+      if (!L->fn) return BM_ERR_UNSUPPORTED;
+    }
+    if (has_event_modes(c) && c->event_mode != BM_EVENTS_CELLS) {
+      L->fn_lanes = pick(c->potential, c->noise, occ, 1);
+      L->smem_lanes = (size_t)L->threads * sizeof(uint32_t) * (size_t)f32_smem_words_per_thread(c->noise, L->gauss, 1);
+      if (!L->fn_lanes) return BM_ERR_UNSUPPORTED;
+    }
   }
-  if (!L->fn) return BM_ERR_UNSUPPORTED;
-  // beyond the 48 KB default a kernel has to opt in (per function and device; repeating the call is harmless)
-  if (L->smem > 44 * 1024 &&  /* the kernels also hold 1792 B of static shared memory (block reduction) */
-      cudaFuncSetAttribute((const void *)L->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L->smem) != cudaSuccess) {
-    cudaGetLastError();
-    return BM_ERR_CUDA;
-  }
+  if (!L->fn && !L->fn_lanes) return BM_ERR_UNSUPPORTED;
+  if (L->fn && opt_in_smem(L->fn, L->smem) != BM_OK) return BM_ERR_CUDA;
+  if (L->fn_lanes && opt_in_smem(L->fn_lanes, L->smem_lanes) != BM_OK) return BM_ERR_CUDA;
   return BM_OK;
 }
 
@@ -250,11 +276,13 @@ static bm_status simulate_range(const bm_config *cfg, const bm_params *params, i
   a.step_end = step_end;
   a.adapt_tol = cfg->adapt_tol;
   a.adapt_levels = cfg->adapt_levels;
+  a.event_mode = cfg->event_mode;
   a.keys = make_keys(seed);
 
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   const unsigned grid = (unsigned)((long long)a.blocks_per_point * n_points);
-  L.fn<<<grid, L.threads, L.smem, st>>>(a);  // a1: (point x path) -> grid
+  if (L.fn) L.fn<<<grid, L.threads, L.smem, st>>>(a);  // a1: (point x path) -> grid
+  if (L.fn_lanes) L.fn_lanes<<<grid, L.threads, L.smem_lanes, st>>>(a);
   if (cudaGetLastError() != cudaSuccess) return BM_ERR_CUDA;
   if (step_end < n_steps) return BM_OK;  // the ensemble reduction belongs to the last chunk
   if (launch_grid_reduce(a.partials, n_points, a.blocks_per_point, out_stats, st) != cudaSuccess) return BM_ERR_CUDA;
@@ -391,9 +419,11 @@ BM_API bm_status bm_kernel_info(const bm_config *cfg, int32_t n_points, int64_t 
   const bm_status ps = pick_kernel(cfg, n_points, n_paths, &L);
   if (ps != BM_OK) return ps;
   cudaFuncAttributes attr;
-  if (cudaFuncGetAttributes(&attr, (const void *)L.fn) != cudaSuccess) { cudaGetLastError(); return BM_ERR_CUDA; }
+  const KernelFn fn = L.fn ? L.fn : L.fn_lanes;  // the per-lane-clock form when cfg forces it
+  const size_t smem = L.fn ? L.smem : L.smem_lanes;
+  if (cudaFuncGetAttributes(&attr, (const void *)fn) != cudaSuccess) { cudaGetLastError(); return BM_ERR_CUDA; }
   int nb = 0, dev = 0, sms = 0;
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, (const void *)L.fn, L.threads, L.smem) != cudaSuccess) { cudaGetLastError(); return BM_ERR_CUDA; }
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, (const void *)fn, L.threads, smem) != cudaSuccess) { cudaGetLastError(); return BM_ERR_CUDA; }
   if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
     cudaGetLastError();
     return BM_ERR_CUDA;

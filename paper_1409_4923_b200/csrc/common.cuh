@@ -38,6 +38,7 @@ struct SimArgs {
   long long step_begin, step_end;
   double adapt_tol;  // BM_SCHEME_ADAPTIVE (row f4): tolerance on |chi| and number of halvings of dt
   int adapt_levels;
+  int event_mode;    // bm_event_mode (fp32 over-damped jump-adapted kernels)
   PhiloxKeys keys;
 };
 
@@ -69,9 +70,24 @@ constexpr int EVQ = 8;  // ring capacity per path and stream (a power of two, <=
 constexpr int EVK = 4;  // refill passes per episode
 constexpr int EV_FIELDS_P = 4, EV_FIELDS_D = 3;  // (cell, off, amplitude, normal), (cell, off, normal)
 
-// 32-bit words of dynamic shared memory per thread of the fp32 path kernel (host and device agree through this)
-__host__ __device__ constexpr int f32_smem_words_per_thread(int noise, int gauss) {
-  return ((noise & BM_NOISE_POISSON) ? EVQ * EV_FIELDS_P : 0) + ((noise & BM_NOISE_DICH) ? EVQ * EV_FIELDS_D : 0) + 4 + 0 * gauss;
+// 32-bit words of dynamic shared memory per thread of the fp32 path kernel (host and device agree through this);
+// lclk: the per-lane-clock form also keeps the normals of one Gaussian call (NB angle parts, NB/2 radii)
+__host__ __device__ constexpr int f32_smem_words_per_thread(int noise, int gauss, int lclk = 0) {
+  const int rings = ((noise & BM_NOISE_POISSON) ? EVQ * EV_FIELDS_P : 0) + ((noise & BM_NOISE_DICH) ? EVQ * EV_FIELDS_D : 0) + 4;
+  // LANES form: one record per thread, with the normals of one Gaussian call, padded to an odd number of words
+  return lclk ? ((rings + ((noise & BM_NOISE_GAUSS) ? (gauss == BM_GAUSS_W32 ? 6 : 12) : 0)) | 1) : rings;
+}
+
+// Event mode of a parameter point (fp32 over-damped jump-adapted kernels; sim_f32.cuh, "per-lane clocks"): expected
+// kicks + flips per path and grid cell above LCLK_EVENTS_PER_CELL.  A function of the point's parameters and step
+// length only (in double), evaluated alike by both forms of the kernel, so every block is taken by exactly one.
+constexpr double LCLK_EVENTS_PER_CELL = 0.02;
+__device__ __forceinline__ bool lane_clock_point(const SimArgs &a, const bm_params &bp, double dt, int noise) {
+  if (a.event_mode != BM_EVENTS_AUTO) return a.event_mode == BM_EVENTS_LANES;
+  double rate = 0.0;
+  if ((noise & BM_NOISE_POISSON) && bp.lambda > 0.0) rate += bp.lambda;
+  if ((noise & BM_NOISE_DICH) && bp.mu_a > 0.0) rate += 0.5 * (bp.mu_a + (bp.mu_b > 0.0 ? bp.mu_b : 0.0));
+  return rate * dt > LCLK_EVENTS_PER_CELL;
 }
 
 constexpr uint32_t PHILOX_M0 = 0xD2511F53u, PHILOX_M1 = 0xCD9E8D57u;

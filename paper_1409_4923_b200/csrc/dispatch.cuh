@@ -9,18 +9,18 @@ typedef void (*KernelFn)(const SimArgs);
 KernelFn pick_f64_overdamped(int potential, int noise, bool chunked, int paths_per_thread);
 KernelFn pick_f64_inertial(int potential, int noise, bool chunked, int paths_per_thread);
 // fp32: one family per (model, sincos, gauss) triple (BM_SINCOS_AUTO / BM_GAUSS_AUTO are resolved by the caller)
-KernelFn pick_f32_od_sfu_w16(int potential, int noise, int occ);
-KernelFn pick_f32_od_sfu_w32(int potential, int noise, int occ);
-KernelFn pick_f32_od_fma_w16(int potential, int noise, int occ);
-KernelFn pick_f32_od_fma_w32(int potential, int noise, int occ);
-KernelFn pick_f32_in_sfu_w16(int potential, int noise, int occ);
-KernelFn pick_f32_in_sfu_w32(int potential, int noise, int occ);
-KernelFn pick_f32_in_fma_w16(int potential, int noise, int occ);
-KernelFn pick_f32_in_fma_w32(int potential, int noise, int occ);
-KernelFn pick_f32_od_sfu_w16p(int potential, int noise, int occ);
-KernelFn pick_f32_od_fma_w16p(int potential, int noise, int occ);
-KernelFn pick_f32_in_sfu_w16p(int potential, int noise, int occ);
-KernelFn pick_f32_in_fma_w16p(int potential, int noise, int occ);
+KernelFn pick_f32_od_sfu_w16(int potential, int noise, int occ, int lclk);
+KernelFn pick_f32_od_sfu_w32(int potential, int noise, int occ, int lclk);
+KernelFn pick_f32_od_fma_w16(int potential, int noise, int occ, int lclk);
+KernelFn pick_f32_od_fma_w32(int potential, int noise, int occ, int lclk);
+KernelFn pick_f32_in_sfu_w16(int potential, int noise, int occ, int lclk);
+KernelFn pick_f32_in_sfu_w32(int potential, int noise, int occ, int lclk);
+KernelFn pick_f32_in_fma_w16(int potential, int noise, int occ, int lclk);
+KernelFn pick_f32_in_fma_w32(int potential, int noise, int occ, int lclk);
+KernelFn pick_f32_od_sfu_w16p(int potential, int noise, int occ, int lclk);
+KernelFn pick_f32_od_fma_w16p(int potential, int noise, int occ, int lclk);
+KernelFn pick_f32_in_sfu_w16p(int potential, int noise, int occ, int lclk);
+KernelFn pick_f32_in_fma_w16p(int potential, int noise, int occ, int lclk);
 
 // the paper's own scheme as printed (sim_literal.cu); over-damped only
 KernelFn pick_literal(int prec, int potential, int noise);

@@ -121,7 +121,7 @@ __device__ __forceinline__ float stage_f32(float base, float x, float k1, float 
     float y = x;
     y = (y >= 1.0f) ? y - 2.0f : y;
     y = (y < -1.0f) ? y + 2.0f : y;
-    return base + ((y >= 0.0f) ? k1 : -k1);
+    return __fadd_rn(base, (y >= 0.0f) ? k1 : -k1);
   } else {
     return fmaf(-k1, x, base);
   }
@@ -134,7 +134,7 @@ __device__ __forceinline__ float stage_f32(float base, float x, float k1, float 
 template <int POT, int SINCOS>
 __device__ __forceinline__ float pc_overdamped_f32(float xarg, float xs, float k0, float k1, float k2, float k0h,
                                                    float k1h, float k2h) {
-  const float x1 = stage_f32<POT, SINCOS>(xs + k0, xarg, k1, k2);
+  const float x1 = stage_f32<POT, SINCOS>(__fadd_rn(xs, k0), xarg, k1, k2);  // never contracted with k0 = h K0
   const float xh = fmaf(0.5f, x1, fmaf(0.5f, xs, k0h));
   const float x2 = stage_f32<POT, SINCOS>(xh, x1, k1h, k2h);
   return stage_f32<POT, SINCOS>(xh, x2, k1h, k2h);
@@ -309,11 +309,13 @@ struct PointF32 {
   float w_turns;     // omega/(2 pi): drive turns per unit time
 };
 
-template <int MODEL, int POT, int NOISE, int SINCOS, int GW, int OCC>
+template <int MODEL, int POT, int NOISE, int SINCOS, int GW, int OCC, int LCLK = 0>
 __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ SimArgs a) {
   constexpr bool HAS_G = NOISE & BM_NOISE_GAUSS, HAS_P = NOISE & BM_NOISE_POISSON, HAS_D = NOISE & BM_NOISE_DICH;
   constexpr bool HAS_EV = HAS_P || HAS_D;
   constexpr bool INERTIAL = MODEL == BM_INERTIAL;
+  static_assert(!LCLK || (HAS_EV && !INERTIAL), "per-lane clocks: over-damped model with a jump source");
+  static_assert(EVQ == 8, "the ring pop of the per-lane-clock form clears bit 3 of the read slot");
   constexpr int NB = GaussLayout<GW>::NB, NP = GaussLayout<GW>::NP;  // grid cells, pairs per Gaussian call
   constexpr float S = Units<POT>::SCALE;
   constexpr unsigned FULL = 0xffffffffu;
@@ -322,13 +324,20 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
 
   extern __shared__ uint32_t smem_words[];
   const int T = blockDim.x, tid = threadIdx.x;
-  uint32_t *const ringP = smem_words + tid;               // [EVQ][NFP][T]
-  uint32_t *const ringD = ringP + EVQ * NFP * T;          // [EVQ][NFD][T]
+  // CELLS form: field-major arrays [slot][field][thread] (conflict-free whatever slot each lane is at; the strides are
+  // run-time values).  LANES form: one record of REC words per thread, [ring P][ring D][cold][normals], REC odd: every
+  // offset inside the record is an immediate, the few lanes that pop an event in a pass rarely share a bank.
+  constexpr int RECW = EVQ * NFP + EVQ * NFD + 4 + (HAS_G ? NB + NP : 0), REC = RECW | 1;
+  const int FS = LCLK ? 1 : T;                              // stride between the fields of one slot
+  const int SSP = LCLK ? NFP : NFP * T, SSD = LCLK ? NFD : NFD * T;  // stride between ring slots
+  uint32_t *const ringP = LCLK ? smem_words + tid * REC : smem_words + tid;
+  uint32_t *const ringD = LCLK ? ringP + EVQ * NFP : ringP + EVQ * NFP * T;
   // state that is touched a few times per run lives in shared memory, not in registers (the 64-register class of the
   // over-damped kernel re-materialises loop constants otherwise): the snapshot at t_i and, per stream, the number of
   // events drawn so far.  The index of a stream's next event = events drawn - events queued - 1 = events applied, so
   // no counter has to follow the events themselves.
-  uint32_t *const cold = ringD + EVQ * NFD * T;           // [4][T]: snap_x, snap_w, drawnP, drawnD
+  uint32_t *const cold = LCLK ? ringD + EVQ * NFD : ringD + EVQ * NFD * T;  // [4]: snap_x, snap_w, drawnP, drawnD
+  uint32_t *const nrm = cold + 4;  // LANES: the block's normals, angle parts [NB] then radii [NP]
 
   const int point = blockIdx.x / a.blocks_per_point;
   const int chunk = blockIdx.x - point * a.blocks_per_point;
@@ -339,6 +348,8 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
 
   const PhiloxKeys &K = a.keys;
   const bm_params bp = a.params[point];
+  // the two forms of the kernel share a launch grid: each takes the parameter points of its own event mode
+  if (HAS_EV && MODEL == BM_OVERDAMPED && lane_clock_point(a, bp, step_length(a, point), NOISE) != (LCLK != 0)) return;
   const double Dd = HAS_G ? bp.D : 0.0;
   const double dtd = step_length(a, point);
   const float dt = (float)dtd;
@@ -453,16 +464,18 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
     io.get2(8, lo, hi); drive0 = __uint_as_float(lo); snap_x = __uint_as_float(hi);
     io.get2(9, lo, hi); snap_w = (int)lo;
   }
-  cold[0 * T] = __float_as_uint(snap_x);
-  cold[1 * T] = (uint32_t)snap_w;
-  cold[2 * T] = drawnP;
-  cold[3 * T] = drawnD;
+  cold[0 * FS] = __float_as_uint(snap_x);
+  cold[1 * FS] = (uint32_t)snap_w;
+  cold[2 * FS] = drawnP;
+  cold[3 * FS] = drawnD;
   int cov = min(nP, nD);  // cell of the last event known to this lane, minimum over the streams
   float cst = P.base + (HAS_D ? (d ? P.Gb : P.Ga) : 0.f);
   const float hh_full = 0.5f * dt;
   // full-step constants of Alg. 1 (loop invariant; k0f, k0h follow cst across a flip)
-  const float k1f = dt * P.kk1, k2f = dt * P.kk2, k1h = hh_full * P.kk1, k2h = hh_full * P.kk2;
-  float k0f = dt * cst, k0h = hh_full * cst;
+  // (products by __fmul_rn: the compiler must not contract them into the additions that follow, or the CELLS and the
+  // LANES form of the kernel, and fast_cell and sub_step, would round differently)
+  const float k1f = __fmul_rn(dt, P.kk1), k2f = __fmul_rn(dt, P.kk2), k1h = __fmul_rn(hh_full, P.kk1), k2h = __fmul_rn(hh_full, P.kk2);
+  float k0f = __fmul_rn(dt, cst), k0h = __fmul_rn(hh_full, cst);
 
   // ---- one refill pass: every lane with room appends one event per stream; returns whether this lane still has a
   //      stream whose last event lies before `limit` and whose ring has room ------------------------------------
@@ -475,22 +488,22 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
       float tf = fP;
       if (cnt > 0) {
         const int s = (rd + cnt - 1) & (EVQ - 1);
-        tc = (int)ringP[(s * NFP + 0) * T];
-        tf = __uint_as_float(ringP[(s * NFP + 1) * T]);
+        tc = (int)ringP[s * SSP + 0 * FS];
+        tf = __uint_as_float(ringP[s * SSP + 1 * FS]);
       }
       tailP = tc;
       if (cnt < EVQ && tc != NEVER) {
-        const uint32_t drawn = cold[2 * T];
-        cold[2 * T] = drawn + 1u;
+        const uint32_t drawn = cold[2 * FS];
+        cold[2 * FS] = drawn + 1u;
         const uint4 w = philox_call(K, g, STREAM_POISSON, drawn);
         int c;
         float f;
         schedule_f32(tc, tf, dt, inv_dt, neg_log_u_f32(w.x) * P.inv_lam_dt, c, f);
         const int s = (rd + cnt) & (EVQ - 1);
-        ringP[(s * NFP + 0) * T] = (uint32_t)c;
-        ringP[(s * NFP + 1) * T] = __float_as_uint(f);
-        ringP[(s * NFP + 2) * T] = __float_as_uint(P.zeta * neg_log_u_f32(w.y));
-        if (HAS_G) ringP[(s * NFP + 3) * T] = __float_as_uint(event_normal(w.z));
+        ringP[s * SSP + 0 * FS] = (uint32_t)c;
+        ringP[s * SSP + 1 * FS] = __float_as_uint(f);
+        ringP[s * SSP + 2 * FS] = __float_as_uint(P.zeta * neg_log_u_f32(w.y));
+        if (HAS_G) ringP[s * SSP + 3 * FS] = __float_as_uint(event_normal(w.z));
         qP += 16;
         tailP = c;
         did = true;
@@ -503,22 +516,22 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
       float tf = fD;
       if (cnt > 0) {
         const int s = (rd + cnt - 1) & (EVQ - 1);
-        tc = (int)ringD[(s * NFD + 0) * T];
-        tf = __uint_as_float(ringD[(s * NFD + 1) * T]);
+        tc = (int)ringD[s * SSD + 0 * FS];
+        tf = __uint_as_float(ringD[s * SSD + 1 * FS]);
       }
       tailD = tc;
       if (cnt < EVQ && tc != NEVER) {
-        const uint32_t drawn = cold[3 * T];
-        cold[3 * T] = drawn + 1u;
+        const uint32_t drawn = cold[3 * FS];
+        cold[3 * FS] = drawn + 1u;
         const uint4 w = philox_call(K, g, STREAM_DICH, drawn);
         const int dn = d ^ ((cnt + 1) & 1);  // the state entered by the last queued flip
         int c;
         float f;
         schedule_f32(tc, tf, dt, inv_dt, neg_log_u_f32(w.x) * (dn ? P.inv_mub_dt : P.inv_mua_dt), c, f);
         const int s = (rd + cnt) & (EVQ - 1);
-        ringD[(s * NFD + 0) * T] = (uint32_t)c;
-        ringD[(s * NFD + 1) * T] = __float_as_uint(f);
-        if (HAS_G) ringD[(s * NFD + 2) * T] = __float_as_uint(event_normal(w.z));
+        ringD[s * SSD + 0 * FS] = (uint32_t)c;
+        ringD[s * SSD + 1 * FS] = __float_as_uint(f);
+        if (HAS_G) ringD[s * SSD + 2 * FS] = __float_as_uint(event_normal(w.z));
         qD += 16;
         tailD = c;
         did = true;
@@ -541,18 +554,18 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
   auto pop_P = [&]() {
     if ((qP >> 4) == 0) { nP = NEVER; return; }  // not reached: a popped event always has a queued successor
     const int s = qP & 15;
-    nP = (int)ringP[(s * NFP + 0) * T];
-    fP = __uint_as_float(ringP[(s * NFP + 1) * T]);
-    z = __uint_as_float(ringP[(s * NFP + 2) * T]);
-    if (HAS_G) gP = __uint_as_float(ringP[(s * NFP + 3) * T]);
+    nP = (int)ringP[s * SSP + 0 * FS];
+    fP = __uint_as_float(ringP[s * SSP + 1 * FS]);
+    z = __uint_as_float(ringP[s * SSP + 2 * FS]);
+    if (HAS_G) gP = __uint_as_float(ringP[s * SSP + 3 * FS]);
     qP = ((qP & ~15) - 16) | ((s + 1) & (EVQ - 1));
   };
   auto pop_D = [&]() {
     if ((qD >> 4) == 0) { nD = NEVER; return; }
     const int s = qD & 15;
-    nD = (int)ringD[(s * NFD + 0) * T];
-    fD = __uint_as_float(ringD[(s * NFD + 1) * T]);
-    if (HAS_G) gD = __uint_as_float(ringD[(s * NFD + 2) * T]);
+    nD = (int)ringD[s * SSD + 0 * FS];
+    fD = __uint_as_float(ringD[s * SSD + 1 * FS]);
+    if (HAS_G) gD = __uint_as_float(ringD[s * SSD + 2 * FS]);
     qD = ((qD & ~15) - 16) | ((s + 1) & (EVQ - 1));
   };
 
@@ -583,7 +596,8 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
     if (refold || POT != BM_POT_SINE2) { wraps = wf; x = xf; } else xf = x;
     if (!INERTIAL) {
       const float xs = HAS_G ? fmaf(na, nb, xf) : xf;
-      x = pc_overdamped_f32<POT, SINCOS>(xf, xs, h * cst, h * P.kk1, h * P.kk2, hh * cst, hh * P.kk1, hh * P.kk2);
+      x = pc_overdamped_f32<POT, SINCOS>(xf, xs, __fmul_rn(h, cst), __fmul_rn(h, P.kk1), __fmul_rn(h, P.kk2), __fmul_rn(hh, cst),
+                                         __fmul_rn(hh, P.kk1), __fmul_rn(hh, P.kk2));
     } else {
       const float vs = HAS_G ? fmaf(na, nb, v) : v;
       pc_inertial_f32<SINCOS>(x, v, xf, vs, h, hh, P.gamma, P.kk1, P.kk2, cst + dr0, cst + dr1);
@@ -602,14 +616,14 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
     dr_tau = dr1;
     tau = te;
     if (HAS_P && isP) {  // a8: kick
-      if (!INERTIAL) x += z; else v += z;
+      if (!INERTIAL) x = __fadd_rn(x, z); else v += z;
       pop_P();
     }
     if (HAS_D && !isP) {  // a8: flip
       d ^= 1;
       cst = P.base + (d ? P.Gb : P.Ga);
-      k0f = dt * cst;
-      k0h = hh_full * cst;
+      k0f = __fmul_rn(dt, cst);
+      k0h = __fmul_rn(hh_full, cst);
       pop_D();
     }
   };
@@ -676,8 +690,8 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
     if ((ctl >> j) & 0x100u) {
       if (n + j >= n_end) return false;
       fold_f32<POT>(x, wraps);
-      cold[0 * T] = __float_as_uint(x);
-      cold[1 * T] = (uint32_t)wraps;
+      cold[0 * FS] = __float_as_uint(x);
+      cold[1 * FS] = (uint32_t)wraps;
     }
     return true;
   };
@@ -717,13 +731,118 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
         careful = __any_sync(FULL, cov < n + NB);  // a lane with more than EVQ events in this block
       }
       unsigned ctl = 0;
-      if (HAS_EV) ctl = __reduce_or_sync(FULL, ev_bits(n)) & 0xFFu;
+      if (HAS_EV && !LCLK) ctl = __reduce_or_sync(FULL, ev_bits(n)) & 0xFFu;
       if (special) {
         if ((unsigned)(n_discard - n) < (unsigned)NB) ctl |= 0x100u << (n_discard - n);
         if (n + NB > n_end) ctl |= (0xFF00u << (n_end - n)) & 0xFF00u;
       }
       fold_f32<POT>(x, wraps);
-      if (UNROLLED && !careful) {
+      if (LCLK && !careful && !special) {
+        // PER-LANE CLOCKS (covered block): every lane walks through the block on its own -- one sub-step per pass,
+        // from its (cell j, offset tau) to its next event in that cell or to the cell's end -- and the warp leaves
+        // the block when its slowest lane has.  Per lane the operations are those of the CELLS form: a cell the lane
+        // crosses without an event of its own is fast_cell, a sub-step that ends on an event is do_event's, the rest
+        // of a cell after its last event is finish_cell's.  The block's normals are needed at a per-lane index, so
+        // they go through shared memory (angle parts [NB], radii [NP]; each thread reads back its own words only).
+        if (HAS_G) {
+          philox_rounds<0, 10>(wn, K);
+          nrm[0] = __float_as_uint(cur.c);
+          nrm[1] = __float_as_uint(cur.s);
+          nrm[NB] = __float_as_uint(cur.r);
+#pragma unroll
+          for (int i = 1; i < NP; ++i) {
+            const Pair q = pair_of<GW>(w, i, P.cn);
+            nrm[2 * i] = __float_as_uint(q.c);
+            nrm[2 * i + 1] = __float_as_uint(q.s);
+            nrm[NB + i] = __float_as_uint(q.r);
+          }
+          cur = pair_of<GW>(wn, 0, P.cn);
+        }
+        int c = n;  // the lane's cell
+        float tau = 0.f;
+        for (;;) {
+          const bool act = c < n + NB;
+          if (!__any_sync(FULL, act)) break;
+          if (act) {
+            const bool evP = HAS_P && nP == c, evD = HAS_D && nD == c;
+            const bool ev = evP || evD;
+            const bool isP = evP && (!evD || fP <= fD);  // a tie applies the kick first (R5), as do_event
+            const float te = ev ? (isP ? fP : fD) : dt;
+            const bool whole = !ev && tau == 0.f;
+            const float h = fmaxf(te - tau, 0.f);
+            float na = 0.f, nb = 0.f;
+            if (HAS_G) {
+              const int j = c - n;
+              const float gc = __uint_as_float(nrm[j]), gr = __uint_as_float(nrm[NB + (j >> 1)]);
+              const float sq = sqrt_approx(h * (ev ? P.s2 : inv_dt));
+              na = ev ? (isP ? gP : gD) : (whole ? gr : gr * gc);
+              nb = whole ? gc : sq;
+            }
+            // sub_step(h, na, nb, ., ., !whole) with the re-fold as a select on the rounding constant
+            {
+              float xf = x;
+              if (POT != BM_POT_QUAD) {
+                float t = fmaf(x, Units<POT>::INV_PERIOD_TH, MAGIC_F);
+                if (whole && POT == BM_POT_SINE2) t = MAGIC_F;  // no re-fold: zero periods taken off, exactly
+                xf = fmaf(t - MAGIC_F, -Units<POT>::PERIOD_TH, x);
+                wraps += __float_as_int(t) - MAGIC_BITS;
+              }
+              const float hh = 0.5f * h;
+              const float xs = HAS_G ? fmaf(na, nb, xf) : xf;
+              x = pc_overdamped_f32<POT, SINCOS>(xf, xs, __fmul_rn(h, cst), __fmul_rn(h, P.kk1), __fmul_rn(h, P.kk2), __fmul_rn(hh, cst),
+                                                 __fmul_rn(hh, P.kk1), __fmul_rn(hh, P.kk2));
+            }
+            tau = ev ? te : 0.f;
+            c += ev ? 0 : 1;
+            if (HAS_P && isP) {  // a8: kick
+              x = __fadd_rn(x, z);
+              const int s = qP & 15;
+              nP = (int)ringP[s * NFP + 0];
+              fP = __uint_as_float(ringP[s * NFP + 1]);
+              z = __uint_as_float(ringP[s * NFP + 2]);
+              if (HAS_G) gP = __uint_as_float(ringP[s * NFP + 3]);
+              qP = (qP - 15) & ~EVQ;  // one event less queued, read slot + 1 modulo EVQ
+            }
+            if (HAS_D && ev && !isP) {  // a8: flip
+              d ^= 1;
+              cst = P.base + (d ? P.Gb : P.Ga);
+              k0f = __fmul_rn(dt, cst);
+              k0h = __fmul_rn(hh_full, cst);
+              const int s = qD & 15;
+              nD = (int)ringD[s * NFD + 0];
+              fD = __uint_as_float(ringD[s * NFD + 1]);
+              if (HAS_G) gD = __uint_as_float(ringD[s * NFD + 2]);
+              qD = (qD - 15) & ~EVQ;
+            }
+          }
+        }
+      } else if (LCLK || careful) {
+        // CAREFUL (some lane has more events in this block than its ring holds; in the per-lane-clock form also the
+        // two blocks that hold t_i and the end of the run): every cell is taken as a slow cell,
+        // in turns of one event per lane with a refill before each turn, so that a lane's next event is always
+        // known before it is needed.  Same arithmetic per lane as the covered path.
+        if (HAS_G) philox_rounds<0, 10>(wn, K);
+#pragma unroll 1
+        for (int i = 0; i < NP; ++i) {
+          Pair nxt = cur;
+          if (HAS_G) nxt = pair_dyn(w, wn, i);
+#pragma unroll 1
+          for (int jj = 0; jj < 2; ++jj) {
+            const int j = 2 * i + jj, c = n + j;
+            if (!special_cell(n, j, ctl)) break;
+            float tau = 0.f, dr_tau = drive0;
+            const float phf = INERTIAL ? __uint_as_float((uint32_t)(ph >> 41) | 0x3F800000u) : 0.f;
+            for (;;) {  // uniform over the warp
+              if (__any_sync(FULL, cov <= c)) refill_episode(c + 1);
+              const bool mine = (HAS_P && nP == c) || (HAS_D && nD == c);
+              if (!__any_sync(FULL, mine)) break;
+              if (mine) do_event(tau, dr_tau, phf);
+            }
+            finish_cell(cur.r, jj ? cur.s : cur.c, tau, dr_tau);
+          }
+          cur = nxt;
+        }
+      } else if (UNROLLED) {
         // COVERED, pair slot by pair slot, unrolled: a slot without event or special cell is the clean path's code
         // for two cells (with the next block's Philox rounds and Box-Muller pair formed alongside, as there)
 #pragma unroll
@@ -752,7 +871,7 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
           }
           cur = nxt;
         }
-      } else if (!careful) {
+      } else {
         // COVERED, rolled over the pair slots (one copy of the slow-cell code)
         if (HAS_G) philox_rounds<0, 10>(wn, K);
 #pragma unroll 1
@@ -778,31 +897,6 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
           }
           cur = nxt;
         }
-      } else {
-        // CAREFUL (some lane has more events in this block than its ring holds): every cell is taken as a slow cell,
-        // in turns of one event per lane with a refill before each turn, so that a lane's next event is always
-        // known before it is needed.  Same arithmetic per lane as the covered path.
-        if (HAS_G) philox_rounds<0, 10>(wn, K);
-#pragma unroll 1
-        for (int i = 0; i < NP; ++i) {
-          Pair nxt = cur;
-          if (HAS_G) nxt = pair_dyn(w, wn, i);
-#pragma unroll 1
-          for (int jj = 0; jj < 2; ++jj) {
-            const int j = 2 * i + jj, c = n + j;
-            if (!special_cell(n, j, ctl)) break;
-            float tau = 0.f, dr_tau = drive0;
-            const float phf = INERTIAL ? __uint_as_float((uint32_t)(ph >> 41) | 0x3F800000u) : 0.f;
-            for (;;) {  // uniform over the warp
-              if (__any_sync(FULL, cov <= c)) refill_episode(c + 1);
-              const bool mine = (HAS_P && nP == c) || (HAS_D && nD == c);
-              if (!__any_sync(FULL, mine)) break;
-              if (mine) do_event(tau, dr_tau, phf);
-            }
-            finish_cell(cur.r, jj ? cur.s : cur.c, tau, dr_tau);
-          }
-          cur = nxt;
-        }
       }
     }
     w = wn;
@@ -810,11 +904,11 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
 
   // events applied per stream = events drawn - events still queued (the ring and the head); it is also the index of
   // the stream's next event, i.e. of the Philox call it came from
-  const uint32_t kP = (HAS_P && cold[2 * T] > 0u) ? cold[2 * T] - (uint32_t)(qP >> 4) - 1u : 0u;
-  const uint32_t kD = (HAS_D && cold[3 * T] > 0u) ? cold[3 * T] - (uint32_t)(qD >> 4) - 1u : 0u;
+  const uint32_t kP = (HAS_P && cold[2 * FS] > 0u) ? cold[2 * FS] - (uint32_t)(qP >> 4) - 1u : 0u;
+  const uint32_t kD = (HAS_D && cold[3 * FS] > 0u) ? cold[3 * FS] - (uint32_t)(qD >> 4) - 1u : 0u;
   const int jumps = (int)(kP + kD);
-  snap_x = __uint_as_float(cold[0 * T]);
-  snap_w = (int)cold[1 * T];
+  snap_x = __uint_as_float(cold[0 * FS]);
+  snap_w = (int)cold[1 * FS];
   if (a.state != nullptr && valid) {  // row f2: checkpoint
     const StateIO io = state_io(a, g);
     io.put2(0, __float_as_uint(x), (uint32_t)wraps);
