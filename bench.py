@@ -263,6 +263,14 @@ FP64_OPS_PER_SUBSTEP = {0: 136.0, 1: 190.0}
 FP64_LANES_PER_SM = 64        # DFMA lanes per SM per clock (bm_pipe_probe: 63)
 
 
+def launches_per_call(B, w, prec_name):
+    """Kernels one bm_simulate call launches: the path kernel and the grid pass of the reduction; the fp32 over-damped
+    jump-adapted kernel with a jump source on is launched in both of its forms (CELLS, LANES) on the same grid."""
+    two_forms = (prec_name == "f32" and w.model == W.OVERDAMPED and w.scheme == W.SCHEME_JUMP_ADAPTED
+                 and (B.noise_mask(w.params) & 6) != 0)
+    return 3 if two_forms else 2
+
+
 def roofline_of(B, w, prec_name, stats, ms_per_step, clocks, info):
     """Roofline of the path kernel (the grid pass is < 0.1 % of a step).  fp32: bound by the XU (MUFU) pipe, algorithmic
     operation count; fp64: the FP64 pipe, instruction count of the kernel as built.  Peak = lanes x SMs x the SM clock
@@ -406,7 +414,7 @@ def run_ours(args):
                                                 "sincos": args.sincos, "substeps_per_step": roof["substeps_per_step"]}),
             "ms_median": float(np.median(ms)), "ms_best": float(min(ms)),
             "substeps_per_s": world * roof["substeps_per_step"] * w.path_steps / (ms_per_step * 1e-3),
-            "clocks": clocks, "e2e": e2e, "gpu_launches": 2 * args.steps, "roofline": roof,
+            "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_call(B, w, args.prec) * args.steps, "roofline": roof,
             "result": {"mean_v": float(stats[0, 1]), "var_v": float(stats[0, 2]), "mean_jumps": jumps}}
 
     # every BASELINE.json config and both precisions beside the headline (3 warm-up + 3 timed full-size steps each)
@@ -426,7 +434,7 @@ def run_ours(args):
                                                                    "regs_per_thread", "launch_threads", "blocks_per_sm",
                                                                    "substeps_per_step")},
                                    "clocks": ck2, "mean_v_point0": float(st2[0, 1])}
-            launches += 2 * 6
+            launches += launches_per_call(B, wc, pn) * 3
             del r2
         line["per_config"] = per
         line["gpu_launches"] += launches

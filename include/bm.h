@@ -73,11 +73,13 @@ typedef enum { BM_GAUSS_AUTO = 0, BM_GAUSS_W32 = 1, BM_GAUSS_W16 = 2, BM_GAUSS_W
 /* BM_F32 over-damped jump-adapted kernels: how a warp steps onto the kick and flip times of its 32 paths (
  * the divergence PAPER.md:412 leaves open).  CELLS: all lanes stay in the same grid cell; a cell in which some lane has
  * an event is taken in two phases (event lanes integrate up to their events, then every lane finishes the cell).
- * LANES: per-lane clocks -- inside a block of 8 grid cells every lane advances from its own (cell, offset) to its own
- * next event or cell boundary, one sub-step per lane and pass, until every lane has reached the end of the block.
+ * LANES: per-lane clocks -- every lane advances from its own (cell, offset) to its own next event or cell boundary, one
+ * sub-step per lane and pass; the warp only agrees on a sliding window of two blocks of 8 grid cells (a lane that is
+ * a block ahead of the slowest one waits), so a pass costs the same however the events are spread over the lanes.
  * AUTO: per PARAMETER POINT, LANES where the expected number of events per path and grid cell exceeds 0.02 (there
- * nearly every cell of a warp holds an event), else CELLS -- the measured break-even.  The two
- * forms perform the same operations per path: results are bit-identical whatever the mode. */
+ * about every second cell of a warp holds an event), else CELLS -- the measured break-even.
+ * The two forms perform the same operations per path: results are bit-identical whatever the mode.  With a jump
+ * source on, bm_simulate launches both forms on the same grid (each block is taken by exactly one of them). */
 typedef enum { BM_EVENTS_AUTO = 0, BM_EVENTS_CELLS = 1, BM_EVENTS_LANES = 2 } bm_event_mode;
 /* noise sources that are switched on; a source that is off ignores its parameters */
 enum { BM_NOISE_GAUSS = 1, BM_NOISE_POISSON = 2, BM_NOISE_DICH = 4 };
@@ -128,7 +130,8 @@ typedef struct {
                             for BM_F32 and the paper-literal scheme. */
   int32_t adapt_levels; /* BM_SCHEME_ADAPTIVE: how often dt may be halved, 0..20 */
   double adapt_tol;    /* BM_SCHEME_ADAPTIVE: tolerance on |chi| (in units of x), >= 0; +inf = never refine */
-  int32_t event_mode;  /* bm_event_mode; must be AUTO unless BM_F32, BM_OVERDAMPED, JUMP_ADAPTED (else BM_ERR_UNSUPPORTED) */
+  int32_t event_mode;  /* bm_event_mode; must be AUTO unless BM_F32, BM_OVERDAMPED, JUMP_ADAPTED with a jump source in
+                          `noise` (else BM_ERR_UNSUPPORTED) */
   int32_t rsv;         /* 0 */
 } bm_config;
 

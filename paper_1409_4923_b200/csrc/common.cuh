@@ -74,14 +74,17 @@ constexpr int EV_FIELDS_P = 4, EV_FIELDS_D = 3;  // (cell, off, amplitude, norma
 // lclk: the per-lane-clock form also keeps the normals of one Gaussian call (NB angle parts, NB/2 radii)
 __host__ __device__ constexpr int f32_smem_words_per_thread(int noise, int gauss, int lclk = 0) {
   const int rings = ((noise & BM_NOISE_POISSON) ? EVQ * EV_FIELDS_P : 0) + ((noise & BM_NOISE_DICH) ? EVQ * EV_FIELDS_D : 0) + 4;
-  // LANES form: one record per thread, with the normals of one Gaussian call, padded to an odd number of words
-  return lclk ? ((rings + ((noise & BM_NOISE_GAUSS) ? (gauss == BM_GAUSS_W32 ? 6 : 12) : 0)) | 1) : rings;
+  // LANES form: one record per thread, with the normals of two Gaussian calls, padded to an odd number of words
+  return lclk ? ((rings + ((noise & BM_NOISE_GAUSS) ? (gauss == BM_GAUSS_W32 ? 16 : 32) : 0)) | 1) : rings;
 }
 
 // Event mode of a parameter point (fp32 over-damped jump-adapted kernels; sim_f32.cuh, "per-lane clocks"): expected
 // kicks + flips per path and grid cell above LCLK_EVENTS_PER_CELL.  A function of the point's parameters and step
 // length only (in double), evaluated alike by both forms of the kernel, so every block is taken by exactly one.
-constexpr double LCLK_EVENTS_PER_CELL = 0.02;
+#ifndef BM_LCLK_EVENTS_PER_CELL
+#define BM_LCLK_EVENTS_PER_CELL 0.02
+#endif
+constexpr double LCLK_EVENTS_PER_CELL = BM_LCLK_EVENTS_PER_CELL;
 __device__ __forceinline__ bool lane_clock_point(const SimArgs &a, const bm_params &bp, double dt, int noise) {
   if (a.event_mode != BM_EVENTS_AUTO) return a.event_mode == BM_EVENTS_LANES;
   double rate = 0.0;

@@ -327,7 +327,7 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
   // CELLS form: field-major arrays [slot][field][thread] (conflict-free whatever slot each lane is at; the strides are
   // run-time values).  LANES form: one record of REC words per thread, [ring P][ring D][cold][normals], REC odd: every
   // offset inside the record is an immediate, the few lanes that pop an event in a pass rarely share a bank.
-  constexpr int RECW = EVQ * NFP + EVQ * NFD + 4 + (HAS_G ? NB + NP : 0), REC = RECW | 1;
+  constexpr int RECW = EVQ * NFP + EVQ * NFD + 4 + (HAS_G ? 4 * NB : 0), REC = RECW | 1;
   const int FS = LCLK ? 1 : T;                              // stride between the fields of one slot
   const int SSP = LCLK ? NFP : NFP * T, SSD = LCLK ? NFD : NFD * T;  // stride between ring slots
   uint32_t *const ringP = LCLK ? smem_words + tid * REC : smem_words + tid;
@@ -337,7 +337,7 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
   // events drawn so far.  The index of a stream's next event = events drawn - events queued - 1 = events applied, so
   // no counter has to follow the events themselves.
   uint32_t *const cold = LCLK ? ringD + EVQ * NFD : ringD + EVQ * NFD * T;  // [4]: snap_x, snap_w, drawnP, drawnD
-  uint32_t *const nrm = cold + 4;  // LANES: the block's normals, angle parts [NB] then radii [NP]
+  uint32_t *const nrm = cold + 4;  // LANES: the normals of two blocks, angle parts [2 NB] then radii [2 NB]
 
   const int point = blockIdx.x / a.blocks_per_point;
   const int chunk = blockIdx.x - point * a.blocks_per_point;
@@ -586,17 +586,22 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
   };
 
   // ---- a5-a8: a sub-step of length h from the lane's current state; noise = na * nb; dr0/dr1 = drive at its ends.
-  //      With h = dt, refold = false and (na, nb) = (gr, gc) this is fast_cell operation by operation, so a lane
+  //      With h = dt, refold = false and (na, nb) = (gr, gc) this is fast_cell(gr, gc, first) operation by operation, so a lane
   //      without an event gets the same result whichever way its warp takes through a cell. -----------------------
-  auto sub_step = [&](float h, float na, float nb, float dr0, float dr1, bool refold) {
+  //      `first`: the lane's first sub-step in a block of NB cells.  The position is re-folded there (a9); when that
+  //      sub-step is a whole cell the force is still evaluated at the position as it stands (the same angle), so the
+  //      cosine does not wait for the fold -- in every path through the kernel, clean block or not.
+  auto sub_step = [&](float h, float na, float nb, float dr0, float dr1, bool refold, bool first) {
     const float hh = 0.5f * h;
     float xf = x;
     int wf = wraps;
     fold_f32<POT>(xf, wf);
-    if (refold || POT != BM_POT_SINE2) { wraps = wf; x = xf; } else xf = x;
+    if (refold || POT != BM_POT_SINE2) { wraps = wf; x = xf; }  // base and argument folded
+    else if (first) wraps = wf;                                  // base folded, argument as it stands
+    else xf = x;
     if (!INERTIAL) {
       const float xs = HAS_G ? fmaf(na, nb, xf) : xf;
-      x = pc_overdamped_f32<POT, SINCOS>(xf, xs, __fmul_rn(h, cst), __fmul_rn(h, P.kk1), __fmul_rn(h, P.kk2), __fmul_rn(hh, cst),
+      x = pc_overdamped_f32<POT, SINCOS>(x, xs, __fmul_rn(h, cst), __fmul_rn(h, P.kk1), __fmul_rn(h, P.kk2), __fmul_rn(hh, cst),
                                          __fmul_rn(hh, P.kk1), __fmul_rn(hh, P.kk2));
     } else {
       const float vs = HAS_G ? fmaf(na, nb, v) : v;
@@ -612,7 +617,7 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
     const float h = fmaxf(te - tau, 0.f);
     float dr1 = 0.f;
     if (INERTIAL) dr1 = P.amp * cos_turns<SINCOS>(fmaf(te, P.w_turns, phf));
-    sub_step(h, HAS_G ? (isP ? gP : gD) : 0.f, HAS_G ? sqrt_approx(h * P.s2) : 0.f, dr_tau, dr1, true);  // Var ~ h (A9)
+    sub_step(h, HAS_G ? (isP ? gP : gD) : 0.f, HAS_G ? sqrt_approx(h * P.s2) : 0.f, dr_tau, dr1, true, false);  // Var ~ h (A9)
     dr_tau = dr1;
     tau = te;
     if (HAS_P && isP) {  // a8: kick
@@ -631,7 +636,7 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
   // ---- SLOW: a cell in which at least one lane of the warp has a kick or a flip.  Event lanes integrate up to each
   //      of their events on their own, then every lane finishes the cell with its own remaining length (a5): the
   //      whole cell, with the fast cell's arithmetic, for a lane without events. ----------------------------------
-  auto finish_cell = [&](float gr, float gc, float tau, float dr_tau) {
+  auto finish_cell = [&](float gr, float gc, float tau, float dr_tau, bool first) {
     const bool whole = tau == 0.f;
     const float h = dt - tau;
     float na = gr, nb = gc;
@@ -641,15 +646,15 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
       ph += dph;
       drive1 = P.amp * cos_turns<SINCOS>(__uint_as_float((uint32_t)(ph >> 41) | 0x3F800000u));
     }
-    sub_step(h, na, nb, dr_tau, drive1, !whole);
+    sub_step(h, na, nb, dr_tau, drive1, !whole, first);
     drive0 = drive1;
   };
-  auto slow_cell = [&](int c, float gr, float gc) {
+  auto slow_cell = [&](int c, float gr, float gc, bool first) {
     float tau = 0.f;         // the lane's offset inside cell c
     float dr_tau = drive0;   // drive at that time
     const float phf = INERTIAL ? __uint_as_float((uint32_t)(ph >> 41) | 0x3F800000u) : 0.f;  // 1 + frac(omega c dt / 2 pi)
     while ((HAS_P && nP == c) || (HAS_D && nD == c)) do_event(tau, dr_tau, phf);
-    finish_cell(gr, gc, tau, dr_tau);
+    finish_cell(gr, gc, tau, dr_tau, first);
   };
 
   // Events of this lane in cells [n, n+32) as a bit mask (bit = cell - n; shl.b32 clamps a shift >= 32 to zero, so
@@ -671,7 +676,7 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
   constexpr bool UNROLLED = BM_F32_UNROLLED(INERTIAL);  // covered non-clean blocks: unrolled pair slots or a rolled slot loop
   uint4 w = make_uint4(0u, 0u, 0u, 0u);
   Pair cur = Pair{0.f, 0.f, 0.f};
-  if (HAS_G) {
+  if (HAS_G && !LCLK) {
     w = philox_call(K, g, STREAM_GAUSS, (uint32_t)(n_begin / NB));
     cur = pair_of<GW>(w, 0, P.cn);
   }
@@ -705,7 +710,152 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
     return GW == BM_GAUSS_W16P ? pair_w16p(ww, P.cn) : pair_w16(ww, P.cn);
   };
 
+  // ---- LANES form: per-lane clocks in a sliding window ------------------------------------------------------------
+  // Every lane walks through the run on its own: one sub-step per pass, from its (cell c, offset tau) to its next event
+  // in that cell or to the cell's end.  The warp only agrees on a WINDOW: lo = the block of NB cells its slowest lane
+  // is in, G = the cell up to which the normals (two blocks in shared memory, at a per-lane index) and the events are
+  // known; a lane that has reached G waits.  A lane that falls behind by an event is caught up with while the others
+  // wait at most for one block, so the number of passes per cell tends to 1 + (events per cell), where blocks taken in
+  // lock-step cost 1 + (the largest number of events of any lane in the block) / NB.  Per lane the operations are those
+  // of the CELLS form: a cell crossed without an event is fast_cell, a sub-step that ends on an event do_event's, the
+  // rest of a cell after its last event finish_cell's: the results agree bit for bit.  Blocks that hold t_i or the end
+  // of the run, and blocks in which a lane has more events than its ring holds, are taken by all lanes together, cell
+  // by cell (the CAREFUL path of the CELLS form).
+  if (LCLK) {
+    constexpr int WC = 2 * NB;  // cells in the window; nrm: angle parts [WC] at c mod WC, then the radius of each cell [WC]
+    int c = n_begin;            // the lane's cell
+    float tau = 0.f;            // and its offset inside it
+    int lo = n_begin, G = n_begin, tried = -1;
+    for (;;) {  // uniform over the warp
+      if (G - lo < WC && G < n_end && tried != lo) {
+        bool ok = !(((unsigned)(n_discard - G) < (unsigned)NB) || (G + NB > n_end));
+        if (ok && __any_sync(FULL, cov < G + NB)) {
+          refill_episode(G + NB);
+          ok = !__any_sync(FULL, cov < G + NB);  // else: a ring is full; try again when the slowest lane has moved on
+        }
+        if (ok) {
+          if (HAS_G) {
+            const uint4 wg = philox_call(K, g, STREAM_GAUSS, (uint32_t)(G / NB));
+            uint32_t *const dst = nrm + (G & (WC - 1));
+#pragma unroll
+            for (int i = 0; i < NP; ++i) {
+              const Pair q = pair_of<GW>(wg, i, P.cn);
+              dst[2 * i] = __float_as_uint(q.c);
+              dst[2 * i + 1] = __float_as_uint(q.s);
+              dst[WC + 2 * i] = dst[WC + 2 * i + 1] = __float_as_uint(q.r);
+            }
+          }
+          G += NB;
+          continue;
+        }
+        tried = lo;
+        if (lo == G) {
+          // every lane stands at the start of block G: cell by cell, all lanes together
+          uint4 wg = make_uint4(0u, 0u, 0u, 0u);
+          if (HAS_G) wg = philox_call(K, g, STREAM_GAUSS, (uint32_t)(G / NB));
+#pragma unroll 1
+          for (int j = 0; j < NB; ++j) {
+            const int cc = G + j;
+            if (cc >= n_end) break;
+            if (cc == n_discard) {  // a10: snapshot at t_i
+              fold_f32<POT>(x, wraps);
+              cold[0 * FS] = __float_as_uint(x);
+              cold[1 * FS] = (uint32_t)wraps;
+            }
+            Pair q = Pair{0.f, 0.f, 0.f};
+            if (HAS_G) {
+              const int i = j >> 1;
+              if (GW == BM_GAUSS_W32) {
+                q = pair_w32(i ? wg.z : wg.x, i ? wg.w : wg.y, P.cn);
+              } else {
+                const uint32_t ww = i == 0 ? wg.x : i == 1 ? wg.y : i == 2 ? wg.z : wg.w;
+                q = GW == BM_GAUSS_W16P ? pair_w16p(ww, P.cn) : pair_w16(ww, P.cn);
+              }
+            }
+            float tj = 0.f, dr_tau = 0.f;
+            for (;;) {
+              if (__any_sync(FULL, cov <= cc)) refill_episode(cc + 1);
+              const bool mine = (HAS_P && nP == cc) || (HAS_D && nD == cc);
+              if (!__any_sync(FULL, mine)) break;
+              if (mine) do_event(tj, dr_tau, 0.f);
+            }
+            finish_cell(q.r, (j & 1) ? q.s : q.c, tj, dr_tau, j == 0);
+          }
+          G += NB;
+          lo = G;
+          c = G;
+          tau = 0.f;
+          tried = -1;
+          continue;
+        }
+      }
+      if (lo >= n_end) break;
+      // passes, until the slowest lane has left block lo (then the window may move on).  lo < G here, so some lane is
+      // below G in every pass.
+      const int lo_end = lo + NB;
+      do {
+      if (c < G) {
+        const bool evP = HAS_P && nP == c, evD = HAS_D && nD == c;
+        const bool ev = evP || evD;
+        const bool isP = evP && (!evD || fP <= fD);  // a tie applies the kick first (R5), as do_event
+        const float te = ev ? (isP ? fP : fD) : dt;
+        const bool whole = !ev && tau == 0.f;
+        const bool first = (c & (NB - 1)) == 0;  // (only looked at when `whole`)
+        const float h = fmaxf(te - tau, 0.f);
+        float na = 0.f, nb = 0.f;
+        if (HAS_G) {
+          const uint32_t *const q = nrm + (c & (WC - 1));
+          const float gc = __uint_as_float(q[0]), gr = __uint_as_float(q[WC]);
+          const float sq = sqrt_approx(h * (ev ? P.s2 : inv_dt));
+          na = ev ? (isP ? gP : gD) : (whole ? gr : gr * gc);
+          nb = whole ? gc : sq;
+        }
+        {  // sub_step(h, na, nb, ., ., !whole, first), the choice of the fold as a select on the rounding constant
+          float xf = x, xa = x;
+          if (POT != BM_POT_QUAD) {
+            float t = fmaf(x, Units<POT>::INV_PERIOD_TH, MAGIC_F);
+            if (POT == BM_POT_SINE2 && whole && !first) t = MAGIC_F;  // no re-fold: zero periods taken off, exactly
+            xf = fmaf(t - MAGIC_F, -Units<POT>::PERIOD_TH, x);
+            wraps += __float_as_int(t) - MAGIC_BITS;
+            xa = (POT == BM_POT_SINE2 && whole) ? x : xf;
+          }
+          const float hh = 0.5f * h;
+          const float xs = HAS_G ? fmaf(na, nb, xf) : xf;
+          x = pc_overdamped_f32<POT, SINCOS>(xa, xs, __fmul_rn(h, cst), __fmul_rn(h, P.kk1), __fmul_rn(h, P.kk2), __fmul_rn(hh, cst),
+                                             __fmul_rn(hh, P.kk1), __fmul_rn(hh, P.kk2));
+        }
+        tau = 0.f;
+        c += 1;
+        if (ev) {  // the lane stays in its cell, at the time of the event
+          tau = te;
+          c -= 1;
+          if (HAS_P && isP) {  // a8: kick
+            x = __fadd_rn(x, z);
+            const int s = qP & 15;
+            nP = (int)ringP[s * NFP + 0];
+            fP = __uint_as_float(ringP[s * NFP + 1]);
+            z = __uint_as_float(ringP[s * NFP + 2]);
+            if (HAS_G) gP = __uint_as_float(ringP[s * NFP + 3]);
+            qP = (qP - 15) & ~EVQ;  // one event less queued, read slot + 1 modulo EVQ
+          }
+          if (HAS_D && !isP) {  // a8: flip
+            d ^= 1;
+            cst = P.base + (d ? P.Gb : P.Ga);
+            const int s = qD & 15;
+            nD = (int)ringD[s * NFD + 0];
+            fD = __uint_as_float(ringD[s * NFD + 1]);
+            if (HAS_G) gD = __uint_as_float(ringD[s * NFD + 2]);
+            qD = (qD - 15) & ~EVQ;
+          }
+        }
+      }
+      } while (!__all_sync(FULL, c >= lo_end));
+      lo = lo_end;
+    }
+  }
+
   uint32_t blk = (uint32_t)(n_begin / NB);
+  if (!LCLK)
   for (int n = n_begin; n < n_end; n += NB) {
     blk++;
     const bool special = ((unsigned)(n_discard - n) < (unsigned)NB) || (n + NB > n_end);
@@ -731,94 +881,13 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
         careful = __any_sync(FULL, cov < n + NB);  // a lane with more than EVQ events in this block
       }
       unsigned ctl = 0;
-      if (HAS_EV && !LCLK) ctl = __reduce_or_sync(FULL, ev_bits(n)) & 0xFFu;
+      if (HAS_EV) ctl = __reduce_or_sync(FULL, ev_bits(n)) & 0xFFu;
       if (special) {
         if ((unsigned)(n_discard - n) < (unsigned)NB) ctl |= 0x100u << (n_discard - n);
         if (n + NB > n_end) ctl |= (0xFF00u << (n_end - n)) & 0xFF00u;
       }
-      fold_f32<POT>(x, wraps);
-      if (LCLK && !careful && !special) {
-        // PER-LANE CLOCKS (covered block): every lane walks through the block on its own -- one sub-step per pass,
-        // from its (cell j, offset tau) to its next event in that cell or to the cell's end -- and the warp leaves
-        // the block when its slowest lane has.  Per lane the operations are those of the CELLS form: a cell the lane
-        // crosses without an event of its own is fast_cell, a sub-step that ends on an event is do_event's, the rest
-        // of a cell after its last event is finish_cell's.  The block's normals are needed at a per-lane index, so
-        // they go through shared memory (angle parts [NB], radii [NP]; each thread reads back its own words only).
-        if (HAS_G) {
-          philox_rounds<0, 10>(wn, K);
-          nrm[0] = __float_as_uint(cur.c);
-          nrm[1] = __float_as_uint(cur.s);
-          nrm[NB] = __float_as_uint(cur.r);
-#pragma unroll
-          for (int i = 1; i < NP; ++i) {
-            const Pair q = pair_of<GW>(w, i, P.cn);
-            nrm[2 * i] = __float_as_uint(q.c);
-            nrm[2 * i + 1] = __float_as_uint(q.s);
-            nrm[NB + i] = __float_as_uint(q.r);
-          }
-          cur = pair_of<GW>(wn, 0, P.cn);
-        }
-        int c = n;  // the lane's cell
-        float tau = 0.f;
-        for (;;) {
-          const bool act = c < n + NB;
-          if (!__any_sync(FULL, act)) break;
-          if (act) {
-            const bool evP = HAS_P && nP == c, evD = HAS_D && nD == c;
-            const bool ev = evP || evD;
-            const bool isP = evP && (!evD || fP <= fD);  // a tie applies the kick first (R5), as do_event
-            const float te = ev ? (isP ? fP : fD) : dt;
-            const bool whole = !ev && tau == 0.f;
-            const float h = fmaxf(te - tau, 0.f);
-            float na = 0.f, nb = 0.f;
-            if (HAS_G) {
-              const int j = c - n;
-              const float gc = __uint_as_float(nrm[j]), gr = __uint_as_float(nrm[NB + (j >> 1)]);
-              const float sq = sqrt_approx(h * (ev ? P.s2 : inv_dt));
-              na = ev ? (isP ? gP : gD) : (whole ? gr : gr * gc);
-              nb = whole ? gc : sq;
-            }
-            // sub_step(h, na, nb, ., ., !whole) with the re-fold as a select on the rounding constant
-            {
-              float xf = x;
-              if (POT != BM_POT_QUAD) {
-                float t = fmaf(x, Units<POT>::INV_PERIOD_TH, MAGIC_F);
-                if (whole && POT == BM_POT_SINE2) t = MAGIC_F;  // no re-fold: zero periods taken off, exactly
-                xf = fmaf(t - MAGIC_F, -Units<POT>::PERIOD_TH, x);
-                wraps += __float_as_int(t) - MAGIC_BITS;
-              }
-              const float hh = 0.5f * h;
-              const float xs = HAS_G ? fmaf(na, nb, xf) : xf;
-              x = pc_overdamped_f32<POT, SINCOS>(xf, xs, __fmul_rn(h, cst), __fmul_rn(h, P.kk1), __fmul_rn(h, P.kk2), __fmul_rn(hh, cst),
-                                                 __fmul_rn(hh, P.kk1), __fmul_rn(hh, P.kk2));
-            }
-            tau = ev ? te : 0.f;
-            c += ev ? 0 : 1;
-            if (HAS_P && isP) {  // a8: kick
-              x = __fadd_rn(x, z);
-              const int s = qP & 15;
-              nP = (int)ringP[s * NFP + 0];
-              fP = __uint_as_float(ringP[s * NFP + 1]);
-              z = __uint_as_float(ringP[s * NFP + 2]);
-              if (HAS_G) gP = __uint_as_float(ringP[s * NFP + 3]);
-              qP = (qP - 15) & ~EVQ;  // one event less queued, read slot + 1 modulo EVQ
-            }
-            if (HAS_D && ev && !isP) {  // a8: flip
-              d ^= 1;
-              cst = P.base + (d ? P.Gb : P.Ga);
-              k0f = __fmul_rn(dt, cst);
-              k0h = __fmul_rn(hh_full, cst);
-              const int s = qD & 15;
-              nD = (int)ringD[s * NFD + 0];
-              fD = __uint_as_float(ringD[s * NFD + 1]);
-              if (HAS_G) gD = __uint_as_float(ringD[s * NFD + 2]);
-              qD = (qD - 15) & ~EVQ;
-            }
-          }
-        }
-      } else if (LCLK || careful) {
-        // CAREFUL (some lane has more events in this block than its ring holds; in the per-lane-clock form also the
-        // two blocks that hold t_i and the end of the run): every cell is taken as a slow cell,
+      if (careful) {
+        // CAREFUL (some lane has more events in this block than its ring holds): every cell is taken as a slow cell,
         // in turns of one event per lane with a refill before each turn, so that a lane's next event is always
         // known before it is needed.  Same arithmetic per lane as the covered path.
         if (HAS_G) philox_rounds<0, 10>(wn, K);
@@ -838,7 +907,7 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
               if (!__any_sync(FULL, mine)) break;
               if (mine) do_event(tau, dr_tau, phf);
             }
-            finish_cell(cur.r, jj ? cur.s : cur.c, tau, dr_tau);
+            finish_cell(cur.r, jj ? cur.s : cur.c, tau, dr_tau, j == 0);
           }
           cur = nxt;
         }
@@ -853,7 +922,7 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
             nxt = (i + 1 < NP) ? pair_of<GW>(w, i + 1, P.cn) : pair_of<GW>(wn, 0, P.cn);
           }
           if (((ctl >> (2 * i)) & 0x303u) == 0u) {
-            fast_cell(cur.r, cur.c, false);
+            fast_cell(cur.r, cur.c, i == 0);
             fast_cell(cur.r, cur.s, false);
           } else {
 #pragma unroll
@@ -862,10 +931,10 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
               if (!special_cell(n, j, ctl)) break;
               const float gc = jj ? cur.s : cur.c;
               if (HAS_EV && ((ctl >> j) & 1u)) {
-                slow_cell(n + j, cur.r, gc);
+                slow_cell(n + j, cur.r, gc, j == 0);
                 ctl |= __reduce_or_sync(FULL, ev_bits(n)) & 0xFFu;  // later events of the same lanes in this block
               } else {
-                fast_cell(cur.r, gc, false);
+                fast_cell(cur.r, gc, j == 0);
               }
             }
           }
@@ -879,7 +948,7 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
           Pair nxt = cur;
           if (HAS_G) nxt = pair_dyn(w, wn, i);
           if (((ctl >> (2 * i)) & 0x303u) == 0u) {
-            fast_cell(cur.r, cur.c, false);
+            fast_cell(cur.r, cur.c, i == 0);
             fast_cell(cur.r, cur.s, false);
           } else {
 #pragma unroll 1
@@ -888,10 +957,10 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
               if (!special_cell(n, j, ctl)) break;
               const float gc = jj ? cur.s : cur.c;
               if (HAS_EV && ((ctl >> j) & 1u)) {
-                slow_cell(n + j, cur.r, gc);
+                slow_cell(n + j, cur.r, gc, j == 0);
                 ctl |= __reduce_or_sync(FULL, ev_bits(n)) & 0xFFu;  // later events of the same lanes in this block
               } else {
-                fast_cell(cur.r, gc, false);
+                fast_cell(cur.r, gc, j == 0);
               }
             }
           }

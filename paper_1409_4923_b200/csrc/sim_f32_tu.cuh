@@ -10,14 +10,14 @@ namespace bm {
 template <int POT, int OCC>
 static KernelFn pick_noise_tu(int noise, int lclk) {
 #if BM_TU_MODEL == 0
-  if (lclk) {  // per-lane clocks: the sources with events only
+  if (lclk) {  // per-lane clocks: the sources with events only; one register class (the wider one measured faster)
     switch (noise & 7) {
-      case 2: return bm_paths_f32<BM_TU_MODEL, POT, 2, BM_TU_SINCOS, BM_TU_GAUSS, OCC, 1>;
-      case 3: return bm_paths_f32<BM_TU_MODEL, POT, 3, BM_TU_SINCOS, BM_TU_GAUSS, OCC, 1>;
-      case 4: return bm_paths_f32<BM_TU_MODEL, POT, 4, BM_TU_SINCOS, BM_TU_GAUSS, OCC, 1>;
-      case 5: return bm_paths_f32<BM_TU_MODEL, POT, 5, BM_TU_SINCOS, BM_TU_GAUSS, OCC, 1>;
-      case 6: return bm_paths_f32<BM_TU_MODEL, POT, 6, BM_TU_SINCOS, BM_TU_GAUSS, OCC, 1>;
-      case 7: return bm_paths_f32<BM_TU_MODEL, POT, 7, BM_TU_SINCOS, BM_TU_GAUSS, OCC, 1>;
+      case 2: return bm_paths_f32<BM_TU_MODEL, POT, 2, BM_TU_SINCOS, BM_TU_GAUSS, 0, 1>;
+      case 3: return bm_paths_f32<BM_TU_MODEL, POT, 3, BM_TU_SINCOS, BM_TU_GAUSS, 0, 1>;
+      case 4: return bm_paths_f32<BM_TU_MODEL, POT, 4, BM_TU_SINCOS, BM_TU_GAUSS, 0, 1>;
+      case 5: return bm_paths_f32<BM_TU_MODEL, POT, 5, BM_TU_SINCOS, BM_TU_GAUSS, 0, 1>;
+      case 6: return bm_paths_f32<BM_TU_MODEL, POT, 6, BM_TU_SINCOS, BM_TU_GAUSS, 0, 1>;
+      case 7: return bm_paths_f32<BM_TU_MODEL, POT, 7, BM_TU_SINCOS, BM_TU_GAUSS, 0, 1>;
       default: return nullptr;
     }
   }
