@@ -28,7 +28,7 @@
 extern "C" {
 #endif
 
-#define BM_VERSION 200 /* 0.2.0 */
+#define BM_VERSION 210 /* 0.2.1: bm_config.event_mode */
 
 #if defined(__GNUC__)
 #define BM_API __attribute__((visibility("default")))

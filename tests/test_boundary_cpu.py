@@ -33,16 +33,22 @@ def test_header_symbols_are_exported(B):
 
 
 def test_struct_layouts_match_header(B):
-    assert C.sizeof(B.BmConfig) == 72
+    assert C.sizeof(B.BmConfig) == 80
     assert len(W.FIELDS) == 16 and len(B.STATS_FIELDS) == 8
     hdr = open(os.path.join(ROOT, "include", "bm.h")).read()
     body = hdr[hdr.index("typedef struct {", hdr.index("One parameter point")):hdr.index("} bm_params;")]
     names = re.findall(r"\b([A-Za-z_]\w*)\s*[,;]", re.sub(r"/\*.*?\*/", "", body, flags=re.S))
     assert tuple(names) == W.FIELDS
+    cbody = hdr[hdr.rindex("typedef struct {", 0, hdr.index("} bm_config;")):hdr.index("} bm_config;")]
+    cnames = re.findall(r"\b(?:int32_t|int64_t|double)\s+([A-Za-z_]\w*)\s*;", re.sub(r"/\*.*?\*/", "", cbody, flags=re.S))
+    assert cnames == [f[0] for f in B.BmConfig._fields_], cnames
+    cfg = B.make_config()
+    cfg.event_mode = 3                       # not a bm_event_mode
+    assert B.bm_workspace_bytes(cfg, 1, 128) == 0
 
 
 def test_version_and_status_strings(B):
-    assert B.bm_version() == 200
+    assert B.bm_version() == 210
     assert B.status_string(B.BM_OK) == "BM_OK" and B.status_string(B.BM_ERR_CUDA) == "BM_ERR_CUDA"
     assert B.status_string(99) == "BM_ERR_UNKNOWN"
 
