@@ -67,19 +67,25 @@ struct PointF64 {
 // [-1/4, 1/4], cos 2 pi x = (-1)^k cos 2 pi r, and cos 2 pi r is a degree-12 polynomial in r^2 (interpolant at the
 // Chebyshev nodes of [0, 1/16]; approximation error 9.5e-17, evaluated in two interleaved Horner chains; absolute
 // error of the result below 3e-16, where the oracle's cos(2 pi xi) itself carries 7e-16 from rounding 2 pi xi).
+__constant__ double COS2PI_E[7] = {2.253668089082175e-05, 0.0037798236737849045, 0.28200596842351006, 7.903536371318447,
+                                    60.24464137187666, 64.9393940226683, 1.0};
+__constant__ double COS2PI_O[6] = {-0.00032289025049633054, -0.03638284043309509, -1.7143907110876637, -26.4262567833744,
+                                    -85.45681720669373, -19.739208802178716};
 __device__ __forceinline__ double cos2pi_f64(double x) {
   const double MAGIC = 6755399441055744.0;  // 1.5 * 2^52: (y + MAGIC) has ulp 1
   const double t = fma(x, 2.0, MAGIC);
   const double k = t - MAGIC;
   const double r = fma(k, -0.5, x);
   const double u = r * r, w = u * u;
-  double e = 2.253668089082175e-05, o = -0.00032289025049633054;
-  e = fma(e, w, 0.0037798236737849045);   o = fma(o, w, -0.03638284043309509);
-  e = fma(e, w, 0.28200596842351006);     o = fma(o, w, -1.7143907110876637);
-  e = fma(e, w, 7.903536371318447);       o = fma(o, w, -26.4262567833744);
-  e = fma(e, w, 60.24464137187666);       o = fma(o, w, -85.45681720669373);
-  e = fma(e, w, 64.9393940226683);        o = fma(o, w, -19.739208802178716);
-  e = fma(e, w, 1.0);
+  // the coefficients come from constant memory: a DFMA takes c[bank][offset] as an operand, where an immediate costs
+  // two UMOV issue slots per coefficient and evaluation
+  double e = COS2PI_E[0], o = COS2PI_O[0];
+  e = fma(e, w, COS2PI_E[1]);   o = fma(o, w, COS2PI_O[1]);
+  e = fma(e, w, COS2PI_E[2]);   o = fma(o, w, COS2PI_O[2]);
+  e = fma(e, w, COS2PI_E[3]);   o = fma(o, w, COS2PI_O[3]);
+  e = fma(e, w, COS2PI_E[4]);   o = fma(o, w, COS2PI_O[4]);
+  e = fma(e, w, COS2PI_E[5]);   o = fma(o, w, COS2PI_O[5]);
+  e = fma(e, w, COS2PI_E[6]);
   const double c = fma(o, u, e);
   // (-1)^k: the parity of k is the lowest mantissa bit of t
   const int hi = __double2hiint(c) ^ (__double2loint(t) << 31);
@@ -99,6 +105,18 @@ __device__ __forceinline__ double minus_dV_f64(const PointF64 &P, double x) {
   } else {
     return -P.A1 * x;
   }
+}
+
+// a(x) = -V'(x) + cst for the path kernels.  SINE2: -V' = -2 pi A1 c - 4 pi A2 (2 c^2 - 1), c = cos 2 pi x, summed in
+// Horner form, c (k1 + k2 c) + (cst + 4 pi A2): two DFMA behind the cosine instead of five FP64 operations (the sum is
+// the oracle's up to the order of its roundings; per-path parity is 1e-8).  k = (k1, k2, 4 pi A2).
+template <int POT>
+__device__ __forceinline__ double drift_f64(const PointF64 &P, const double (&k)[3], double x, double cst) {
+  if (POT == BM_POT_SINE2) {
+    const double c = cos2pi_f64(x);
+    return fma(c, fma(k[1], c, k[0]), cst + k[2]);
+  }
+  return minus_dV_f64<POT>(P, x) + cst;
 }
 
 struct StateF64 {
@@ -153,6 +171,7 @@ __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimA
   const bool onD = HAS_D && P.mu_a > 0.0;
   const long long n_end = CHUNKED ? a.step_end : a.n_steps;
   const double amp_dt = sqrt(2.0 * P.D * dt);  // noise amplitude of an unsplit grid step (the same expression as below)
+  const double kf[3] = {-2.0 * M_PI * P.A1, -8.0 * M_PI * P.A2, 4.0 * M_PI * P.A2};  // drift_f64
 
   bool valid[N], tracing[N];
   unsigned long long g[N], m[N];
@@ -271,15 +290,15 @@ __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimA
       // Alg. 1
       double F1[N], xb[N], F2[N];
 #pragma unroll
-      for (int q = 0; q < N; ++q) F1[q] = minus_dV_f64<POT>(P, s[q].xi) + cst[q];
+      for (int q = 0; q < N; ++q) F1[q] = drift_f64<POT>(P, kf, s[q].xi, cst[q]);
 #pragma unroll
       for (int q = 0; q < N; ++q) xb[q] = s[q].xi + F1[q] * h[q] + dxi[q];
 #pragma unroll
-      for (int q = 0; q < N; ++q) F2[q] = minus_dV_f64<POT>(P, xb[q]) + cst[q];
+      for (int q = 0; q < N; ++q) F2[q] = drift_f64<POT>(P, kf, xb[q], cst[q]);
 #pragma unroll
       for (int q = 0; q < N; ++q) xb[q] = s[q].xi + 0.5 * (F1[q] + F2[q]) * h[q] + dxi[q];
 #pragma unroll
-      for (int q = 0; q < N; ++q) F2[q] = minus_dV_f64<POT>(P, xb[q]) + cst[q];
+      for (int q = 0; q < N; ++q) F2[q] = drift_f64<POT>(P, kf, xb[q], cst[q]);
 #pragma unroll
       for (int q = 0; q < N; ++q) { xn[q] = s[q].xi + 0.5 * (F1[q] + F2[q]) * h[q] + dxi[q]; vn[q] = s[q].v; }
     } else {
@@ -288,20 +307,20 @@ __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimA
 #pragma unroll
       for (int q = 0; q < N; ++q) {
         const double t = __dadd_rn(__dmul_rn((double)n[q], dt), __dsub_rn(dt, rem[q]));
-        A1v[q] = -P.gamma * s[q].v + minus_dV_f64<POT>(P, s[q].xi) + P.amp * cos(P.omega * t) + cst[q];
+        A1v[q] = -P.gamma * s[q].v + drift_f64<POT>(P, kf, s[q].xi, cst[q]) + P.amp * cos(P.omega * t);
         drive[q] = P.amp * cos(P.omega * __dadd_rn(t, h[q]));
       }
 #pragma unroll
       for (int q = 0; q < N; ++q) { xb[q] = s[q].xi + s[q].v * h[q]; vb[q] = s[q].v + A1v[q] * h[q] + dxi[q]; }
 #pragma unroll
-      for (int q = 0; q < N; ++q) { A2x[q] = vb[q]; A2v[q] = -P.gamma * vb[q] + minus_dV_f64<POT>(P, xb[q]) + drive[q] + cst[q]; }
+      for (int q = 0; q < N; ++q) { A2x[q] = vb[q]; A2v[q] = -P.gamma * vb[q] + drift_f64<POT>(P, kf, xb[q], cst[q]) + drive[q]; }
 #pragma unroll
       for (int q = 0; q < N; ++q) {
         xb[q] = s[q].xi + 0.5 * (s[q].v + A2x[q]) * h[q];
         vb[q] = s[q].v + 0.5 * (A1v[q] + A2v[q]) * h[q] + dxi[q];
       }
 #pragma unroll
-      for (int q = 0; q < N; ++q) { A2x[q] = vb[q]; A2v[q] = -P.gamma * vb[q] + minus_dV_f64<POT>(P, xb[q]) + drive[q] + cst[q]; }
+      for (int q = 0; q < N; ++q) { A2x[q] = vb[q]; A2v[q] = -P.gamma * vb[q] + drift_f64<POT>(P, kf, xb[q], cst[q]) + drive[q]; }
 #pragma unroll
       for (int q = 0; q < N; ++q) {
         xn[q] = s[q].xi + 0.5 * (s[q].v + A2x[q]) * h[q];
