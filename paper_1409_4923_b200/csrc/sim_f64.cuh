@@ -119,6 +119,10 @@ __device__ __forceinline__ double drift_f64(const PointF64 &P, const double (&k)
   return minus_dV_f64<POT>(P, x) + cst;
 }
 
+// noise amplitude of a sub-step cut short by an event (kept out of line: inlined, the compiler evaluates the square
+// root in every iteration and selects afterwards -- ten FP64 operations per sub-step for the one in 500 that needs them)
+static __device__ __noinline__ double amp_of_substep_f64(double D, double h) { return sqrt(2.0 * D * h); }
+
 struct StateF64 {
   double xi;
   long long wraps;
@@ -282,7 +286,9 @@ __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimA
       }
       const double Gd = onD ? (d[q] ? P.Fb : -P.Fa) : 0.0;
       cst[q] = P.c0 + Gd;
-      dxi[q] = HAS_G ? ((h[q] == dt) ? amp_dt : sqrt(2.0 * P.D * h[q])) * gn[q] : 0.0;
+      double amp = amp_dt;
+      if (HAS_G && h[q] != dt) amp = amp_of_substep_f64(P.D, h[q]);
+      dxi[q] = HAS_G ? amp * gn[q] : 0.0;
     }
     // a6 / a7: the predictor-corrector sub-step, stage by stage over the thread's paths (independent chains)
     double xn[N], vn[N];
