@@ -3,6 +3,8 @@
 // It follows DESIGN.md readings R3-R9 operation by operation, so that per-path results track the fp64
 // oracle to ~1e-13 (only libm-vs-CUDA transcendental rounding and FMA contraction differ).
 #pragma once
+#include <type_traits>
+
 #include "common.cuh"
 
 namespace bm {
@@ -243,11 +245,15 @@ __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimA
   // of every active lane, so instead each lane keeps TWO blocks and the whole warp draws the next one every fourth
   // iteration: by then the older block is used up whatever the lane's phase.  (A single launch starts all lanes at
   // m = 0; they stay in phase and one block is enough.)
-  for (unsigned long long it = 0;; ++it) {
+  // One iteration = one sub-step of every active path.  J >= 0 (a single launch): the sub-step takes normal J of the
+  // Philox block in flight -- the lanes of a warp stay in phase, so the time loop is unrolled by four and the index
+  // of the normal is static; J = 0 draws the block.  J < 0: the index follows the path's own m.
+  auto iteration = [&](auto JT, unsigned long long it) -> bool {
+    constexpr int J = decltype(JT)::value;
     bool act[N], any = false;
 #pragma unroll
     for (int q = 0; q < N; ++q) { act[q] = n[q] < n_end; any |= act[q]; }
-    if (!any) break;
+    if (!any) return false;
     // a5: sub-step length; a3/a4: the sub-step's Gaussian
     double h[N], gn[N], cst[N], dxi[N];
 #pragma unroll
@@ -258,12 +264,12 @@ __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimA
       gn[q] = 0.0;
       if (HAS_G && act[q]) {
         if (!CHUNKED) {
-          if ((m[q] & 3ull) == 0) {
+          if (J >= 0 ? J == 0 : (m[q] & 3ull) == 0) {
             const uint4 w = philox_call(a.keys, g[q], STREAM_GAUSS, (uint32_t)(m[q] >> 2));
             box_muller_f64(w.x, w.y, gq[q][0], gq[q][1]);
             box_muller_f64(w.z, w.w, gq[q][2], gq[q][3]);
           }
-          const int j = (int)(m[q] & 3ull);
+          const int j = J >= 0 ? J : (int)(m[q] & 3ull);
           gn[q] = (j == 0) ? gq[q][0] : (j == 1) ? gq[q][1] : (j == 2) ? gq[q][2] : gq[q][3];
         } else {
           if ((it & 3ull) == 0) {  // warp-uniform: the block after the one this iteration's normal comes from
@@ -288,7 +294,7 @@ __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimA
       cst[q] = P.c0 + Gd;
       double amp = amp_dt;
       if (HAS_G && h[q] != dt) amp = amp_of_substep_f64(P.D, h[q]);
-      dxi[q] = HAS_G ? amp * gn[q] : 0.0;
+      dxi[q] = HAS_G ? __dmul_rn(amp, gn[q]) : 0.0;  // (never contracted into the sums that use it: a path must not depend on which copy of the code runs it)
     }
     // a6 / a7: the predictor-corrector sub-step, stage by stage over the thread's paths (independent chains)
     double xn[N], vn[N];
@@ -372,6 +378,18 @@ __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimA
         }
         if (n[q] == a.n_discard) snap[q] = s[q];
       }
+    }
+    return true;
+  };
+  // unrolled: the over-damped kernel with one path per thread (measured: C1 89.5 -> 84.7 ms; the inertial kernel, with
+  // 117 registers and a longer body, loses 5 % to the larger code, C2 266 -> 280 ms)
+  if (CHUNKED || N > 1 || INERTIAL) {
+    for (unsigned long long it = 0; iteration(std::integral_constant<int, -1>(), it); ++it) {}
+  } else {
+    while (iteration(std::integral_constant<int, 0>(), 0ull)) {
+      iteration(std::integral_constant<int, 1>(), 0ull);
+      iteration(std::integral_constant<int, 2>(), 0ull);
+      iteration(std::integral_constant<int, 3>(), 0ull);
     }
   }
 
