@@ -1,0 +1,31 @@
+"""Prints the polynomial coefficients of the fp64 kernels' own elementary functions (sim_f64.cuh: cos2pi_f64, log_u_f64,
+sincospi_f64): interpolants at the Chebyshev nodes of the argument range, computed with mpmath at 60 digits and rounded
+to double.  Run by hand when a range or degree changes; the output is pasted into sim_f64.cuh.  Not part of the oracle."""
+import mpmath as mp
+
+mp.mp.dps = 60
+
+
+def cheb_fit(f, a, b, n):
+    xs = [(a + b) / 2 + (b - a) / 2 * mp.cos(mp.pi * (2 * k + 1) / (2 * n)) for k in range(n)]
+    A, y = mp.matrix(n, n), mp.matrix(n, 1)
+    for i, x in enumerate(xs):
+        for j in range(n):
+            A[i, j] = x ** j
+        y[i] = f(x)
+    c = mp.lu_solve(A, y)
+    return [c[i] for i in range(n)]
+
+
+def show(name, c):
+    print(f"{name}[{len(c)}] = {{" + ", ".join(repr(float(v)) for v in c) + "};   // c0 + c1 z + ...")
+
+
+sixteenth = mp.mpf(1) / 16
+show("SINPI_C", cheb_fit(lambda z: mp.sin(mp.pi * mp.sqrt(z)) / mp.sqrt(z), mp.mpf(0), sixteenth, 8))   # sin(pi r) / r, z = r^2
+show("COSPI_C", cheb_fit(lambda z: mp.cos(mp.pi * mp.sqrt(z)), mp.mpf(0), sixteenth, 8))                 # cos(pi r)
+smax = (mp.sqrt(2) - 1) / (mp.sqrt(2) + 1)                     # s = f / (2 + f), f = m - 1, m in [sqrt(1/2), sqrt(2))
+show("LOGP_C", cheb_fit(lambda z: (mp.log((1 + mp.sqrt(z)) / (1 - mp.sqrt(z))) / mp.sqrt(z) - 2) / z, mp.mpf(0), smax * smax * mp.mpf("1.0001"), 7))
+ln2 = mp.log(2)
+hi = mp.floor(ln2 * 2 ** 32) / 2 ** 32                           # 32 significant bits: k * LN2_HI is exact for |k| < 2^20
+print("LN2_HI =", repr(float(hi)), " LN2_LO =", repr(float(ln2 - hi)))

@@ -15,13 +15,101 @@ __device__ __forceinline__ double period_f64() { return POT == BM_POT_SINE2 ? 1.
 // u(w) = (w + 1/2) 2^-32  (R3)
 __device__ __forceinline__ double u01_f64(uint32_t w) { return ((double)w + 0.5) * (1.0 / 4294967296.0); }
 
+// ---- elementary functions of the Gaussian stream, written for the arguments they get here ------------------------
+// Branch-free (so that the time loop can interleave them with the predictor-corrector chain, see the kernel) and with
+// their coefficients in constant memory (a DFMA takes c[bank][offset] as an operand; the library routines load each
+// 64-bit coefficient with two UMOV).  Coefficients: csrc/make_poly_f64.py.  Each is within ~1 ulp of the correctly rounded
+// value on its range; tests/test_gpu_parity.py compares the resulting normals with the oracle's (libm) to 5e-15.
+__constant__ double SINPI_C[8] = {3.141592653589793, -5.16771278004997, 2.5501640398773415, -0.5992645293202978,
+                                  0.08214588658005621, -0.007370429884712669, 0.00046628272951211076, -2.1717401400090533e-05};
+__constant__ double COSPI_C[8] = {1.0, -4.934802200544679, 4.058712126416747, -1.3352627688519174, 0.23533063019088787,
+                                  -0.025806885652951306, 0.0019294657440800042, -0.00010356747255199479};
+__constant__ double LOGP_C[7] = {0.666666666666667, 0.39999999999899444, 0.2857142862600327, 0.22222211130259878,
+                                 0.18182889455674947, 0.15331710618210773, 0.14616585424888623};
+
+// u(w) of R3 without an integer conversion: 2^52 + w has w in its low mantissa bits
+__device__ __forceinline__ double u01_bits_f64(uint32_t w) {
+  const double t = __hiloint2double(0x43300000, (int)w) - 4503599627370496.0;  // = w, exactly
+  return fma(t, 1.0 / 4294967296.0, 1.0 / 8589934592.0);                        // (w + 1/2) 2^-32, exactly
+}
+
+// ln u for a normal u in (0, 1): u = 2^k m, m in [sqrt(1/2), sqrt(2)); with f = m - 1, s = f / (2 + f), z = s^2:
+// ln m = 2 atanh s = f - s (f - z P(z)).  The quotient by a reciprocal seed and two Newton steps, then one correction.
+__device__ __forceinline__ double log_u_f64(double u) {
+  int hi = __double2hiint(u);
+  hi += 0x3ff00000 - 0x3fe6a09e;  // mantissas above sqrt(2) carry into the exponent
+  const int k = (hi >> 20) - 0x3ff;
+  const double m = __hiloint2double((hi & 0x000fffff) + 0x3fe6a09e, __double2loint(u));
+  const double f = m - 1.0, y = 2.0 + f;
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(y));
+  double e = fma(-y, r, 1.0);
+  r = fma(r, e, r);
+  e = fma(-y, r, 1.0);
+  r = fma(r, e, r);
+  double sq = f * r;
+  sq = fma(fma(-y, sq, f), r, sq);  // s = f / y
+  const double z = sq * sq;
+  double p = LOGP_C[6];
+  p = fma(p, z, LOGP_C[5]);
+  p = fma(p, z, LOGP_C[4]);
+  p = fma(p, z, LOGP_C[3]);
+  p = fma(p, z, LOGP_C[2]);
+  p = fma(p, z, LOGP_C[1]);
+  p = fma(p, z, LOGP_C[0]);
+  const double lm = fma(-sq, fma(-z, p, f), f);  // f - s (f - z P)
+  const double dk = (double)k;
+  return fma(dk, 0.6931471803691238, fma(dk, 1.9082149292705877e-10, lm));  // k ln2 in two parts: the first product is exact
+}
+
+// sqrt x for a normal x > 0: reciprocal-root seed, two coupled Newton steps on (g, h) -> (sqrt x, 1 / (2 sqrt x)), one correction
+__device__ __forceinline__ double sqrt_pos_f64(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double g = x * y, h = 0.5 * y;
+  double r = fma(-g, h, 0.5);
+  g = fma(g, r, g);
+  h = fma(h, r, h);
+  r = fma(-g, h, 0.5);
+  g = fma(g, r, g);
+  h = fma(h, r, h);
+  return fma(fma(-g, g, x), h, g);
+}
+
+// (sin pi a, cos pi a) for 0 <= a <= 2: q = nearest integer to 2a, r = a - q/2 in [-1/4, 1/4] (exact), polynomials in
+// r^2 (two independent Horner chains), then the quadrant: swap for odd q, signs from q and q + 1.
+__device__ __forceinline__ void sincospi_f64(double a, double &sn, double &cs) {
+  const double MAGIC = 6755399441055744.0;  // 1.5 * 2^52
+  const double t = fma(a, 2.0, MAGIC);
+  const int q = __double2loint(t);
+  const double r = fma(t - MAGIC, -0.5, a);
+  const double z = r * r;
+  double ps = SINPI_C[7], pc = COSPI_C[7];
+  ps = fma(ps, z, SINPI_C[6]); pc = fma(pc, z, COSPI_C[6]);
+  ps = fma(ps, z, SINPI_C[5]); pc = fma(pc, z, COSPI_C[5]);
+  ps = fma(ps, z, SINPI_C[4]); pc = fma(pc, z, COSPI_C[4]);
+  ps = fma(ps, z, SINPI_C[3]); pc = fma(pc, z, COSPI_C[3]);
+  ps = fma(ps, z, SINPI_C[2]); pc = fma(pc, z, COSPI_C[2]);
+  ps = fma(ps, z, SINPI_C[1]); pc = fma(pc, z, COSPI_C[1]);
+  ps = fma(ps, z, SINPI_C[0]); pc = fma(pc, z, COSPI_C[0]);
+  ps *= r;
+  const bool odd = q & 1;
+  const double s0 = odd ? pc : ps, c0 = odd ? ps : pc;
+  // sin: q = 0, 1 -> +, 2, 3 -> -;   cos: q = 0 -> +, 1, 2 -> -, 3 -> + (q = 4 as q = 0)
+  sn = __hiloint2double(__double2hiint(s0) ^ ((q & 2) << 30), __double2loint(s0));
+  cs = __hiloint2double(__double2hiint(c0) ^ (((q + 1) & 2) << 30), __double2loint(c0));
+}
+
 // Box-Muller pair from two words (R3): r = sqrt(-2 ln u(wa)); (r cos 2 pi u(wb), r sin 2 pi u(wb))
+__device__ __forceinline__ double bm_radius_f64(uint32_t wa) { return sqrt_pos_f64(-2.0 * log_u_f64(u01_bits_f64(wa))); }
+__device__ __forceinline__ void bm_angle_f64(uint32_t wb, double r, double &g0, double &g1) {
+  double sn, cs;
+  sincospi_f64(2.0 * u01_bits_f64(wb), sn, cs);
+  g0 = r * cs;
+  g1 = r * sn;
+}
 __device__ __forceinline__ void box_muller_f64(uint32_t wa, uint32_t wb, double &g0, double &g1) {
-  const double r = sqrt(-2.0 * log(u01_f64(wa)));
-  double s, c;
-  sincospi(2.0 * u01_f64(wb), &s, &c);
-  g0 = r * c;
-  g1 = r * s;
+  bm_angle_f64(wb, bm_radius_f64(wa), g0, g1);
 }
 
 // the Gaussian call in progress at a checkpoint is recomputed, not stored (kept out of line: it runs once per launch)
@@ -248,6 +336,8 @@ __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimA
   // One iteration = one sub-step of every active path.  J >= 0 (a single launch): the sub-step takes normal J of the
   // Philox block in flight -- the lanes of a warp stay in phase, so the time loop is unrolled by four and the index
   // of the normal is static; J = 0 draws the block.  J < 0: the index follows the path's own m.
+  uint4 gw = make_uint4(0u, 0u, 0u, 0u);  // unrolled form: words, an intermediate and the normals of the block in production
+  double glog = 0.0, gnx[4] = {0.0, 0.0, 0.0, 0.0};
   auto iteration = [&](auto JT, unsigned long long it) -> bool {
     constexpr int J = decltype(JT)::value;
     bool act[N], any = false;
@@ -264,7 +354,7 @@ __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimA
       gn[q] = 0.0;
       if (HAS_G && act[q]) {
         if (!CHUNKED) {
-          if (J >= 0 ? J == 0 : (m[q] & 3ull) == 0) {
+          if (J < 0 && (m[q] & 3ull) == 0) {
             const uint4 w = philox_call(a.keys, g[q], STREAM_GAUSS, (uint32_t)(m[q] >> 2));
             box_muller_f64(w.x, w.y, gq[q][0], gq[q][1]);
             box_muller_f64(w.z, w.w, gq[q][2], gq[q][3]);
@@ -295,6 +385,21 @@ __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimA
       double amp = amp_dt;
       if (HAS_G && h[q] != dt) amp = amp_of_substep_f64(P.D, h[q]);
       dxi[q] = HAS_G ? __dmul_rn(amp, gn[q]) : 0.0;  // (never contracted into the sums that use it: a path must not depend on which copy of the code runs it)
+    }
+    // Unrolled form: a quarter of the NEXT block of normals is produced beside each sub-step -- branch-free code in the
+    // same basic block as the predictor-corrector chain, whose stalls (three cosines behind each other) it fills.
+    // J = 0: the Philox call and ln u_a; 1: radius and angle of pair a; 2: ln u_b and radius b; 3: angle of pair b.
+    if (J >= 0 && HAS_G) {
+      if (J == 0) {
+        gw = philox_call(a.keys, g[0], STREAM_GAUSS, (uint32_t)(m[0] >> 2) + 1u);
+        glog = log_u_f64(u01_bits_f64(gw.x));
+      } else if (J == 1) {
+        bm_angle_f64(gw.y, sqrt_pos_f64(-2.0 * glog), gnx[0], gnx[1]);
+      } else if (J == 2) {
+        glog = sqrt_pos_f64(-2.0 * log_u_f64(u01_bits_f64(gw.z)));
+      } else {
+        bm_angle_f64(gw.w, glog, gnx[2], gnx[3]);
+      }
     }
     // a6 / a7: the predictor-corrector sub-step, stage by stage over the thread's paths (independent chains)
     double xn[N], vn[N];
@@ -379,6 +484,10 @@ __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimA
         if (n[q] == a.n_discard) snap[q] = s[q];
       }
     }
+    if (J == 3 && HAS_G) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) gq[0][j] = gnx[j];
+    }
     return true;
   };
   // unrolled: the over-damped kernel with one path per thread (measured: C1 89.5 -> 84.7 ms; the inertial kernel, with
@@ -386,6 +495,11 @@ __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimA
   if (CHUNKED || N > 1 || INERTIAL) {
     for (unsigned long long it = 0; iteration(std::integral_constant<int, -1>(), it); ++it) {}
   } else {
+    if (HAS_G) {  // block 0 in place; from then on block b + 1 is produced while block b is used
+      const uint4 w = philox_call(a.keys, g[0], STREAM_GAUSS, 0u);
+      box_muller_f64(w.x, w.y, gq[0][0], gq[0][1]);
+      box_muller_f64(w.z, w.w, gq[0][2], gq[0][3]);
+    }
     while (iteration(std::integral_constant<int, 0>(), 0ull)) {
       iteration(std::integral_constant<int, 1>(), 0ull);
       iteration(std::integral_constant<int, 2>(), 0ull);
