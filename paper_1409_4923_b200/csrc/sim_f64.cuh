@@ -418,6 +418,13 @@ __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimA
       for (int q = 0; q < N; ++q) F2[q] = drift_f64<POT>(P, kf, xb[q], cst[q]);
 #pragma unroll
       for (int q = 0; q < N; ++q) { xn[q] = s[q].xi + 0.5 * (F1[q] + F2[q]) * h[q] + dxi[q]; vn[q] = s[q].v; }
+      // (an empty asm that takes the stage's results together with xn: the compiler would otherwise sink the stage
+      // below the branches of the event handling, out of the block it is meant to share with the chain)
+      if (J >= 0 && HAS_G) {
+        if (J == 0 || J == 2) asm volatile("" : "+d"(xn[0]), "+d"(glog));
+        if (J == 1) asm volatile("" : "+d"(xn[0]), "+d"(gnx[0]), "+d"(gnx[1]));
+        if (J == 3) asm volatile("" : "+d"(xn[0]), "+d"(gnx[2]), "+d"(gnx[3]));
+      }
     } else {
       // R7: two-component version, additive noise in v only, drive evaluated at t and t+h
       double A1v[N], xb[N], vb[N], drive[N], A2x[N], A2v[N];
@@ -490,8 +497,9 @@ __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimA
     }
     return true;
   };
-  // unrolled: the over-damped kernel with one path per thread (measured: C1 89.5 -> 84.7 ms; the inertial kernel, with
-  // 117 registers and a longer body, loses 5 % to the larger code, C2 266 -> 280 ms)
+  // unrolled: the over-damped kernel with one path per thread (measured: C1 89.5 -> 84.7 ms unrolled, -> 76.4 with the
+  // next block of normals produced beside the sub-steps; the inertial kernel, with 117 registers and a longer body, loses
+  // to the larger code: C2 266 -> 280 ms unrolled, 249.5 -> 253.8 ms unrolled and staged, 128 registers and spills)
   if (CHUNKED || N > 1 || INERTIAL) {
     for (unsigned long long it = 0; iteration(std::integral_constant<int, -1>(), it); ++it) {}
   } else {
