@@ -266,6 +266,7 @@ FP64_LANES_PER_SM = 64        # DFMA lanes per SM per clock (bm_pipe_probe: 63)
 def launches_per_call(B, w, prec_name):
     """Kernels one bm_simulate call launches: the path kernel and the grid pass of the reduction; the fp32 over-damped
     jump-adapted kernel with a jump source on is launched in both of its forms (CELLS, LANES) on the same grid."""
+    from paper_1409_4923_b200 import workloads as W
     two_forms = (prec_name == "f32" and w.model == W.OVERDAMPED and w.scheme == W.SCHEME_JUMP_ADAPTED
                  and (B.noise_mask(w.params) & 6) != 0)
     return 3 if two_forms else 2
