@@ -36,8 +36,9 @@ UNIT = "path-steps/s"
 XU_OPS_PER_SUBSTEP = {0: 5.0, 1: 6.0}
 XU_LANES_PER_SM = 16          # MUFU lanes per SM per clock (4 per SM sub-partition); confirmed by bm_pipe_probe
 # dram__bytes_read.sum + dram__bytes_write.sum of one path-kernel launch from the committed `ncu --set full` captures
-# (profiles/r1_f32_v5.md): parameters and per-block partials only, the path is register-resident.  Bytes per launch.
-NCU_DRAM_BYTES = {("C1", "f32"): 68864, ("C2", "f32"): 56064}
+# (profiles/r2_f32_v7.md; C4: its CELLS and LANES launch together): parameters and per-block partials only, the path is
+# register-resident.  Bytes per call.
+NCU_DRAM_BYTES = {("C1", "f32"): 67840, ("C2", "f32"): 54784, ("C3", "f32"): 87552, ("C4", "f32"): 4710400}
 
 
 def parse():
@@ -257,9 +258,9 @@ class Runner:
         return max(e0.elapsed_time(e1), 1e3 * (time.perf_counter() - t0))
 
 
-# FP64-pipe instructions per sub-step of the fp64 kernels as built (sm__inst_executed_pipe_fp64 of the committed
-# `ncu --set full` captures / warp sub-steps, profiles/r2_f64.md): the count the fp64 roofline fraction is formed with.
-FP64_OPS_PER_SUBSTEP = {0: 136.0, 1: 190.0}
+# FP64-pipe arithmetic instructions (DFMA, DMUL, DADD, DSETP) per sub-step of the fp64 kernels as built, from the executed
+# counts of the committed `ncu --set full` captures (profiles/r2_f64_v2.md): the count the fp64 roofline fraction is formed with.
+FP64_OPS_PER_SUBSTEP = {0: 113.5, 1: 168.3}
 FP64_LANES_PER_SM = 64        # DFMA lanes per SM per clock (bm_pipe_probe: 63)
 
 
@@ -288,7 +289,7 @@ def roofline_of(B, w, prec_name, stats, ms_per_step, clocks, info):
     else:
         per_path = FP64_OPS_PER_SUBSTEP[w.model] * substeps
         lanes, pipe = FP64_LANES_PER_SM, "fp64"
-        what = "FP64-pipe instructions of the kernel as built (profiles/r2_f64.md)"
+        what = "FP64-pipe instructions of the kernel as built (profiles/r2_f64_v2.md)"
     ops = per_path * w.n_points * w.n_paths
     peak = lanes * info["sm_count"] * sm_mhz * 1e6 / 1e9
     achieved = ops / (ms_per_step * 1e-3) / 1e9
