@@ -248,6 +248,13 @@ BM_API bm_status bm_philox_fill(uint64_t seed, uint64_t path0, int32_t n_paths, 
 BM_API bm_status bm_gauss_fill(int32_t prec, int32_t gauss, uint64_t seed, uint64_t path0, int32_t n_paths, uint64_t m0,
                         int32_t n_m, void *out, void *stream);
 
+/* The variate transform alone (a4; eq. 27, reading R3) on GIVEN words, for its edge cases (u next to 0 and
+ * to 1, angles on the quadrant boundaries), which the Philox stream only reaches by chance: out[2i], out[2i+1] = the
+ * Box-Muller pair of (words[2i], words[2i+1]) -- radius from the first word, angle from the second -- by the device code
+ * of the path kernels.  prec BM_F64: out is double*; BM_F32: float*, the W32 assignment.  words, out: device, 8- and
+ * 16-byte aligned.  Errors: BM_ERR_INVALID_ARG. */
+BM_API bm_status bm_box_muller_words(int32_t prec, const uint32_t *words, int32_t n_pairs, void *out, void *stream);
+
 /* Registers per thread, threads per block, resident blocks per SM, SM count and the Gaussian assignment selected
  * (bm_gauss, never AUTO; 0 for BM_F64), for the path kernel bm_simulate would launch for (cfg, n_points, n_paths)
  * (measurement aid; HOST outputs, each may be NULL). */

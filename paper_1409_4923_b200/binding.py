@@ -31,7 +31,7 @@ BM_STATE_SLOTS, BM_CHUNK_ALIGN = 16, 8
  BM_MOM_VAR_V0) = range(9)
 BM_MOM_STRIDE = 10
 EXPORTS = ("bm_workspace_bytes", "bm_simulate", "bm_simulate_dt", "bm_state_bytes", "bm_simulate_chunk", "bm_state_histogram",
-           "bm_state_moments", "bm_simulate_host", "bm_philox_fill", "bm_gauss_fill",
+           "bm_state_moments", "bm_simulate_host", "bm_philox_fill", "bm_gauss_fill", "bm_box_muller_words",
            "bm_kernel_info", "bm_pipe_probe", "bm_status_string", "bm_version")
 STATS_FIELDS = ("n", "mean_v", "var_v", "mean_xT", "var_xT", "mean_jumps", "mean_substeps", "rsv")
 
@@ -83,6 +83,8 @@ def lib():
         L.bm_philox_fill.restype = C.c_int
         L.bm_gauss_fill.argtypes = [i32, i32, u64, u64, i32, u64, i32, vp, vp]
         L.bm_gauss_fill.restype = C.c_int
+        L.bm_box_muller_words.argtypes = [i32, vp, i32, vp, vp]
+        L.bm_box_muller_words.restype = C.c_int
         ip = C.POINTER(C.c_int32)
         L.bm_kernel_info.argtypes = [cfgp, i32, i64, ip, ip, ip, ip, ip]
         L.bm_kernel_info.restype = C.c_int
@@ -272,6 +274,13 @@ def bm_kernel_info(cfg, n_points=1, n_paths=1 << 30):
         raise BmError(rc, "bm_kernel_info")
     return {"regs_per_thread": r.value, "launch_threads": b.value, "blocks_per_sm": o.value, "sm_count": s.value,
             "gauss": int(w.value)}
+
+
+def bm_box_muller_words(prec, words, n_pairs, out, stream=None):
+    """words: CUDA uint32/int32 tensor [n_pairs, 2]; out: float64 (BM_F64) or float32 (BM_F32) CUDA tensor [n_pairs, 2]."""
+    rc = lib().bm_box_muller_words(prec, C.c_void_p(words.data_ptr()), n_pairs, C.c_void_p(out.data_ptr()), _stream_ptr(stream))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_box_muller_words")
 
 
 def bm_pipe_probe(op, iters, blocks, threads, sink, stream=None):

@@ -69,6 +69,30 @@ cudaError_t launch_gauss_fill(int prec, int gauss, const PhiloxKeys &K, unsigned
   return cudaGetLastError();
 }
 
+// The variate transforms on GIVEN words (a4; bm_box_muller_words): pair i of `words` -> two standard normals, by the
+// device code of the path kernels (fp64: the own ln / sqrt / sincospi of sim_f64.cuh; fp32: box_muller_f32, W32).
+__global__ void box_muller_words_kernel(int prec, const uint32_t *__restrict__ words, int n_pairs, void *out) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_pairs) return;
+  const uint32_t wa = words[2 * i], wb = words[2 * i + 1];
+  if (prec == BM_F64) {
+    double g0, g1;
+    box_muller_f64(wa, wb, g0, g1);
+    reinterpret_cast<double *>(out)[2 * i] = g0;
+    reinterpret_cast<double *>(out)[2 * i + 1] = g1;
+  } else {
+    float g0, g1;
+    box_muller_f32(wa, wb, g0, g1);
+    reinterpret_cast<float *>(out)[2 * i] = g0;
+    reinterpret_cast<float *>(out)[2 * i + 1] = g1;
+  }
+}
+
+cudaError_t launch_box_muller_words(int prec, const uint32_t *words, int n_pairs, void *out, cudaStream_t st) {
+  box_muller_words_kernel<<<(unsigned)((n_pairs + 127) / 128), 128, 0, st>>>(prec, words, n_pairs, out);
+  return cudaGetLastError();
+}
+
 // Grid pass (a11): one warp per parameter point merges that point's per-block partials.  Lane l takes partials
 // l, l+32, ... in order, then the warp tree merges the 32 lane results: a fixed order for a given
 // (n_paths, block size), hence bit-reproducible.

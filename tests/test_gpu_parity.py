@@ -479,3 +479,49 @@ def test_per_point_dt_equal_entries_reproduce_scalar_dt(B):
                          w.seed, st, pa)
         torch.cuda.synchronize()
         assert np.array_equal(st.cpu().numpy(), s0) and np.array_equal(pa.cpu().numpy(), p0)
+
+
+def test_box_muller_edge_words_against_the_definition(B):
+    """The kernels' own fp64 ln / sqrt / sincospi (sim_f64.cuh) on the words the Philox stream reaches only by chance: u next
+    to 0 and to 1 (w = 0, 2^32 - 1), angles on and next to the quadrant boundaries, mantissas around sqrt(2) (the split of
+    ln u = k ln 2 + ln m), every exponent k.  Expected values: eq. (27), with u(w) = (w + 1/2) 2^-32 (R3),
+    evaluated with mpmath at 40 digits -- the definition itself, not the oracle's libm value (which carries the rounding
+    of 2 pi u: up to 4e-16 r in a normal)."""
+    import mpmath as mp
+    import torch
+    mp.mp.dps = 40
+    edge = [0, 1, 2, 3, 2 ** 32 - 1, 2 ** 32 - 2, 2 ** 31, 2 ** 31 - 1, 2 ** 31 + 1, 2 ** 30, 2 ** 30 - 1, 2 ** 30 + 1,
+            3 * 2 ** 30, 3 * 2 ** 30 - 1, 3 * 2 ** 30 + 1, 2 ** 29, 5 * 2 ** 29, 7 * 2 ** 29 + 1,
+            int(2 ** 32 / mp.sqrt(2)), int(2 ** 32 / mp.sqrt(2)) + 1, int(2 ** 31 / mp.sqrt(2)), int(2 ** 31 * mp.sqrt(2)) - 1]
+    edge += [2 ** k for k in range(1, 32)] + [2 ** k - 1 for k in range(2, 32)] + [2 ** k + 1 for k in range(2, 32)]
+    rng = np.random.default_rng(20141409)
+    rnd = [int(v) for v in rng.integers(0, 2 ** 32, 200)]
+    pairs = [(a, b) for a in edge for b in (0, 2 ** 30, 2 ** 31 - 1, 2 ** 31, 3 * 2 ** 30 + 1, 2 ** 32 - 1, 123456789)]
+    pairs += [(a, b) for b in edge for a in (0, 2 ** 32 - 1, 987654321)] + list(zip(rnd[:100], rnd[100:]))
+    words = torch.tensor(np.array(pairs, dtype=np.uint32).view(np.int32), dtype=torch.int32, device="cuda")
+    out = torch.zeros((len(pairs), 2), dtype=torch.float64, device="cuda")
+    B.bm_box_muller_words(B.BM_F64, words, len(pairs), out)
+    got = out.cpu().numpy()
+    worst = 0.0
+    for (wa, wb), g in zip(pairs, got):
+        ua, ub = (mp.mpf(wa) + mp.mpf(1) / 2) / 2 ** 32, (mp.mpf(wb) + mp.mpf(1) / 2) / 2 ** 32
+        r = mp.sqrt(-2 * mp.log(ua))
+        e0, e1 = r * mp.cos(2 * mp.pi * ub), r * mp.sin(2 * mp.pi * ub)
+        for e, v in ((e0, g[0]), (e1, g[1])):
+            # absolute error in units of the ulp of the RADIUS: a normal next to a zero of the angle is a small
+            # difference of O(r) terms and is good to ulp(r), not to its own ulp
+            err = abs(mp.mpf(float(v)) - e) / mp.mpf(float(np.spacing(float(r))))
+            worst = max(worst, float(err))
+    assert worst <= 2.0, f"fp64 Box-Muller: {worst:.2f} ulp of the radius from the definition"
+    # fp32 W32 transform: MUFU accuracy class (lg2, sqrt, sin, cos approximations), u on a 2^-23 grid (R3)
+    out32 = torch.zeros((len(pairs), 2), dtype=torch.float32, device="cuda")
+    B.bm_box_muller_words(B.BM_F32, words, len(pairs), out32)
+    g32 = out32.cpu().numpy().astype(np.float64)
+    assert np.isfinite(g32).all() and np.abs(g32).max() < 6.0
+    # the fp32 reading of R3: u = ((w >> 9) + 1) 2^-23 for the radius, (w >> 9) 2^-23 turns for the angle
+    wa, wb = np.array([p[0] for p in pairs], dtype=np.int64), np.array([p[1] for p in pairs], dtype=np.int64)
+    r32 = np.sqrt(-2.0 * np.log(((wa >> 9) + 1) * 2.0 ** -23))
+    ang = 2.0 * np.pi * (wb >> 9) * 2.0 ** -23
+    exp32 = np.stack([r32 * np.cos(ang), r32 * np.sin(ang)], axis=1)
+    d32 = np.abs(g32 - exp32).max()
+    assert d32 < 2e-5, f"fp32 Box-Muller (MUFU lg2, sqrt, sin, cos): {d32:.2e} from the definition"
