@@ -29,3 +29,12 @@ show("LOGP_C", cheb_fit(lambda z: (mp.log((1 + mp.sqrt(z)) / (1 - mp.sqrt(z))) /
 ln2 = mp.log(2)
 hi = mp.floor(ln2 * 2 ** 32) / 2 ** 32                           # 32 significant bits: k * LN2_HI is exact for |k| < 2^20
 print("LN2_HI =", repr(float(hi)), " LN2_LO =", repr(float(ln2 - hi)))
+# drive cosine of the inertial model (cos_drive_f64): sin(r) / r and cos(r) in z = r^2 on |r| <= pi/4, and pi/2 in three
+# pieces (33 + 33 + 53 bits: k * PIO2_1 and k * PIO2_2 are exact for |k| < 2^20)
+qz = (mp.pi / 4) ** 2 * mp.mpf("1.0001")
+show("SIN_C", cheb_fit(lambda z: mp.sin(mp.sqrt(z)) / mp.sqrt(z), mp.mpf(0), qz, 8))
+show("COS_C", cheb_fit(lambda z: mp.cos(mp.sqrt(z)), mp.mpf(0), qz, 8))
+pio2 = mp.pi / 2
+p1 = mp.floor(pio2 * 2 ** 32) / 2 ** 32
+p2 = mp.floor((pio2 - p1) * 2 ** 65) / 2 ** 65
+print("PIO2_1 =", repr(float(p1)), " PIO2_2 =", repr(float(p2)), " PIO2_3 =", repr(float(pio2 - p1 - p2)), " TWO_OVER_PI =", repr(float(2 / mp.pi)))

@@ -100,6 +100,37 @@ __device__ __forceinline__ void sincospi_f64(double a, double &sn, double &cs) {
   cs = __hiloint2double(__double2hiint(c0) ^ (((q + 1) & 2) << 30), __double2loint(c0));
 }
 
+// cos x for the drive of the inertial model, |x| < 2^20 (omega t: 1.3e4 at the end of C3): k = nearest integer to
+// x 2/pi, r = x - k pi/2 with pi/2 in three pieces (the first two products are exact), sin r and cos r as polynomials in
+// r^2 on |r| <= pi/4 (both evaluated: two independent chains), then the quadrant.  Branch-free, constants from constant
+// memory; the library's cos spends ~30 UMOV per call on its coefficients and keeps a branch for huge arguments.
+__constant__ double SIN_C[8] = {1.0, -0.16666666666666666, 0.008333333333333321, -0.0001984126984125347, 2.755731921355806e-06,
+                                -2.5052104778015328e-08, 1.6058352290975984e-10, -7.57808328312409e-13};
+__constant__ double COS_C[8] = {1.0, -0.5, 0.04166666666666645, -0.0013888888888861082, 2.4801587283874084e-05,
+                                -2.755731309595641e-07, 2.0875582146477433e-09, -1.1353367957830792e-11};
+__device__ __forceinline__ double cos_drive_f64(double x) {
+  const double MAGIC = 6755399441055744.0;  // 1.5 * 2^52
+  const double t = fma(x, 0.6366197723675814, MAGIC);
+  const int q = __double2loint(t);
+  const double k = t - MAGIC;
+  double r = fma(-k, 1.5707963267341256, x);
+  r = fma(-k, 6.077100506303966e-11, r);
+  r = fma(-k, 2.0222662487959506e-21, r);
+  const double z = r * r;
+  double ps = SIN_C[7], pc = COS_C[7];
+  ps = fma(ps, z, SIN_C[6]); pc = fma(pc, z, COS_C[6]);
+  ps = fma(ps, z, SIN_C[5]); pc = fma(pc, z, COS_C[5]);
+  ps = fma(ps, z, SIN_C[4]); pc = fma(pc, z, COS_C[4]);
+  ps = fma(ps, z, SIN_C[3]); pc = fma(pc, z, COS_C[3]);
+  ps = fma(ps, z, SIN_C[2]); pc = fma(pc, z, COS_C[2]);
+  ps = fma(ps, z, SIN_C[1]); pc = fma(pc, z, COS_C[1]);
+  ps = fma(ps, z, SIN_C[0]); pc = fma(pc, z, COS_C[0]);
+  ps *= r;
+  // cos(r + q pi/2): q = 0 -> cos r, 1 -> -sin r, 2 -> -cos r, 3 -> sin r
+  const double v = (q & 1) ? ps : pc;
+  return __hiloint2double(__double2hiint(v) ^ (((q + 1) & 2) << 30), __double2loint(v));
+}
+
 // Box-Muller pair from two words (R3): r = sqrt(-2 ln u(wa)); (r cos 2 pi u(wb), r sin 2 pi u(wb))
 __device__ __forceinline__ double bm_radius_f64(uint32_t wa) { return sqrt_pos_f64(-2.0 * log_u_f64(u01_bits_f64(wa))); }
 __device__ __forceinline__ void bm_angle_f64(uint32_t wb, double r, double &g0, double &g1) {
@@ -244,7 +275,7 @@ __device__ __forceinline__ double unfolded_f64(const StateF64 &s) {
 // ensemble (C1, C2: 3.5 warps per scheduler) leaves the FP64 pipe idle most of the time; two independent chains per
 // thread fill it.  A path's arithmetic does not depend on NPATH (same operations in the same order per path).
 template <int MODEL, int POT, int NOISE, bool CHUNKED, int NPATH>
-__global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimArgs a) {
+__global__ void __launch_bounds__(256, 2) bm_paths_f64(const __grid_constant__ SimArgs a) {  // two blocks of 256 per SM: <= 128 registers (C2: 256 blocks on 148 SMs)
   constexpr bool HAS_G = NOISE & BM_NOISE_GAUSS, HAS_P = NOISE & BM_NOISE_POISSON, HAS_D = NOISE & BM_NOISE_DICH;
   constexpr bool INERTIAL = MODEL == BM_INERTIAL;
   constexpr int N = NPATH;
@@ -431,8 +462,8 @@ __global__ void __launch_bounds__(256) bm_paths_f64(const __grid_constant__ SimA
 #pragma unroll
       for (int q = 0; q < N; ++q) {
         const double t = __dadd_rn(__dmul_rn((double)n[q], dt), __dsub_rn(dt, rem[q]));
-        A1v[q] = -P.gamma * s[q].v + drift_f64<POT>(P, kf, s[q].xi, cst[q]) + P.amp * cos(P.omega * t);
-        drive[q] = P.amp * cos(P.omega * __dadd_rn(t, h[q]));
+        A1v[q] = -P.gamma * s[q].v + drift_f64<POT>(P, kf, s[q].xi, cst[q]) + P.amp * cos_drive_f64(P.omega * t);
+        drive[q] = P.amp * cos_drive_f64(P.omega * __dadd_rn(t, h[q]));
       }
 #pragma unroll
       for (int q = 0; q < N; ++q) { xb[q] = s[q].xi + s[q].v * h[q]; vb[q] = s[q].v + A1v[q] * h[q] + dxi[q]; }
