@@ -674,6 +674,7 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
   // (its consumer is near, so the instruction scheduler fills the stalls of the serial predictor-corrector chain with
   // it), and the Philox call of the next block is issued at the top of the block.
   constexpr bool UNROLLED = BM_F32_UNROLLED(INERTIAL);  // covered non-clean blocks: unrolled pair slots or a rolled slot loop
+  constexpr bool FIRST = !INERTIAL;  // re-fold in the lane's first sub-step of a non-clean block
   uint4 w = make_uint4(0u, 0u, 0u, 0u);
   Pair cur = Pair{0.f, 0.f, 0.f};
   if (HAS_G && !LCLK) {
@@ -886,6 +887,9 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
         if ((unsigned)(n_discard - n) < (unsigned)NB) ctl |= 0x100u << (n_discard - n);
         if (n + NB > n_end) ctl |= (0xFF00u << (n_end - n)) & 0xFF00u;
       }
+      // the inertial kernel (one form only) folds once at the top of a non-clean block; the over-damped one folds in
+      // the lane's first sub-step of the block (FIRST), which is what its two forms can both do
+      if (INERTIAL) fold_f32<POT>(x, wraps);
       if (careful) {
         // CAREFUL (some lane has more events in this block than its ring holds): every cell is taken as a slow cell,
         // in turns of one event per lane with a refill before each turn, so that a lane's next event is always
@@ -907,7 +911,7 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
               if (!__any_sync(FULL, mine)) break;
               if (mine) do_event(tau, dr_tau, phf);
             }
-            finish_cell(cur.r, jj ? cur.s : cur.c, tau, dr_tau, j == 0);
+            finish_cell(cur.r, jj ? cur.s : cur.c, tau, dr_tau, FIRST && j == 0);
           }
           cur = nxt;
         }
@@ -922,7 +926,7 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
             nxt = (i + 1 < NP) ? pair_of<GW>(w, i + 1, P.cn) : pair_of<GW>(wn, 0, P.cn);
           }
           if (((ctl >> (2 * i)) & 0x303u) == 0u) {
-            fast_cell(cur.r, cur.c, i == 0);
+            fast_cell(cur.r, cur.c, FIRST && i == 0);
             fast_cell(cur.r, cur.s, false);
           } else {
 #pragma unroll
@@ -931,10 +935,10 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
               if (!special_cell(n, j, ctl)) break;
               const float gc = jj ? cur.s : cur.c;
               if (HAS_EV && ((ctl >> j) & 1u)) {
-                slow_cell(n + j, cur.r, gc, j == 0);
+                slow_cell(n + j, cur.r, gc, FIRST && j == 0);
                 ctl |= __reduce_or_sync(FULL, ev_bits(n)) & 0xFFu;  // later events of the same lanes in this block
               } else {
-                fast_cell(cur.r, gc, j == 0);
+                fast_cell(cur.r, gc, FIRST && j == 0);
               }
             }
           }
@@ -948,7 +952,7 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
           Pair nxt = cur;
           if (HAS_G) nxt = pair_dyn(w, wn, i);
           if (((ctl >> (2 * i)) & 0x303u) == 0u) {
-            fast_cell(cur.r, cur.c, i == 0);
+            fast_cell(cur.r, cur.c, FIRST && i == 0);
             fast_cell(cur.r, cur.s, false);
           } else {
 #pragma unroll 1
@@ -957,10 +961,10 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
               if (!special_cell(n, j, ctl)) break;
               const float gc = jj ? cur.s : cur.c;
               if (HAS_EV && ((ctl >> j) & 1u)) {
-                slow_cell(n + j, cur.r, gc, j == 0);
+                slow_cell(n + j, cur.r, gc, FIRST && j == 0);
                 ctl |= __reduce_or_sync(FULL, ev_bits(n)) & 0xFFu;  // later events of the same lanes in this block
               } else {
-                fast_cell(cur.r, gc, j == 0);
+                fast_cell(cur.r, gc, FIRST && j == 0);
               }
             }
           }
