@@ -129,12 +129,15 @@ __device__ __forceinline__ float stage_f32(float base, float x, float k1, float 
 
 // a6: Alg. 1 over a sub-step h with drift a(x) = K0 + f(x), f = -V' without its constant:
 //   x1 = xs + h a(x);  x2 = xs + h/2 (a(x) + a(x1));  x' = xs + h/2 (a(x) + a(x2)),   xs = x + noise.
-// k0 = h K0, k1 = h K1, k2 = h K2 (and their halves).  With xh = (xs + x1)/2 + k0/2 = xs + h/2 a(x) + k0/2 the
+// k1 = h K1, k2 = h K2, k0h = h/2 K0, k1h, k2h likewise.  With xh = (xs + x1)/2 + k0/2 = xs + h/2 a(x) + k0/2 the
 // last two stages are xh + (h/2) f(.).  `xarg` is where a(x) is evaluated (x before folding: same angle).
+// The constant part of the first stage enters as ONE multiply-add, fma(h, K0, xs): written out, so that every path
+// through the kernels rounds it alike (left to the compiler, xs + h K0 is contracted in one place and not in another),
+// and no register has to hold h K0.
 template <int POT, int SINCOS>
-__device__ __forceinline__ float pc_overdamped_f32(float xarg, float xs, float k0, float k1, float k2, float k0h,
+__device__ __forceinline__ float pc_overdamped_f32(float xarg, float xs, float h, float K0, float k1, float k2, float k0h,
                                                    float k1h, float k2h) {
-  const float x1 = stage_f32<POT, SINCOS>(__fadd_rn(xs, k0), xarg, k1, k2);  // never contracted with k0 = h K0
+  const float x1 = stage_f32<POT, SINCOS>(fmaf(h, K0, xs), xarg, k1, k2);
   const float xh = fmaf(0.5f, x1, fmaf(0.5f, xs, k0h));
   const float x2 = stage_f32<POT, SINCOS>(xh, x1, k1h, k2h);
   return stage_f32<POT, SINCOS>(xh, x2, k1h, k2h);
@@ -471,11 +474,11 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
   int cov = min(nP, nD);  // cell of the last event known to this lane, minimum over the streams
   float cst = P.base + (HAS_D ? (d ? P.Gb : P.Ga) : 0.f);
   const float hh_full = 0.5f * dt;
-  // full-step constants of Alg. 1 (loop invariant; k0f, k0h follow cst across a flip)
+  // full-step constants of Alg. 1 (loop invariant; k0h follows cst across a flip)
   // (products by __fmul_rn: the compiler must not contract them into the additions that follow, or the CELLS and the
   // LANES form of the kernel, and fast_cell and sub_step, would round differently)
   const float k1f = __fmul_rn(dt, P.kk1), k2f = __fmul_rn(dt, P.kk2), k1h = __fmul_rn(hh_full, P.kk1), k2h = __fmul_rn(hh_full, P.kk2);
-  float k0f = __fmul_rn(dt, cst), k0h = __fmul_rn(hh_full, cst);
+  float k0h = __fmul_rn(hh_full, cst);
 
   // ---- one refill pass: every lane with room appends one event per stream; returns whether this lane still has a
   //      stream whose last event lies before `limit` and whose ring has room ------------------------------------
@@ -575,7 +578,7 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
     if (do_fold || POT != BM_POT_SINE2) fold_f32<POT>(xf, wraps);
     if (!INERTIAL) {
       const float xs = HAS_G ? fmaf(gr, gc, xf) : xf;
-      x = pc_overdamped_f32<POT, SINCOS>(POT == BM_POT_SINE2 ? x : xf, xs, k0f, k1f, k2f, k0h, k1h, k2h);
+      x = pc_overdamped_f32<POT, SINCOS>(POT == BM_POT_SINE2 ? x : xf, xs, dt, cst, k1f, k2f, k0h, k1h, k2h);
     } else {
       ph += dph;
       const float drive1 = P.amp * cos_turns<SINCOS>(__uint_as_float((uint32_t)(ph >> 41) | 0x3F800000u));
@@ -601,7 +604,7 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
     else xf = x;
     if (!INERTIAL) {
       const float xs = HAS_G ? fmaf(na, nb, xf) : xf;
-      x = pc_overdamped_f32<POT, SINCOS>(x, xs, __fmul_rn(h, cst), __fmul_rn(h, P.kk1), __fmul_rn(h, P.kk2), __fmul_rn(hh, cst),
+      x = pc_overdamped_f32<POT, SINCOS>(x, xs, h, cst, __fmul_rn(h, P.kk1), __fmul_rn(h, P.kk2), __fmul_rn(hh, cst),
                                          __fmul_rn(hh, P.kk1), __fmul_rn(hh, P.kk2));
     } else {
       const float vs = HAS_G ? fmaf(na, nb, v) : v;
@@ -627,7 +630,6 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
     if (HAS_D && !isP) {  // a8: flip
       d ^= 1;
       cst = P.base + (d ? P.Gb : P.Ga);
-      k0f = __fmul_rn(dt, cst);
       k0h = __fmul_rn(hh_full, cst);
       pop_D();
     }
@@ -822,7 +824,7 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
           }
           const float hh = 0.5f * h;
           const float xs = HAS_G ? fmaf(na, nb, xf) : xf;
-          x = pc_overdamped_f32<POT, SINCOS>(xa, xs, __fmul_rn(h, cst), __fmul_rn(h, P.kk1), __fmul_rn(h, P.kk2), __fmul_rn(hh, cst),
+          x = pc_overdamped_f32<POT, SINCOS>(xa, xs, h, cst, __fmul_rn(h, P.kk1), __fmul_rn(h, P.kk2), __fmul_rn(hh, cst),
                                              __fmul_rn(hh, P.kk1), __fmul_rn(hh, P.kk2));
         }
         tau = 0.f;
