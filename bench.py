@@ -38,7 +38,7 @@ XU_LANES_PER_SM = 16          # MUFU lanes per SM per clock (4 per SM sub-partit
 # dram__bytes_read.sum + dram__bytes_write.sum of one path-kernel launch from the committed `ncu --set full` captures
 # (profiles/r2_f32_v7.md; C4: its CELLS and LANES launch together): parameters and per-block partials only, the path is
 # register-resident.  Bytes per call.
-NCU_DRAM_BYTES = {("C1", "f32"): 67840, ("C2", "f32"): 54784, ("C3", "f32"): 87552, ("C4", "f32"): 4710400}
+NCU_DRAM_BYTES = {("C1", "f32"): 66816, ("C2", "f32"): 54784, ("C3", "f32"): 87296, ("C4", "f32"): 4686336}
 
 
 def parse():
@@ -260,7 +260,7 @@ class Runner:
 
 # FP64-pipe arithmetic instructions (DFMA, DMUL, DADD, DSETP) per sub-step of the fp64 kernels as built, from the executed
 # counts of the committed `ncu --set full` captures (profiles/r2_f64_v2.md): the count the fp64 roofline fraction is formed with.
-FP64_OPS_PER_SUBSTEP = {0: 113.5, 1: 168.3}
+FP64_OPS_PER_SUBSTEP = {0: 113.5, 1: 178.3}
 FP64_LANES_PER_SM = 64        # DFMA lanes per SM per clock (bm_pipe_probe: 63)
 
 
