@@ -305,7 +305,7 @@ __global__ void __launch_bounds__(256, 2) bm_paths_f64(const __grid_constant__ S
   uint32_t kP[N], kD[N];
   // normals in flight: one Philox block of four (a single launch), two blocks (CHUNKED, see the time loop)
   constexpr int GQ = CHUNKED ? 8 : 4;
-  double rP[N], rD[N], z[N], rem[N], jumps[N], gq[N][GQ];
+  double rP[N], rD[N], z[N], rem[N], gq[N][GQ];
   unsigned long long blk0[N];  // CHUNKED: Gaussian block the path was in when the launch started
   double *trace[N];
   long long n[N];
@@ -336,7 +336,6 @@ __global__ void __launch_bounds__(256, 2) bm_paths_f64(const __grid_constant__ S
     n[q] = CHUNKED ? a.step_begin : 0;
     m[q] = 0;
     rem[q] = dt;
-    jumps[q] = 0.0;
 #pragma unroll
     for (int j = 0; j < GQ; ++j) gq[q][j] = 0.0;
     snap[q] = s[q];
@@ -344,7 +343,7 @@ __global__ void __launch_bounds__(256, 2) bm_paths_f64(const __grid_constant__ S
       CkptF64 c;
       ckpt_load_f64(a, g[q], c);
       s[q].xi = c.xi; s[q].wraps = c.wraps; s[q].v = c.v; rP[q] = c.rP; rD[q] = c.rD; z[q] = c.z; kP[q] = c.kP; kD[q] = c.kD;
-      d[q] = c.d; m[q] = c.m; jumps[q] = c.jumps; snap[q].xi = c.sxi; snap[q].wraps = c.swraps; snap[q].v = c.sv;
+      d[q] = c.d; m[q] = c.m; snap[q].xi = c.sxi; snap[q].wraps = c.swraps; snap[q].v = c.sv;
     }
     blk0[q] = m[q] >> 2;
     if (CHUNKED && HAS_G) {  // the block the path is in (the next one is drawn in iteration 0 of the loop)
@@ -494,7 +493,6 @@ __global__ void __launch_bounds__(256, 2) bm_paths_f64(const __grid_constant__ S
         rP[q] -= h[q];
         if (rP[q] <= 0.0) {  // kick kP (a8)
           if (!INERTIAL) s[q].xi += z[q]; else s[q].v += z[q];
-          jumps[q] += 1.0;
           kP[q]++;
           const uint4 w = philox_call(a.keys, g[q], STREAM_POISSON, kP[q]);
           rP[q] = -log(u01_f64(w.x)) / P.lambda;
@@ -505,7 +503,6 @@ __global__ void __launch_bounds__(256, 2) bm_paths_f64(const __grid_constant__ S
         rD[q] -= h[q];
         if (rD[q] <= 0.0) {  // flip
           d[q] = 1 - d[q];
-          jumps[q] += 1.0;
           kD[q]++;
           const uint4 w = philox_call(a.keys, g[q], STREAM_DICH, kD[q]);
           rD[q] = -log(u01_f64(w.x)) / (d[q] ? P.mu_b : P.mu_a);
@@ -553,7 +550,7 @@ __global__ void __launch_bounds__(256, 2) bm_paths_f64(const __grid_constant__ S
     if (CHUNKED && a.state != nullptr) {  // row f2: checkpoint (chunks end on completed grid steps, so rem = dt)
       CkptF64 c;
       c.xi = s[q].xi; c.wraps = s[q].wraps; c.v = s[q].v; c.rP = rP[q]; c.rD = rD[q]; c.z = z[q]; c.kP = kP[q]; c.kD = kD[q];
-      c.d = d[q]; c.m = m[q]; c.jumps = jumps[q]; c.sxi = snap[q].xi; c.swraps = snap[q].wraps; c.sv = snap[q].v;
+      c.d = d[q]; c.m = m[q]; c.jumps = (double)(kP[q] + kD[q]); c.sxi = snap[q].xi; c.swraps = snap[q].wraps; c.sv = snap[q].v;
       ckpt_store_f64(a, g[q], c);
     }
     // a10: eq. (30)
@@ -562,10 +559,10 @@ __global__ void __launch_bounds__(256, 2) bm_paths_f64(const __grid_constant__ S
     const double vbar = ((double)(s[q].wraps - snap[q].wraps) * period_f64<POT>() + (s[q].xi - snap[q].xi)) / span;
     if (a.out_paths && (!CHUNKED || a.step_end >= a.n_steps)) {
       double *o = a.out_paths + g[q] * BM_OUT_STRIDE;
-      o[BM_OUT_XT] = xT; o[BM_OUT_VT] = s[q].v; o[BM_OUT_VBAR] = vbar; o[BM_OUT_JUMPS] = jumps[q];
+      o[BM_OUT_XT] = xT; o[BM_OUT_VT] = s[q].v; o[BM_OUT_VBAR] = vbar; o[BM_OUT_JUMPS] = (double)(kP[q] + kD[q]);
       o[BM_OUT_SUBSTEPS] = (double)m[q]; o[BM_OUT_XTI] = unfolded_f64<POT>(snap[q]);
     }
-    mine = merge(mine, leaf(vbar, xT, jumps[q], (double)m[q]));
+    mine = merge(mine, leaf(vbar, xT, (double)(kP[q] + kD[q]), (double)m[q]));  // events applied = the two stream indices
   }
   if (CHUNKED && a.step_end < a.n_steps) return;  // not the last chunk: the partials are not used (uniform over the grid)
   block_reduce_store(mine, a.partials + (long long)blockIdx.x * PARTIAL_STRIDE);
