@@ -155,6 +155,15 @@ __device__ __forceinline__ void ffma2(float a0, float a1, float b0, float b1, fl
   asm("mov.b64 {%0, %1}, %2;" : "=f"(r0), "=f"(r1) : "l"(pr));
 }
 
+// Two independent fp32 products in one instruction (FMUL2): a * (b0, b1), each half rounded as a scalar FMUL.
+__device__ __forceinline__ void fmul2(float a, float b0, float b1, float &r0, float &r1) {
+  unsigned long long pa, pb, pr;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(pa) : "f"(a), "f"(a));
+  asm("mov.b64 %0, {%1, %2};" : "=l"(pb) : "f"(b0), "f"(b1));
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(pr) : "l"(pa), "l"(pb));
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(r0), "=f"(r1) : "l"(pr));
+}
+
 // a7: R7.  y = (x, v), A = (v, -gamma v + f(x) + b(t)); noise in v only (vs = v + noise).  b0 = constant force +
 // drive at t, b1 = the same at t + h; kk1, kk2 are the (unscaled) potential constants in theta units.
 // The two components of the model give pairs of independent multiply-adds at every stage -- (x + h v, x + h/2 v),
@@ -604,8 +613,10 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
     else xf = x;
     if (!INERTIAL) {
       const float xs = HAS_G ? fmaf(na, nb, xf) : xf;
-      x = pc_overdamped_f32<POT, SINCOS>(x, xs, h, cst, __fmul_rn(h, P.kk1), __fmul_rn(h, P.kk2), __fmul_rn(hh, cst),
-                                         __fmul_rn(hh, P.kk1), __fmul_rn(hh, P.kk2));
+      float k1, k2, k1h, k2h;
+      fmul2(h, P.kk1, P.kk2, k1, k2);
+      fmul2(hh, P.kk1, P.kk2, k1h, k2h);
+      x = pc_overdamped_f32<POT, SINCOS>(x, xs, h, cst, k1, k2, __fmul_rn(hh, cst), k1h, k2h);
     } else {
       const float vs = HAS_G ? fmaf(na, nb, v) : v;
       pc_inertial_f32<SINCOS>(x, v, xf, vs, h, hh, P.gamma, P.kk1, P.kk2, cst + dr0, cst + dr1);
@@ -824,8 +835,10 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
           }
           const float hh = 0.5f * h;
           const float xs = HAS_G ? fmaf(na, nb, xf) : xf;
-          x = pc_overdamped_f32<POT, SINCOS>(xa, xs, h, cst, __fmul_rn(h, P.kk1), __fmul_rn(h, P.kk2), __fmul_rn(hh, cst),
-                                             __fmul_rn(hh, P.kk1), __fmul_rn(hh, P.kk2));
+          float k1, k2, k1h, k2h;
+          fmul2(h, P.kk1, P.kk2, k1, k2);
+          fmul2(hh, P.kk1, P.kk2, k1h, k2h);
+          x = pc_overdamped_f32<POT, SINCOS>(xa, xs, h, cst, k1, k2, __fmul_rn(hh, cst), k1h, k2h);
         }
         tau = 0.f;
         c += 1;
