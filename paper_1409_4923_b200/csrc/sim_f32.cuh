@@ -1,8 +1,8 @@
-// sim_f32.cuh -- fp32 path kernel (the throughput kernel), v6.  One thread = one realization; position, next events,
+// sim_f32.cuh -- fp32 path kernel (the throughput kernel), v7.  One thread = one realization; position, next events,
 // Gaussian cache and observable snapshot stay in registers for the whole run.
 //
 // Same method as the fp64 kernel (R1-R9), arranged for fp32 accuracy and for the SM's pipes
-// (profiles/r1_f32_v5.md and profiles/r2_*.md are the measurements this layout answers):
+// (profiles/r2_f32_v7.md holds the measurements this layout answers):
 //  * the position is carried as theta = 2 pi x / L (radians of the potential's phase), folded to [-pi, pi) with an
 //    int32 wrap counter by a round-to-nearest "magic add" (no F2I/FRND, which share the 16-lane XU
 //    pipe with MUFU).  In these units a force cosine is FMUL.RZ + MUFU.COS with no scaling multiply in front;
@@ -33,6 +33,10 @@
 //    BM_GAUSS_W16P: W16 with the angle's sine and cosine as polynomials on the FMA pipe (two MUFU per pair);
 //  * transcendental functions: MUFU.{COS,SIN,LG2,SQRT} (SFU variant) or, for the force cosine,
 //    an even polynomial on the FMA pipe (FMA variant) -- a measured choice (DESIGN.md s.6).
+//  * where events are dense (more than 0.02 per path and cell) the over-damped kernel runs in its LANES form instead:
+//    per-lane clocks in a sliding window of two blocks (bm_config.event_mode; "LANES form" below).  Both forms perform
+//    the same operations per path -- products and sums that the compiler could contract differently in the two are
+//    written out (fmaf, __fmul_rn, FMUL2) -- so their results agree bit for bit;
 // fp32 results are judged statistically against the fp64 oracle (3 combined standard errors).
 #pragma once
 #include "common.cuh"
