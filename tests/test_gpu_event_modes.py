@@ -177,3 +177,34 @@ def test_event_mode_argument_errors(B):
     bad = B.config_for(w, B.BM_F32)
     bad.event_mode = 3
     assert B.bm_workspace_bytes(bad, 1, 64) == 0
+
+
+def test_per_point_step_length_decides_the_form(B, orc):
+    """bm_simulate_dt: the event mode of a point follows lambda times ITS step length.  The same kick rate at dt = 2e-4
+    (0.008 events per cell: CELLS) and at dt = 2e-3 (0.08: LANES) in one call; AUTO = CELLS = LANES bit for bit, and each
+    point against the oracle run at its own dt."""
+    import torch
+    dev = torch.device("cuda:0")
+    n_paths, n_steps = 1024 + 7, 3000
+    params = W.params_table(3, A1=1.0, A2=0.25, F=0.02, D=0.01, lambda_=40.0, zeta=0.1)
+    dts = np.array([2e-4, 2e-3, 1e-3])
+    out = {}
+    for mode in (B.BM_EVENTS_AUTO, B.BM_EVENTS_CELLS, B.BM_EVENTS_LANES):
+        cfg = B.make_config(prec=B.BM_F32, noise=3, n_discard=300, event_mode=mode)
+        st = torch.zeros((3, 8), dtype=torch.float64, device=dev)
+        pa = torch.zeros((3 * n_paths, B.BM_OUT_STRIDE), dtype=torch.float64, device=dev)
+        B.bm_simulate_dt(cfg, torch.from_numpy(params).to(dev), torch.from_numpy(dts).to(dev), 3, n_paths, n_steps, W.SEED, st, pa)
+        torch.cuda.synchronize()
+        out[mode] = (st.cpu().numpy(), pa.cpu().numpy())
+    for mode in (B.BM_EVENTS_CELLS, B.BM_EVENTS_LANES):
+        assert np.array_equal(out[mode][1].view(np.uint64), out[B.BM_EVENTS_AUTO][1].view(np.uint64))
+        assert np.array_equal(out[mode][0].view(np.uint64), out[B.BM_EVENTS_AUTO][0].view(np.uint64))
+    paths = out[B.BM_EVENTS_AUTO][1]
+    for k in range(3):
+        # path g of point k of the sweep = path g of a one-point run whose table has k rows before it: ids select it
+        w = W.Workload("dtp", W.OVERDAMPED, params, n_paths, n_steps, float(dts[k]), 300)
+        ids = np.arange(k * n_paths, (k + 1) * n_paths)
+        ref, _ = oracle_run(orc, w, ids=ids)
+        mine = paths[k * n_paths:(k + 1) * n_paths]
+        assert_3se(mine, ref, B.BM_OUT_VBAR, f"point {k} (dt = {dts[k]}) <v>")
+        assert_counts_close(mine[:, B.BM_OUT_JUMPS], ref[:, orc.OUT_JUMPS], f"point {k}")
