@@ -368,7 +368,10 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
   if (HAS_EV && MODEL == BM_OVERDAMPED && lane_clock_point(a, bp, step_length(a, point), NOISE) != (LCLK != 0)) return;
   const double Dd = HAS_G ? bp.D : 0.0;
   const double dtd = step_length(a, point);
-  const float dt = (float)dtd;
+  float dt = (float)dtd;
+  // (an empty asm makes dt a value the compiler has to keep: in the 64-register class it would rather convert the double
+  // kernel parameter again at every use -- an F2F on the XU pipe in each of the slow-cell copies)
+  asm volatile("" : "+f"(dt));
   const float inv_dt = (float)(1.0 / dtd);
   const double lam = HAS_P ? bp.lambda : 0.0, zet = HAS_P ? bp.zeta : 0.0;
   PointF32 P;
