@@ -493,8 +493,10 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
   // full-step constants of Alg. 1 (loop invariant; k0h follows cst across a flip)
   // (products by __fmul_rn: the compiler must not contract them into the additions that follow, or the CELLS and the
   // LANES form of the kernel, and fast_cell and sub_step, would round differently)
-  const float k1f = __fmul_rn(dt, P.kk1), k2f = __fmul_rn(dt, P.kk2), k1h = __fmul_rn(hh_full, P.kk1), k2h = __fmul_rn(hh_full, P.kk2);
+  float k1f = __fmul_rn(dt, P.kk1), k2f = __fmul_rn(dt, P.kk2), k1h = __fmul_rn(hh_full, P.kk1), k2h = __fmul_rn(hh_full, P.kk2);
   float k0h = __fmul_rn(hh_full, cst);
+  // (64-register class: kept as values, or the compiler multiplies them out again in every pair of cells)
+  if (OCC && !LCLK) asm volatile("" : "+f"(k1f), "+f"(k2f), "+f"(k1h), "+f"(k2h));
 
   // ---- one refill pass: every lane with room appends one event per stream; returns whether this lane still has a
   //      stream whose last event lies before `limit` and whose ring has room ------------------------------------
