@@ -70,12 +70,13 @@ constexpr int EVQ = 8;  // ring capacity per path and stream (a power of two, <=
 constexpr int EVK = 4;  // refill passes per episode
 constexpr int EV_FIELDS_P = 4, EV_FIELDS_D = 3;  // (cell, off, amplitude, normal), (cell, off, normal)
 
-// 32-bit words of dynamic shared memory per thread of the fp32 path kernel (host and device agree through this);
-// lclk: the per-lane-clock form also keeps the normals of one Gaussian call (NB angle parts, NB/2 radii)
+// 32-bit words of dynamic shared memory per thread of the fp32 path kernel (host and device agree through this): one
+// record per thread, padded to an odd number of words; lclk: the per-lane-clock form also keeps the normals of two
+// Gaussian calls in it
 __host__ __device__ constexpr int f32_smem_words_per_thread(int noise, int gauss, int lclk = 0) {
   const int rings = ((noise & BM_NOISE_POISSON) ? EVQ * EV_FIELDS_P : 0) + ((noise & BM_NOISE_DICH) ? EVQ * EV_FIELDS_D : 0) + 4;
   // LANES form: one record per thread, with the normals of two Gaussian calls, padded to an odd number of words
-  return lclk ? ((rings + ((noise & BM_NOISE_GAUSS) ? (gauss == BM_GAUSS_W32 ? 16 : 32) : 0)) | 1) : rings;
+  return (rings + ((lclk && (noise & BM_NOISE_GAUSS)) ? (gauss == BM_GAUSS_W32 ? 16 : 32) : 0)) | 1;
 }
 
 // Event mode of a parameter point (fp32 over-damped jump-adapted kernels; sim_f32.cuh, "per-lane clocks"): expected

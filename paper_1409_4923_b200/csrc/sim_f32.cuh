@@ -287,7 +287,7 @@ __device__ __forceinline__ void gauss_block_standard_f32(const PhiloxKeys &K, un
 // ---- event queues (a5, a8) -----------------------------------------------------------------------------------
 // The kick and flip times of a path do not depend on its motion, so they are drawn AHEAD of time: per path and jump
 // stream the next event sits in registers (cell, offset, amplitude, normal of the sub-step that ends on it) and up to
-// EVQ later ones in a ring in shared memory ([slot][field][thread]: conflict-free whatever the lanes' slots are).
+// EVQ later ones in a ring in shared memory (one record per thread, odd word stride: see the layout in the kernel).
 // The rings are refilled by the whole warp at once, in uniform control flow at the top of a block of cells, EVK
 // events per lane and episode, so one pass of Philox rounds serves up to 32 events instead of the one or two lanes
 // that happen to have an event in a cell.  An episode starts when the last queued event of some lane falls into the
@@ -339,20 +339,22 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
   constexpr int NFP = HAS_P ? EV_FIELDS_P : 0, NFD = HAS_D ? EV_FIELDS_D : 0;
 
   extern __shared__ uint32_t smem_words[];
-  const int T = blockDim.x, tid = threadIdx.x;
-  // CELLS form: field-major arrays [slot][field][thread] (conflict-free whatever slot each lane is at; the strides are
-  // run-time values).  LANES form: one record of REC words per thread, [ring P][ring D][cold][normals], REC odd: every
-  // offset inside the record is an immediate, the few lanes that pop an event in a pass rarely share a bank.
-  constexpr int RECW = EVQ * NFP + EVQ * NFD + 4 + (HAS_G ? 4 * NB : 0), REC = RECW | 1;
-  const int FS = LCLK ? 1 : T;                              // stride between the fields of one slot
-  const int SSP = LCLK ? NFP : NFP * T, SSD = LCLK ? NFD : NFD * T;  // stride between ring slots
-  uint32_t *const ringP = LCLK ? smem_words + tid * REC : smem_words + tid;
-  uint32_t *const ringD = LCLK ? ringP + EVQ * NFP : ringP + EVQ * NFP * T;
+  const int tid = threadIdx.x;
+  // One record of REC words per thread, [ring P][ring D][cold]( + [normals] in the LANES form), REC odd: every offset
+  // inside the record is an immediate of the load or store, and the few lanes that pop an event at the same time rarely
+  // share a bank (lanes 32 / gcd apart in the odd stride).  (A field-major layout [slot][field][thread] is conflict-free
+  // whatever slot each lane is at, but its strides are run-time values: the 64-register class rebuilt the addresses at
+  // every pop, ~10 instructions; measured: C1 12.79 -> 12.70 ms, C2 39.0 -> 38.5 ms with the records.)
+  constexpr int RECW = EVQ * NFP + EVQ * NFD + 4 + ((LCLK && HAS_G) ? 4 * NB : 0), REC = RECW | 1;
+  constexpr int FS = 1;                 // stride between the fields of one slot
+  constexpr int SSP = NFP, SSD = NFD;   // stride between ring slots
+  uint32_t *const ringP = smem_words + tid * REC;
+  uint32_t *const ringD = ringP + EVQ * NFP;
   // state that is touched a few times per run lives in shared memory, not in registers (the 64-register class of the
   // over-damped kernel re-materialises loop constants otherwise): the snapshot at t_i and, per stream, the number of
   // events drawn so far.  The index of a stream's next event = events drawn - events queued - 1 = events applied, so
   // no counter has to follow the events themselves.
-  uint32_t *const cold = LCLK ? ringD + EVQ * NFD : ringD + EVQ * NFD * T;  // [4]: snap_x, snap_w, drawnP, drawnD
+  uint32_t *const cold = ringD + EVQ * NFD;  // [4]: snap_x, snap_w, drawnP, drawnD
   uint32_t *const nrm = cold + 4;  // LANES: the normals of two blocks, angle parts [2 NB] then radii [2 NB]
 
   const int point = blockIdx.x / a.blocks_per_point;
