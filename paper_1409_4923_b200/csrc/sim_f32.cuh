@@ -331,7 +331,7 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
   constexpr bool HAS_EV = HAS_P || HAS_D;
   constexpr bool INERTIAL = MODEL == BM_INERTIAL;
   static_assert(!LCLK || (HAS_EV && !INERTIAL), "per-lane clocks: over-damped model with a jump source");
-  static_assert(EVQ == 8, "the ring pop of the per-lane-clock form clears bit 3 of the read slot");
+  static_assert(EVQ == 8, "the ring pop clears bit 3 of the read slot");
   constexpr int NB = GaussLayout<GW>::NB, NP = GaussLayout<GW>::NP;  // grid cells, pairs per Gaussian call
   constexpr float S = Units<POT>::SCALE;
   constexpr unsigned FULL = 0xffffffffu;
@@ -574,22 +574,22 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
       if (pass + 1 >= EVK && !__any_sync(FULL, more)) break;
     }
   };
+  // (a popped event always has a queued successor: the block is covered, or -- careful path -- the rings were refilled
+  // before the turn; so the ring is never empty here)
   auto pop_P = [&]() {
-    if ((qP >> 4) == 0) { nP = NEVER; return; }  // not reached: a popped event always has a queued successor
     const int s = qP & 15;
     nP = (int)ringP[s * SSP + 0 * FS];
     fP = __uint_as_float(ringP[s * SSP + 1 * FS]);
     z = __uint_as_float(ringP[s * SSP + 2 * FS]);
     if (HAS_G) gP = __uint_as_float(ringP[s * SSP + 3 * FS]);
-    qP = ((qP & ~15) - 16) | ((s + 1) & (EVQ - 1));
+    qP = (qP - 15) & ~EVQ;  // one event less queued, read slot + 1 modulo EVQ (EVQ = 8: bit 3 of the slot is the wrap)
   };
   auto pop_D = [&]() {
-    if ((qD >> 4) == 0) { nD = NEVER; return; }
     const int s = qD & 15;
     nD = (int)ringD[s * SSD + 0 * FS];
     fD = __uint_as_float(ringD[s * SSD + 1 * FS]);
     if (HAS_G) gD = __uint_as_float(ringD[s * SSD + 2 * FS]);
-    qD = ((qD & ~15) - 16) | ((s + 1) & (EVQ - 1));
+    qD = (qD - 15) & ~EVQ;
   };
 
   // ---- FAST: a full grid step without events in this lane (h = dt); noise = gr * gc ----------------------------
