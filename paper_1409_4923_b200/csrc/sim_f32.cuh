@@ -39,6 +39,8 @@
 //    written out (fmaf, __fmul_rn, FMUL2) -- so their results agree bit for bit;
 // fp32 results are judged statistically against the fp64 oracle (3 combined standard errors).
 #pragma once
+#include <type_traits>
+
 #include "common.cuh"
 
 
@@ -310,6 +312,23 @@ __device__ __forceinline__ void gauss_block_standard_f32(const PhiloxKeys &K, un
 #define BM_F32_BOUNDS(model, occ) __launch_bounds__((model) == BM_INERTIAL ? 256 : 512, ((model) != BM_INERTIAL && (occ)) ? 2 : 1)
 #endif
 
+// A thread's record in dynamic shared memory, addressed in the shared state space: one 32-bit base kept in a register and
+// immediate word offsets.  (Through generic pointers the 64-register class rebuilt the shared window's base -- S2R, MOV,
+// IADD3, LEA, S2R, IMAD -- in every slow cell.)  volatile + "memory": a load is never moved across a store of the record.
+struct SmemRec {
+  uint32_t base;
+  template <int W>
+  __device__ __forceinline__ uint32_t ld(uint32_t dyn_bytes = 0u) const {
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1+%2];" : "=r"(v) : "r"(base + dyn_bytes), "n"(4 * W) : "memory");
+    return v;
+  }
+  template <int W>
+  __device__ __forceinline__ void st(uint32_t v, uint32_t dyn_bytes = 0u) const {
+    asm volatile("st.shared.u32 [%0+%1], %2;" : : "r"(base + dyn_bytes), "n"(4 * W), "r"(v) : "memory");
+  }
+};
+
 // Per-point constants, fp32, theta units (theta = SCALE x)
 struct PointF32 {
   float kk1, kk2;    // SINE2: SCALE * (-V') = base-part + c (kk1 + kk2 c), c = cos theta.  PWL/QUAD: kk1 = A1
@@ -346,16 +365,14 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
   // whatever slot each lane is at, but its strides are run-time values: the 64-register class rebuilt the addresses at
   // every pop, ~10 instructions; measured: C1 12.79 -> 12.70 ms, C2 39.0 -> 38.5 ms with the records.)
   constexpr int RECW = EVQ * NFP + EVQ * NFD + 4 + ((LCLK && HAS_G) ? 4 * NB : 0), REC = RECW | 1;
-  constexpr int FS = 1;                 // stride between the fields of one slot
-  constexpr int SSP = NFP, SSD = NFD;   // stride between ring slots
-  uint32_t *const ringP = smem_words + tid * REC;
-  uint32_t *const ringD = ringP + EVQ * NFP;
-  // state that is touched a few times per run lives in shared memory, not in registers (the 64-register class of the
-  // over-damped kernel re-materialises loop constants otherwise): the snapshot at t_i and, per stream, the number of
-  // events drawn so far.  The index of a stream's next event = events drawn - events queued - 1 = events applied, so
-  // no counter has to follow the events themselves.
-  uint32_t *const cold = ringD + EVQ * NFD;  // [4]: snap_x, snap_w, drawnP, drawnD
-  uint32_t *const nrm = cold + 4;  // LANES: the normals of two blocks, angle parts [2 NB] then radii [2 NB]
+  constexpr int OFF_D = EVQ * NFP, OFF_COLD = EVQ * (NFP + NFD), OFF_NRM = OFF_COLD + 4;  // word offsets in the record
+  // [ring P: EVQ x NFP][ring D: EVQ x NFD][cold: snap_x, snap_w, drawnP, drawnD][LANES: normals of two blocks]
+  // State that is touched a few times per run lives here, not in registers: the snapshot at t_i and, per stream, the
+  // number of events drawn so far.  The index of a stream's next event = events drawn - events queued - 1 = events
+  // applied, so no counter has to follow the events themselves.
+  SmemRec R;
+  R.base = (uint32_t)__cvta_generic_to_shared(smem_words + tid * REC);
+  asm volatile("" : "+r"(R.base));  // a value to keep, not an address to rebuild
 
   const int point = blockIdx.x / a.blocks_per_point;
   const int chunk = blockIdx.x - point * a.blocks_per_point;
@@ -485,10 +502,10 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
     io.get2(8, lo, hi); drive0 = __uint_as_float(lo); snap_x = __uint_as_float(hi);
     io.get2(9, lo, hi); snap_w = (int)lo;
   }
-  cold[0 * FS] = __float_as_uint(snap_x);
-  cold[1 * FS] = (uint32_t)snap_w;
-  cold[2 * FS] = drawnP;
-  cold[3 * FS] = drawnD;
+  R.template st<OFF_COLD + 0>(__float_as_uint(snap_x));
+  R.template st<OFF_COLD + 1>((uint32_t)snap_w);
+  R.template st<OFF_COLD + 2>(drawnP);
+  R.template st<OFF_COLD + 3>(drawnD);
   int cov = min(nP, nD);  // cell of the last event known to this lane, minimum over the streams
   float cst = P.base + (HAS_D ? (d ? P.Gb : P.Ga) : 0.f);
   const float hh_full = 0.5f * dt;
@@ -511,22 +528,22 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
       float tf = fP;
       if (cnt > 0) {
         const int s = (rd + cnt - 1) & (EVQ - 1);
-        tc = (int)ringP[s * SSP + 0 * FS];
-        tf = __uint_as_float(ringP[s * SSP + 1 * FS]);
+        tc = (int)R.template ld<0>(s * (NFP * 4));
+        tf = __uint_as_float(R.template ld<1>(s * (NFP * 4)));
       }
       tailP = tc;
       if (cnt < EVQ && tc != NEVER) {
-        const uint32_t drawn = cold[2 * FS];
-        cold[2 * FS] = drawn + 1u;
+        const uint32_t drawn = R.template ld<OFF_COLD + 2>();
+        R.template st<OFF_COLD + 2>(drawn + 1u);
         const uint4 w = philox_call(K, g, STREAM_POISSON, drawn);
         int c;
         float f;
         schedule_f32(tc, tf, dt, inv_dt, neg_log_u_f32(w.x) * P.inv_lam_dt, c, f);
         const int s = (rd + cnt) & (EVQ - 1);
-        ringP[s * SSP + 0 * FS] = (uint32_t)c;
-        ringP[s * SSP + 1 * FS] = __float_as_uint(f);
-        ringP[s * SSP + 2 * FS] = __float_as_uint(P.zeta * neg_log_u_f32(w.y));
-        if (HAS_G) ringP[s * SSP + 3 * FS] = __float_as_uint(event_normal(w.z));
+        R.template st<0>((uint32_t)c, s * (NFP * 4));
+        R.template st<1>(__float_as_uint(f), s * (NFP * 4));
+        R.template st<2>(__float_as_uint(P.zeta * neg_log_u_f32(w.y)), s * (NFP * 4));
+        if (HAS_G) R.template st<3>(__float_as_uint(event_normal(w.z)), s * (NFP * 4));
         qP += 16;
         tailP = c;
         did = true;
@@ -539,22 +556,22 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
       float tf = fD;
       if (cnt > 0) {
         const int s = (rd + cnt - 1) & (EVQ - 1);
-        tc = (int)ringD[s * SSD + 0 * FS];
-        tf = __uint_as_float(ringD[s * SSD + 1 * FS]);
+        tc = (int)R.template ld<OFF_D + 0>(s * (NFD * 4));
+        tf = __uint_as_float(R.template ld<OFF_D + 1>(s * (NFD * 4)));
       }
       tailD = tc;
       if (cnt < EVQ && tc != NEVER) {
-        const uint32_t drawn = cold[3 * FS];
-        cold[3 * FS] = drawn + 1u;
+        const uint32_t drawn = R.template ld<OFF_COLD + 3>();
+        R.template st<OFF_COLD + 3>(drawn + 1u);
         const uint4 w = philox_call(K, g, STREAM_DICH, drawn);
         const int dn = d ^ ((cnt + 1) & 1);  // the state entered by the last queued flip
         int c;
         float f;
         schedule_f32(tc, tf, dt, inv_dt, neg_log_u_f32(w.x) * (dn ? P.inv_mub_dt : P.inv_mua_dt), c, f);
         const int s = (rd + cnt) & (EVQ - 1);
-        ringD[s * SSD + 0 * FS] = (uint32_t)c;
-        ringD[s * SSD + 1 * FS] = __float_as_uint(f);
-        if (HAS_G) ringD[s * SSD + 2 * FS] = __float_as_uint(event_normal(w.z));
+        R.template st<OFF_D + 0>((uint32_t)c, s * (NFD * 4));
+        R.template st<OFF_D + 1>(__float_as_uint(f), s * (NFD * 4));
+        if (HAS_G) R.template st<OFF_D + 2>(__float_as_uint(event_normal(w.z)), s * (NFD * 4));
         qD += 16;
         tailD = c;
         did = true;
@@ -578,17 +595,17 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
   // before the turn; so the ring is never empty here)
   auto pop_P = [&]() {
     const int s = qP & 15;
-    nP = (int)ringP[s * SSP + 0 * FS];
-    fP = __uint_as_float(ringP[s * SSP + 1 * FS]);
-    z = __uint_as_float(ringP[s * SSP + 2 * FS]);
-    if (HAS_G) gP = __uint_as_float(ringP[s * SSP + 3 * FS]);
+    nP = (int)R.template ld<0>(s * (NFP * 4));
+    fP = __uint_as_float(R.template ld<1>(s * (NFP * 4)));
+    z = __uint_as_float(R.template ld<2>(s * (NFP * 4)));
+    if (HAS_G) gP = __uint_as_float(R.template ld<3>(s * (NFP * 4)));
     qP = (qP - 15) & ~EVQ;  // one event less queued, read slot + 1 modulo EVQ (EVQ = 8: bit 3 of the slot is the wrap)
   };
   auto pop_D = [&]() {
     const int s = qD & 15;
-    nD = (int)ringD[s * SSD + 0 * FS];
-    fD = __uint_as_float(ringD[s * SSD + 1 * FS]);
-    if (HAS_G) gD = __uint_as_float(ringD[s * SSD + 2 * FS]);
+    nD = (int)R.template ld<OFF_D + 0>(s * (NFD * 4));
+    fD = __uint_as_float(R.template ld<OFF_D + 1>(s * (NFD * 4)));
+    if (HAS_G) gD = __uint_as_float(R.template ld<OFF_D + 2>(s * (NFD * 4)));
     qD = (qD - 15) & ~EVQ;
   };
 
@@ -720,8 +737,8 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
     if ((ctl >> j) & 0x100u) {
       if (n + j >= n_end) return false;
       fold_f32<POT>(x, wraps);
-      cold[0 * FS] = __float_as_uint(x);
-      cold[1 * FS] = (uint32_t)wraps;
+      R.template st<OFF_COLD + 0>(__float_as_uint(x));
+      R.template st<OFF_COLD + 1>((uint32_t)wraps);
     }
     return true;
   };
@@ -761,13 +778,19 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
         if (ok) {
           if (HAS_G) {
             const uint4 wg = philox_call(K, g, STREAM_GAUSS, (uint32_t)(G / NB));
-            uint32_t *const dst = nrm + (G & (WC - 1));
-#pragma unroll
-            for (int i = 0; i < NP; ++i) {
-              const Pair q = pair_of<GW>(wg, i, P.cn);
-              dst[2 * i] = __float_as_uint(q.c);
-              dst[2 * i + 1] = __float_as_uint(q.s);
-              dst[WC + 2 * i] = dst[WC + 2 * i + 1] = __float_as_uint(q.r);
+            const uint32_t dst = (uint32_t)(G & (WC - 1)) * 4u;
+            auto put_pair = [&](auto IT, const Pair &q) {
+              constexpr int I = decltype(IT)::value;
+              R.template st<OFF_NRM + 2 * I>(__float_as_uint(q.c), dst);
+              R.template st<OFF_NRM + 2 * I + 1>(__float_as_uint(q.s), dst);
+              R.template st<OFF_NRM + WC + 2 * I>(__float_as_uint(q.r), dst);
+              R.template st<OFF_NRM + WC + 2 * I + 1>(__float_as_uint(q.r), dst);
+            };
+            put_pair(std::integral_constant<int, 0>(), pair_of<GW>(wg, 0, P.cn));
+            put_pair(std::integral_constant<int, 1>(), pair_of<GW>(wg, 1, P.cn));
+            if (NP == 4) {
+              put_pair(std::integral_constant<int, 2>(), pair_of<GW>(wg, 2, P.cn));
+              put_pair(std::integral_constant<int, 3>(), pair_of<GW>(wg, 3, P.cn));
             }
           }
           G += NB;
@@ -784,8 +807,8 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
             if (cc >= n_end) break;
             if (cc == n_discard) {  // a10: snapshot at t_i
               fold_f32<POT>(x, wraps);
-              cold[0 * FS] = __float_as_uint(x);
-              cold[1 * FS] = (uint32_t)wraps;
+              R.template st<OFF_COLD + 0>(__float_as_uint(x));
+              R.template st<OFF_COLD + 1>((uint32_t)wraps);
             }
             Pair q = Pair{0.f, 0.f, 0.f};
             if (HAS_G) {
@@ -829,8 +852,8 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
         const float h = fmaxf(te - tau, 0.f);
         float na = 0.f, nb = 0.f;
         if (HAS_G) {
-          const uint32_t *const q = nrm + (c & (WC - 1));
-          const float gc = __uint_as_float(q[0]), gr = __uint_as_float(q[WC]);
+          const uint32_t q = (uint32_t)(c & (WC - 1)) * 4u;
+          const float gc = __uint_as_float(R.template ld<OFF_NRM>(q)), gr = __uint_as_float(R.template ld<OFF_NRM + WC>(q));
           const float sq = sqrt_approx(h * (ev ? P.s2 : inv_dt));
           na = ev ? (isP ? gP : gD) : (whole ? gr : gr * gc);
           nb = whole ? gc : sq;
@@ -859,19 +882,19 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
           if (HAS_P && isP) {  // a8: kick
             x = __fadd_rn(x, z);
             const int s = qP & 15;
-            nP = (int)ringP[s * NFP + 0];
-            fP = __uint_as_float(ringP[s * NFP + 1]);
-            z = __uint_as_float(ringP[s * NFP + 2]);
-            if (HAS_G) gP = __uint_as_float(ringP[s * NFP + 3]);
+            nP = (int)R.template ld<0>(s * (NFP * 4));
+            fP = __uint_as_float(R.template ld<1>(s * (NFP * 4)));
+            z = __uint_as_float(R.template ld<2>(s * (NFP * 4)));
+            if (HAS_G) gP = __uint_as_float(R.template ld<3>(s * (NFP * 4)));
             qP = (qP - 15) & ~EVQ;  // one event less queued, read slot + 1 modulo EVQ
           }
           if (HAS_D && !isP) {  // a8: flip
             d ^= 1;
             cst = P.base + (d ? P.Gb : P.Ga);
             const int s = qD & 15;
-            nD = (int)ringD[s * NFD + 0];
-            fD = __uint_as_float(ringD[s * NFD + 1]);
-            if (HAS_G) gD = __uint_as_float(ringD[s * NFD + 2]);
+            nD = (int)R.template ld<OFF_D + 0>(s * (NFD * 4));
+            fD = __uint_as_float(R.template ld<OFF_D + 1>(s * (NFD * 4)));
+            if (HAS_G) gD = __uint_as_float(R.template ld<OFF_D + 2>(s * (NFD * 4)));
             qD = (qD - 15) & ~EVQ;
           }
         }
@@ -1003,11 +1026,11 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
 
   // events applied per stream = events drawn - events still queued (the ring and the head); it is also the index of
   // the stream's next event, i.e. of the Philox call it came from
-  const uint32_t kP = (HAS_P && cold[2 * FS] > 0u) ? cold[2 * FS] - (uint32_t)(qP >> 4) - 1u : 0u;
-  const uint32_t kD = (HAS_D && cold[3 * FS] > 0u) ? cold[3 * FS] - (uint32_t)(qD >> 4) - 1u : 0u;
+  const uint32_t kP = (HAS_P && R.template ld<OFF_COLD + 2>() > 0u) ? R.template ld<OFF_COLD + 2>() - (uint32_t)(qP >> 4) - 1u : 0u;
+  const uint32_t kD = (HAS_D && R.template ld<OFF_COLD + 3>() > 0u) ? R.template ld<OFF_COLD + 3>() - (uint32_t)(qD >> 4) - 1u : 0u;
   const int jumps = (int)(kP + kD);
-  snap_x = __uint_as_float(cold[0 * FS]);
-  snap_w = (int)cold[1 * FS];
+  snap_x = __uint_as_float(R.template ld<OFF_COLD + 0>());
+  snap_w = (int)R.template ld<OFF_COLD + 1>();
   if (a.state != nullptr && valid) {  // row f2: checkpoint
     const StateIO io = state_io(a, g);
     io.put2(0, __float_as_uint(x), (uint32_t)wraps);
