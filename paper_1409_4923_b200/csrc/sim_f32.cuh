@@ -939,8 +939,9 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
       // the inertial kernel (one form only) folds once at the top of a non-clean block; the over-damped one folds in
       // the lane's first sub-step of the block (FIRST), which is what its two forms can both do
       if (INERTIAL) fold_f32<POT>(x, wraps);
-      if (careful) {
-        // CAREFUL (some lane has more events in this block than its ring holds): every cell is taken as a slow cell,
+      if (careful || special) {
+        // CAREFUL (some lane has more events in this block than its ring holds; also the two blocks of a run that hold
+        // t_i and its end, so that the covered paths below carry no test for them): every cell is taken as a slow cell,
         // in turns of one event per lane with a refill before each turn, so that a lane's next event is always
         // known before it is needed.  Same arithmetic per lane as the covered path.
         if (HAS_G) philox_rounds<0, 10>(wn, K);
@@ -974,14 +975,13 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
             next_rounds(wn, i);
             nxt = (i + 1 < NP) ? pair_of<GW>(w, i + 1, P.cn) : pair_of<GW>(wn, 0, P.cn);
           }
-          if (((ctl >> (2 * i)) & 0x303u) == 0u) {
+          if (((ctl >> (2 * i)) & 3u) == 0u) {
             fast_cell(cur.r, cur.c, FIRST && i == 0);
             fast_cell(cur.r, cur.s, false);
           } else {
 #pragma unroll
             for (int jj = 0; jj < 2; ++jj) {
               const int j = 2 * i + jj;
-              if (!special_cell(n, j, ctl)) break;
               const float gc = jj ? cur.s : cur.c;
               if (HAS_EV && ((ctl >> j) & 1u)) {
                 slow_cell(n + j, cur.r, gc, FIRST && j == 0);
@@ -1000,14 +1000,13 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
         for (int i = 0; i < NP; ++i) {
           Pair nxt = cur;
           if (HAS_G) nxt = pair_dyn(w, wn, i);
-          if (((ctl >> (2 * i)) & 0x303u) == 0u) {
+          if (((ctl >> (2 * i)) & 3u) == 0u) {
             fast_cell(cur.r, cur.c, FIRST && i == 0);
             fast_cell(cur.r, cur.s, false);
           } else {
 #pragma unroll 1
             for (int jj = 0; jj < 2; ++jj) {
               const int j = 2 * i + jj;
-              if (!special_cell(n, j, ctl)) break;
               const float gc = jj ? cur.s : cur.c;
               if (HAS_EV && ((ctl >> j) & 1u)) {
                 slow_cell(n + j, cur.r, gc, FIRST && j == 0);
