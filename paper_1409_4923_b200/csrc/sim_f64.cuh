@@ -34,7 +34,7 @@ __device__ __forceinline__ double u01_bits_f64(uint32_t w) {
 }
 
 // ln u for a normal u in (0, 1): u = 2^k m, m in [sqrt(1/2), sqrt(2)); with f = m - 1, s = f / (2 + f), z = s^2:
-// ln m = 2 atanh s = f - s (f - z P(z)).  The quotient by a reciprocal seed and two Newton steps, then one correction.
+// ln m = 2 atanh s = f - s (f - z P(z)).  The quotient by a reciprocal seed, one Newton step, then one correction.
 __device__ __forceinline__ double log_u_f64(double u) {
   int hi = __double2hiint(u);
   hi += 0x3ff00000 - 0x3fe6a09e;  // mantissas above sqrt(2) carry into the exponent
@@ -43,10 +43,8 @@ __device__ __forceinline__ double log_u_f64(double u) {
   const double f = m - 1.0, y = 2.0 + f;
   double r;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(y));
-  double e = fma(-y, r, 1.0);
-  r = fma(r, e, r);
-  e = fma(-y, r, 1.0);
-  r = fma(r, e, r);
+  const double e = fma(-y, r, 1.0);
+  r = fma(r, e, r);  // one Newton step on the seed: a relative error of ~2^-40; the correction below squares it again
   double sq = f * r;
   sq = fma(fma(-y, sq, f), r, sq);  // s = f / y
   const double z = sq * sq;
@@ -62,17 +60,14 @@ __device__ __forceinline__ double log_u_f64(double u) {
   return fma(dk, 0.6931471803691238, fma(dk, 1.9082149292705877e-10, lm));  // k ln2 in two parts: the first product is exact
 }
 
-// sqrt x for a normal x > 0: reciprocal-root seed, two coupled Newton steps on (g, h) -> (sqrt x, 1 / (2 sqrt x)), one correction
+// sqrt x for a normal x > 0: reciprocal-root seed, one coupled Newton step on (g, h) -> (sqrt x, 1 / (2 sqrt x)), one correction
 __device__ __forceinline__ double sqrt_pos_f64(double x) {
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
   double g = x * y, h = 0.5 * y;
-  double r = fma(-g, h, 0.5);
+  const double r = fma(-g, h, 0.5);
   g = fma(g, r, g);
-  h = fma(h, r, h);
-  r = fma(-g, h, 0.5);
-  g = fma(g, r, g);
-  h = fma(h, r, h);
+  h = fma(h, r, h);  // one coupled step on the seed: ~2^-40; the correction below squares it again
   return fma(fma(-g, g, x), h, g);
 }
 
