@@ -260,7 +260,7 @@ class Runner:
 
 # FP64-pipe arithmetic instructions (DFMA, DMUL, DADD, DSETP) per sub-step of the fp64 kernels as built, from the executed
 # counts of the committed `ncu --set full` captures (profiles/r2_f64_v2.md): the count the fp64 roofline fraction is formed with.
-FP64_OPS_PER_SUBSTEP = {0: 113.5, 1: 178.3}
+FP64_OPS_PER_SUBSTEP = {0: 110.9, 1: 175.7}
 FP64_LANES_PER_SM = 64        # DFMA lanes per SM per clock (bm_pipe_probe: 63)
 
 
