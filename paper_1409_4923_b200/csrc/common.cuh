@@ -76,7 +76,8 @@ constexpr int EV_FIELDS_P = 4, EV_FIELDS_D = 3;  // (cell, off, amplitude, norma
 __host__ __device__ constexpr int f32_smem_words_per_thread(int noise, int gauss, int lclk = 0) {
   const int rings = ((noise & BM_NOISE_POISSON) ? EVQ * EV_FIELDS_P : 0) + ((noise & BM_NOISE_DICH) ? EVQ * EV_FIELDS_D : 0) + 4;
   // LANES form: one record per thread, with the normals of two Gaussian calls, padded to an odd number of words
-  return (rings + ((lclk && (noise & BM_NOISE_GAUSS)) ? (gauss == BM_GAUSS_W32 ? 16 : 32) : 0)) | 1;
+  const int extra = !(noise & BM_NOISE_GAUSS) ? 0 : lclk ? (gauss == BM_GAUSS_W32 ? 16 : 32) : (gauss == BM_GAUSS_W32 ? 0 : 4);
+  return (rings + extra) | 1;  // CELLS form, W16 / W16P: four words for the pairs of the rolled paths
 }
 
 // Event mode of a parameter point (fp32 over-damped jump-adapted kernels; sim_f32.cuh, "per-lane clocks"): expected

@@ -364,9 +364,10 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
   // share a bank (lanes 32 / gcd apart in the odd stride).  (A field-major layout [slot][field][thread] is conflict-free
   // whatever slot each lane is at, but its strides are run-time values: the 64-register class rebuilt the addresses at
   // every pop, ~10 instructions; measured: C1 12.79 -> 12.70 ms, C2 39.0 -> 38.5 ms with the records.)
-  constexpr int RECW = EVQ * NFP + EVQ * NFD + 4 + ((LCLK && HAS_G) ? 4 * NB : 0), REC = RECW | 1;
+  constexpr int RECW = EVQ * NFP + EVQ * NFD + 4 + (HAS_G ? (LCLK ? 4 * NB : (GW == BM_GAUSS_W32 ? 0 : 4)) : 0), REC = RECW | 1;
   constexpr int OFF_D = EVQ * NFP, OFF_COLD = EVQ * (NFP + NFD), OFF_NRM = OFF_COLD + 4;  // word offsets in the record
-  // [ring P: EVQ x NFP][ring D: EVQ x NFD][cold: snap_x, snap_w, drawnP, drawnD][LANES: normals of two blocks]
+  // [ring P: EVQ x NFP][ring D: EVQ x NFD][cold: snap_x, snap_w, drawnP, drawnD][LANES: normals of two blocks; CELLS, W16:
+  // the four words the rolled paths form their pairs from]
   // State that is touched a few times per run lives here, not in registers: the snapshot at t_i and, per stream, the
   // number of events drawn so far.  The index of a stream's next event = events drawn - events queued - 1 = events
   // applied, so no counter has to follow the events themselves.
@@ -748,8 +749,18 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
       const bool last = i + 1 >= NP;
       return pair_w32(last ? w1.x : w0.z, last ? w1.y : w0.w, P.cn);
     }
-    const uint32_t ww = i == 0 ? w0.y : i == 1 ? w0.z : i == 2 ? w0.w : w1.x;
+    // (the word of pair i + 1 with a run-time i: from the record, where stash_words put w0.y, w0.z, w0.w, w1.x -- one
+    // load instead of a four-way select)
+    const uint32_t ww = R.template ld<OFF_NRM>((uint32_t)i * 4u);
     return GW == BM_GAUSS_W16P ? pair_w16p(ww, P.cn) : pair_w16(ww, P.cn);
+  };
+  auto stash_words = [&](const uint4 &w0, const uint4 &w1) {
+    if (HAS_G && GW != BM_GAUSS_W32) {
+      R.template st<OFF_NRM + 0>(w0.y);
+      R.template st<OFF_NRM + 1>(w0.z);
+      R.template st<OFF_NRM + 2>(w0.w);
+      R.template st<OFF_NRM + 3>(w1.x);
+    }
   };
 
   // ---- LANES form: per-lane clocks in a sliding window ------------------------------------------------------------
@@ -945,6 +956,7 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
         // in turns of one event per lane with a refill before each turn, so that a lane's next event is always
         // known before it is needed.  Same arithmetic per lane as the covered path.
         if (HAS_G) philox_rounds<0, 10>(wn, K);
+        stash_words(w, wn);
 #pragma unroll 1
         for (int i = 0; i < NP; ++i) {
           Pair nxt = cur;
@@ -996,6 +1008,7 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
       } else {
         // COVERED, rolled over the pair slots (one copy of the slow-cell code)
         if (HAS_G) philox_rounds<0, 10>(wn, K);
+        stash_words(w, wn);
 #pragma unroll 1
         for (int i = 0; i < NP; ++i) {
           Pair nxt = cur;
