@@ -38,7 +38,7 @@ XU_LANES_PER_SM = 16          # MUFU lanes per SM per clock (4 per SM sub-partit
 # dram__bytes_read.sum + dram__bytes_write.sum of one path-kernel launch from the committed `ncu --set full` captures
 # (profiles/r2_f32_v7.md; C4: its CELLS and LANES launch together): parameters and per-block partials only, the path is
 # register-resident.  Bytes per call.
-NCU_DRAM_BYTES = {("C1", "f32"): 64768, ("C2", "f32"): 54016, ("C3", "f32"): 86528, ("C4", "f32"): 4353280}
+NCU_DRAM_BYTES = {("C1", "f32"): 64512, ("C2", "f32"): 53760, ("C3", "f32"): 86272, ("C4", "f32"): 4351488}
 
 
 def parse():
