@@ -238,6 +238,30 @@ BM_API bm_status bm_simulate_host(const bm_config *cfg, const bm_params *params,
                            int64_t n_steps, double dt, uint64_t seed, bm_stats *out_stats, double *out_paths,
                            void *stream);
 
+/*
+ * bm_simulate for callers that cannot allocate device memory.  bm_simulate asks the caller for `workspace`; this entry
+ * takes none.  It is meant for code that has no allocator to call: a plug-in inside an application that owns the GPU
+ * heap, a real-time loop where cudaMalloc (which may synchronise the device and has no time bound) is off limits, a
+ * process whose device memory is already fully committed.  The scratch is a fixed array of BM_STATIC_SCRATCH_BYTES
+ * inside the library's device image: every GPU on which libbm.so is loaded holds those 4 MiB from module load until the
+ * process exits, used or not.  The call performs no cudaMalloc, cudaFree, pool or other allocating routine.
+ *   Arguments, outputs, errors and results: exactly bm_simulate's (same kernels, same reduction tree, bit-identical
+ *   out_stats / out_paths / out_trace); params, out_* are DEVICE pointers the caller owns, as there.
+ *   Limit: bm_workspace_bytes(cfg, n_points, n_paths) <= BM_STATIC_SCRATCH_BYTES, i.e. at most 65 536 thread blocks
+ *   (n_points x ceil(n_paths / block size)); beyond it the call returns BM_ERR_WORKSPACE and launches nothing.
+ *   First call on a device: looks up the array's device address (cudaGetSymbolAddress, with the calling thread's current
+ *   device) and keeps it; make that first call outside any stream capture.  Later calls on that device skip the look-up.
+ *   Sharing: all calls on one device use the same array, and it keeps whatever the last call wrote.  Nothing in it needs
+ *   clearing (each call overwrites every slot it later reads), but two calls that may run on the GPU at the same time --
+ *   different streams, or different host threads without ordering between their streams -- race on it and corrupt each
+ *   other's statistics.  Keep calls on one device in one stream, or order them with events.  bm_simulate with
+ *   caller-owned workspaces has no such restriction.
+ */
+enum { BM_STATIC_SCRATCH_BYTES = 4 * 1024 * 1024 };
+BM_API bm_status bm_simulate_static(const bm_config *cfg, const bm_params *params, int32_t n_points, int64_t n_paths,
+                             int64_t n_steps, double dt, uint64_t seed, bm_stats *out_stats, double *out_paths,
+                             double *out_trace, void *stream);
+
 /* Raw Philox4x32-10 words (R1, R2): out[p][j][0..3] = call (seed, g = path0+p, stream_id, idx = idx0+j). */
 BM_API bm_status bm_philox_fill(uint64_t seed, uint64_t path0, int32_t n_paths, uint32_t stream_id, uint32_t idx0,
                          int32_t n_idx, uint32_t *out, void *stream);

@@ -30,7 +30,8 @@ BM_STATE_SLOTS, BM_CHUNK_ALIGN = 16, 8
 (BM_MOM_N, BM_MOM_MEAN_X, BM_MOM_VAR_X, BM_MOM_MEAN_V, BM_MOM_VAR_V, BM_MOM_MEAN_DX, BM_MOM_VAR_DX, BM_MOM_COV_V0V,
  BM_MOM_VAR_V0) = range(9)
 BM_MOM_STRIDE = 10
-EXPORTS = ("bm_workspace_bytes", "bm_simulate", "bm_simulate_dt", "bm_state_bytes", "bm_simulate_chunk", "bm_state_histogram",
+BM_STATIC_SCRATCH_BYTES = 4 * 1024 * 1024
+EXPORTS = ("bm_workspace_bytes", "bm_simulate", "bm_simulate_static", "bm_simulate_dt", "bm_state_bytes", "bm_simulate_chunk", "bm_state_histogram",
            "bm_state_moments", "bm_simulate_host", "bm_philox_fill", "bm_gauss_fill", "bm_box_muller_words",
            "bm_kernel_info", "bm_pipe_probe", "bm_status_string", "bm_version")
 STATS_FIELDS = ("n", "mean_v", "var_v", "mean_xT", "var_xT", "mean_jumps", "mean_substeps", "rsv")
@@ -67,6 +68,8 @@ def lib():
         L.bm_workspace_bytes.restype = C.c_size_t
         L.bm_simulate.argtypes = [cfgp, vp, i32, i64, i64, dbl, u64, vp, vp, vp, vp, C.c_size_t, vp]
         L.bm_simulate.restype = C.c_int
+        L.bm_simulate_static.argtypes = [cfgp, vp, i32, i64, i64, dbl, u64, vp, vp, vp, vp]
+        L.bm_simulate_static.restype = C.c_int
         L.bm_simulate_dt.argtypes = [cfgp, vp, vp, i32, i64, i64, u64, vp, vp, vp, C.c_size_t, vp]
         L.bm_simulate_dt.restype = C.c_int
         L.bm_state_bytes.argtypes = [cfgp, i32, i64]
@@ -161,6 +164,28 @@ def bm_simulate(cfg, params, n_points, n_paths, n_steps, dt, seed, out_stats, ou
     if rc != BM_OK:
         raise BmError(rc, "bm_simulate")
     return workspace
+
+
+def bm_simulate_static(cfg, params, n_points, n_paths, n_steps, dt, seed, out_stats, out_paths=None, out_trace=None,
+                       stream=None):
+    """bm_simulate for callers that cannot allocate device memory (a plug-in in someone else's GPU heap, a real-time loop
+    that must not call cudaMalloc): no workspace argument and no allocation of any kind, here or in the library -- the
+    reduction's scratch is a fixed BM_STATIC_SCRATCH_BYTES array inside libbm.so.  Same tensors and results as
+    bm_simulate.  Raises BmError(BM_ERR_WORKSPACE) when the launch would need more than that (over 65 536 thread
+    blocks).  Calls on one device share the array: do not let two of them overlap on the GPU (one stream, or events)."""
+    import torch
+    assert params.is_cuda and params.dtype == torch.float64 and params.is_contiguous() and params.numel() == 16 * n_points
+    assert out_stats.is_cuda and out_stats.dtype == torch.float64 and out_stats.is_contiguous() and out_stats.numel() == 8 * n_points
+    if out_paths is not None:
+        assert out_paths.is_cuda and out_paths.dtype == torch.float64 and out_paths.numel() == n_points * n_paths * BM_OUT_STRIDE
+    if out_trace is not None:
+        assert out_trace.is_cuda and out_trace.dtype == torch.float64 and out_trace.numel() == cfg.trace_paths * cfg.trace_steps * 2
+    op = C.c_void_p(out_paths.data_ptr()) if out_paths is not None else None
+    ot = C.c_void_p(out_trace.data_ptr()) if out_trace is not None else None
+    rc = lib().bm_simulate_static(C.byref(cfg), C.c_void_p(params.data_ptr()), n_points, n_paths, n_steps, float(dt),
+                                  int(seed), C.c_void_p(out_stats.data_ptr()), op, ot, _stream_ptr(stream))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_simulate_static")
 
 
 def bm_simulate_dt(cfg, params, dt_points, n_points, n_paths, n_steps, seed, out_stats, out_paths=None, workspace=None,
