@@ -38,7 +38,10 @@ XU_LANES_PER_SM = 16          # MUFU lanes per SM per clock (4 per SM sub-partit
 # dram__bytes_read.sum + dram__bytes_write.sum of one path-kernel launch from the committed `ncu --set full` captures
 # (profiles/r2_f32_v7.md; C4: its CELLS and LANES launch together): parameters and per-block partials only, the path is
 # register-resident.  Bytes per call.
-NCU_DRAM_BYTES = {("C1", "f32"): 64512, ("C2", "f32"): 53760, ("C3", "f32"): 86272, ("C4", "f32"): 4351488}
+# Each constant is tied to the kernel it was captured from by that kernel's registers per thread (bm_kernel_info): when the
+# kernel bm_simulate launches today no longer has that count, the capture is stale and `traffic` is reported as null.
+NCU_DRAM_BYTES = {("C1", "f32"): (64512, 84), ("C2", "f32"): (53760, 87), ("C3", "f32"): (86272, 87),
+                  ("C4", "f32"): (4351488, 64)}
 
 
 def parse():
@@ -47,7 +50,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C1", choices=["C0", "C1", "C2", "C3", "C4", "M1", "M2"])
+    ap.add_argument("--workload", default="C1", choices=["C0", "C1", "C2", "C3", "C4", "M1", "M2", "A1"])
     ap.add_argument("--prec", default="f32", choices=["f32", "f64"])
     ap.add_argument("--sincos", default="auto", choices=["auto", "sfu", "fma"])
     ap.add_argument("--block-threads", type=int, default=0)
@@ -74,7 +77,7 @@ def workload_of(args):
 
 
 def workload_config(w, args, extra=None):
-    c = {"workload": f"{w.name}: BASELINE.json configs[{w.name[1]}]" if w.name[1:].isdigit() else w.name,
+    c = {"workload": f"{w.name}: BASELINE.json configs[{w.name[1]}]" if (w.name[0] == "C" and w.name[1:].isdigit()) else w.name,
          "n_points": int(w.n_points), "n_paths_per_point": int(w.n_paths), "n_steps": int(w.n_steps),
          "dt": w.dt, "n_discard": int(w.n_discard), "seed": int(w.seed),
          "model": "inertial" if w.model == 1 else "overdamped",
@@ -258,9 +261,22 @@ class Runner:
         return max(e0.elapsed_time(e1), 1e3 * (time.perf_counter() - t0))
 
 
-# FP64-pipe arithmetic instructions (DFMA, DMUL, DADD, DSETP) per sub-step of the fp64 kernels as built, from the executed
-# counts of the committed `ncu --set full` captures (profiles/r2_f64_v2.md): the count the fp64 roofline fraction is formed with.
-FP64_OPS_PER_SUBSTEP = {0: 110.9, 1: 175.7}
+# ALGORITHMIC FP64 operations (add, multiply or fused multiply-add = 1) per sub-step, counted from the formulae of the
+# method at the accuracy the 1e-8 per-path parity needs ("fp64 operation count"), not from the
+# compiled kernel: the count the fp64 roofline fraction `frac` is formed with.
+#   force a(x): cos 2 pi x = 5 (reduction, r^2, r^4) + 11 (degree-12 even polynomial, two chains) + 1 (join) = 17, then
+#               c (k1 + k2 c) + const = 2                                          -> 19, three per sub-step = 57, + 1 for const
+#   one normal = half a Box-Muller pair: (2 x 2 uniforms + 18 ln + 1 + 7 sqrt + 19 sincospi + 1 + 2 products) / 2  = 26
+#   over-damped update lines of Alg. 1 (h/2 once, three lines, amp * g)                                            = 10
+#   inertial: update lines of x and v = 21, ONE new drive cosine per sub-step (the one at t is the previous sub-step's
+#             at t + h): 21 + omega t, t + h, amp * cos = 24
+# Not counted: the jump scheduler's comparisons, the fold, conversions, selects -- whatever the compiler or the chosen
+# code shape adds.  over-damped 57 + 1 + 10 + 26 = 94, inertial 57 + 1 + 21 + 24 + 26 = 129.
+FP64_ALG_OPS_PER_SUBSTEP = {0: 94.0, 1: 129.0}
+# FP64-pipe instructions (DFMA, DMUL, DADD, DSETP) per sub-step EXECUTED by the kernels as built, from the committed
+# `ncu --set full` captures (profiles/r2_f64_v2.md), each with the registers per thread of the kernel it was counted on:
+# reported as `pipe_utilisation` (how busy the FP64 pipe is, whatever it is busy with), null when the kernel has changed.
+FP64_BUILT_OPS_PER_SUBSTEP = {0: (110.9, 120), 1: (175.7, 128)}
 FP64_LANES_PER_SM = 64        # DFMA lanes per SM per clock (bm_pipe_probe: 63)
 
 
@@ -274,12 +290,14 @@ def launches_per_call(B, w, prec_name):
 
 
 def roofline_of(B, w, prec_name, stats, ms_per_step, clocks, info):
-    """Roofline of the path kernel (the grid pass is < 0.1 % of a step).  fp32: bound by the XU (MUFU) pipe, algorithmic
-    operation count; fp64: the FP64 pipe, instruction count of the kernel as built.  Peak = lanes x SMs x the SM clock
-    SAMPLED during the timed region (falls back to the maximum clock when nvidia-smi gave nothing)."""
+    """Roofline of the path kernel (the grid pass is < 0.1 % of a step), in ALGORITHMIC operations of the binding pipe:
+    fp32: MUFU-class operations on the XU pipe; fp64: FP64 operations of the method's formulae (FP64_ALG_OPS_PER_SUBSTEP).
+    Peak = lanes x SMs x the SM clock SAMPLED during the timed region (the maximum clock when nvidia-smi gave nothing).
+    fp64 also carries `pipe_utilisation`: the same fraction formed with the instructions the kernel as built executes."""
     substeps = float(stats[:, 6].mean())                # counted by the kernel
     jumps = float(stats[:, 5].mean())
     sm_mhz = clocks.get("sm_mhz") or clocks.get("sm_max_mhz") or 1965.0
+    extra = {}
     if prec_name == "f32":
         per_path = XU_OPS_PER_SUBSTEP[w.model] * substeps + 2.0 * jumps
         if w.scheme == 1:   # the paper's scheme as printed: no Gaussian transcendental; 3 force cosines only for SINE2
@@ -287,19 +305,33 @@ def roofline_of(B, w, prec_name, stats, ms_per_step, clocks, info):
         lanes, pipe = XU_LANES_PER_SM, "xu (MUFU)"
         what = "algorithmic MUFU-class operations (DESIGN.md section 6)"
     else:
-        per_path = FP64_OPS_PER_SUBSTEP[w.model] * substeps
+        per_path = FP64_ALG_OPS_PER_SUBSTEP[w.model] * substeps
         lanes, pipe = FP64_LANES_PER_SM, "fp64"
-        what = "FP64-pipe instructions of the kernel as built (profiles/r2_f64_v2.md)"
+        what = "algorithmic FP64 operations of the method's formulae (DESIGN.md section 6, fp64 operation count)"
     ops = per_path * w.n_points * w.n_paths
     peak = lanes * info["sm_count"] * sm_mhz * 1e6 / 1e9
     achieved = ops / (ms_per_step * 1e-3) / 1e9
+    if prec_name == "f64":
+        built, regs = FP64_BUILT_OPS_PER_SUBSTEP[w.model]
+        fresh = w.scheme == 0 and info["regs_per_thread"] == regs
+        extra = {"pipe_utilisation": (built * substeps * w.n_points * w.n_paths / (ms_per_step * 1e-3) / 1e9 / peak) if fresh else None,
+                 "pipe_utilisation_source": f"{built} executed FP64-pipe instructions per sub-step (profiles/r2_f64_v2.md, kernel with "
+                                            f"{regs} registers per thread)" + ("" if fresh else "; the kernel launched now differs: stale")}
     return {"bound": "alu", "pipe": pipe, "achieved": achieved, "peak": peak, "unit": "Gop/s", "frac": achieved / peak,
             "ops_per_path_step": per_path / w.n_steps, "ops_counted": what,
             "peak_source": f"derived: {lanes} lanes/SM/clk x {info['sm_count']} SMs x {sm_mhz:.0f} MHz (SM clock sampled "
                            "during the timed region; lane counts confirmed by bm_pipe_probe, profiles/pipes_r2.json)",
             "kernel_ms": ms_per_step, "regs_per_thread": info["regs_per_thread"],
             "launch_threads": info["launch_threads"], "blocks_per_sm": info["blocks_per_sm"],
-            "substeps_per_step": substeps / w.n_steps}
+            "substeps_per_step": substeps / w.n_steps, **extra}
+
+
+def traffic_of(w, prec_name, info, scale_steps=1.0):
+    """dram bytes of one launch from the committed ncu capture, or None when that capture is of another kernel."""
+    rec = NCU_DRAM_BYTES.get((w.name, prec_name))
+    if rec is None or scale_steps != 1.0 or info["regs_per_thread"] != rec[1]:
+        return None
+    return rec[0]
 
 
 def measure(B, torch, w, prec_name, args, seed, dev, stream, flush, steps, warmup, barrier, sampler_index, sincos=0, gauss=0,
@@ -332,7 +364,10 @@ def measure(B, torch, w, prec_name, args, seed, dev, stream, flush, steps, warmu
     return run, ms, clocks, run.stats.cpu().numpy().copy()
 
 
-PER_CONFIG = (("C0", "f32"), ("C2", "f32"), ("C3", "f32"), ("C4", "f32"), ("C1", "f64"), ("C2", "f64"))
+# every kernel family the library ships, timed in the default run: the five BASELINE.json configs in fp32, C1 / C2 in
+# fp64, the paper's own programs (scheme as printed) and the adaptive scheme (row f4) on C1's physics
+PER_CONFIG = (("C0", "f32"), ("C2", "f32"), ("C3", "f32"), ("C4", "f32"), ("C1", "f64"), ("C2", "f64"), ("M1", "f32"),
+              ("M2", "f32"), ("A1", "f64"))
 
 
 def run_ours(args):
@@ -403,9 +438,10 @@ def run_ours(args):
         probe_ms.append(e0.elapsed_time(e1))
     roof["peak_probe"] = info["sm_count"] * 4 * 256 * 1000 * 64 / (min(probe_ms) * 1e-3) / 1e9
     roof["frac_of_probe"] = roof["achieved"] / roof["peak_probe"]
-    roof["traffic"] = NCU_DRAM_BYTES.get((w.name, args.prec)) if args.scale_steps == 1.0 else None
+    roof["traffic"] = traffic_of(w, args.prec, info, args.scale_steps)
     roof["traffic_source"] = ("a constant from the committed ncu --set full capture of this kernel (profiles/, dram bytes of "
-                              "one launch: parameters and per-block partials; independent of n_steps), not read in this run")
+                              "one launch: parameters and per-block partials; independent of n_steps), not read in this run; null when "
+                              "the kernel launched now has another register count than the captured one")
     roof["kernel"] = "bm_paths_literal" if w.scheme == 1 else ("bm_paths_f32" if args.prec == "f32" else "bm_paths_f64")
     roof["gauss"] = {1: "w32", 2: "w16", 3: "w16p"}.get(info["gauss"], "n/a")
     jumps = float(stats[:, 5].mean())
@@ -419,9 +455,18 @@ def run_ours(args):
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_call(B, w, args.prec) * args.steps, "roofline": roof,
             "result": {"mean_v": float(stats[0, 1]), "var_v": float(stats[0, 2]), "mean_jumps": jumps}}
 
-    # every BASELINE.json config and both precisions beside the headline (3 warm-up + 3 timed full-size steps each)
+    # every BASELINE.json config, both precisions and every other kernel family beside the headline (3 warm-up + 3 timed
+    # full-size steps each), compactly INSIDE the roofline object
     if world == 1 and not args.no_per_config and args.scale_steps == 1.0 and args.workload == "C1" and args.prec == "f32":
-        per = {}
+        def compact(name, pn, wc, mps, best, rf, ck):
+            meaningful = not (pn == "f32" and wc.scheme == 1 and wc.potential != 0)   # PWL as printed: no MUFU in the step
+            return {"ms": round(mps, 4), "ms_best": round(best, 4), "value": wc.path_steps / (mps * 1e-3),
+                    "frac": round(rf["frac"], 4) if meaningful else None,
+                    "pipe_utilisation": (round(rf["pipe_utilisation"], 4) if rf.get("pipe_utilisation") else None) if pn == "f64" else None,
+                    "ops_per_path_step": round(rf["ops_per_path_step"], 4), "substeps_per_step": round(rf["substeps_per_step"], 5),
+                    "regs": rf["regs_per_thread"], "threads": rf["launch_threads"],
+                    "sm_mhz": ck.get("sm_mhz"), "reasons": ck.get("reasons", [])}
+        per = {"C1_f32": compact("C1", "f32", w, ms_per_step, float(min(ms)), roof, clocks)}
         launches = 0
         for name, pn in PER_CONFIG:
             wc = W.CONFIGS[name]()
@@ -429,19 +474,13 @@ def run_ours(args):
             i2 = B.bm_kernel_info(r2.cfg, wc.n_points, wc.n_paths)
             mps = float(np.mean(ms2))
             rf = roofline_of(B, wc, pn, st2, mps, ck2, i2)
-            per[f"{name}_{pn}"] = {"workload": name, "dtype": pn, "n_points": int(wc.n_points), "n_paths_per_point": int(wc.n_paths),
-                                   "n_steps": int(wc.n_steps), "steps": 3, "warmup": 3, "ms_per_step": mps,
-                                   "ms_best": float(min(ms2)), "value": wc.path_steps / (mps * 1e-3), "unit": UNIT,
-                                   "roofline": {k: rf[k] for k in ("pipe", "achieved", "peak", "unit", "frac", "ops_per_path_step",
-                                                                   "regs_per_thread", "launch_threads", "blocks_per_sm",
-                                                                   "substeps_per_step")},
-                                   "clocks": ck2, "mean_v_point0": float(st2[0, 1])}
+            per[f"{name}_{pn}"] = compact(name, pn, wc, mps, float(min(ms2)), rf, ck2)
             launches += launches_per_call(B, wc, pn) * 3
             del r2
-        line["per_config"] = per
+        roof["per_config"] = per
         line["gpu_launches"] += launches
-        line["fp64"] = {"value": per["C1_f64"]["value"], "unit": UNIT, "ms_per_step": per["C1_f64"]["ms_per_step"],
-                        "frac_fp64_pipe": per["C1_f64"]["roofline"]["frac"]}
+        line["fp64"] = {"value": per["C1_f64"]["value"], "unit": UNIT, "ms_per_step": per["C1_f64"]["ms"],
+                        "frac": per["C1_f64"]["frac"], "pipe_utilisation": per["C1_f64"]["pipe_utilisation"]}
     elif world == 1 and not args.no_fp64 and args.prec == "f32":
         r64 = Runner(B, torch, w, B.BM_F64, sc, args.block_threads, seed, dev, stream)
         r64.device_step()

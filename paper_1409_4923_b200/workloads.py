@@ -124,4 +124,12 @@ def m2():
                     40_000, min(1 / mu_a, 1 / mu_b) / 200, 4_000, potential=POT_PWL, scheme=SCHEME_PAPER_LITERAL)
 
 
-CONFIGS = {"C0": c0, "C1": c1, "C2": c2, "C3": c3, "C4": c4, "M1": m1, "M2": m2}
+def a1():
+    """Dynamic step size control from chi on C1's physics: 65536 paths x 2e4 grid
+    steps of 1e-3, each halved up to 4 times where |chi| exceeds 1e-5.  A bench case (fp64 only), not a BASELINE config."""
+    w = c1()
+    return Workload("A1", OVERDAMPED, w.params, w.n_paths, 20_000, w.dt, 2_000, scheme=SCHEME_ADAPTIVE,
+                    extra=dict(adapt_tol=1e-5, adapt_levels=4))
+
+
+CONFIGS = {"C0": c0, "C1": c1, "C2": c2, "C3": c3, "C4": c4, "M1": m1, "M2": m2, "A1": a1}
