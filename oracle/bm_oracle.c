@@ -177,6 +177,12 @@ static double unfolded(const pos_t *s, double L) { return (double)s->wraps * L +
 
 /* R4  initial condition from init-stream call 0: x0 = L w0 2^-32 (or x0_fixed), v0 = v0_lo + (v0_hi-v0_lo) u(w1),
  *     d = 1 (state +Fb) iff u(w2) < mu_a/(mu_a+mu_b)  (stationary law of eq. 14). */
+/* Rate of leaving the dichotomous state d (eq. 14).  A non-positive mu_b means that +Fb is never left (the reading
+ * include/bm.h states for bm_params.mu_b and DESIGN.md section 1 repeats: "mu_b = 0 with mu_a > 0 makes +F_b absorbing"):
+ * the rate is taken as 0, so the sojourn -ln(u)/0 is +infinity and the stationary weight of +Fb is 1 -- never a negative
+ * waiting time. */
+static double mu_leave(const orc_params *p, int d) { return d ? (p->mu_b > 0.0 ? p->mu_b : 0.0) : p->mu_a; }
+
 static void init_path(const orc_config *cfg, const orc_params *p, uint64_t seed, uint64_t g, double L, pos_t *s,
                       int *d) {
   uint32_t w[4];
@@ -186,10 +192,8 @@ static void init_path(const orc_config *cfg, const orc_params *p, uint64_t seed,
   s->wraps = 0;
   s->v = (cfg->model == ORC_INERTIAL) ? p->v0_lo + (p->v0_hi - p->v0_lo) * orc_u01(w[1]) : 0.0;
   fold(s, L);
-  *d = (p->mu_a > 0.0) ? (orc_u01(w[2]) < p->mu_a / (p->mu_a + p->mu_b) ? 1 : 0) : -1;
+  *d = (p->mu_a > 0.0) ? (orc_u01(w[2]) < p->mu_a / (p->mu_a + mu_leave(p, 1)) ? 1 : 0) : -1;
 }
-
-static double mu_leave(const orc_params *p, int d) { return d ? p->mu_b : p->mu_a; }
 
 /* ------------------------------------------------------------------------------------------------
  * R5  Jump-adapted time loop ("variable time steps which must be adapted to each sequence

@@ -26,7 +26,8 @@ __global__ void __launch_bounds__(256) bm_paths_adaptive_f64(const __grid_consta
     PointF64 P;
     P.A1 = bp.A1; P.A2 = bp.A2; P.D = HAS_G ? bp.D : 0.0;
     P.lambda = HAS_P ? bp.lambda : 0.0; P.zeta = HAS_P ? bp.zeta : 0.0;
-    P.Fa = bp.Fa; P.Fb = bp.Fb; P.mu_a = bp.mu_a; P.mu_b = bp.mu_b;
+    P.Fa = bp.Fa; P.Fb = bp.Fb; P.mu_a = bp.mu_a;
+    P.mu_b = bp.mu_b > 0.0 ? bp.mu_b : 0.0;  // mu_b <= 0: +Fb is absorbing (bm.h: bm_params)
     P.gamma = 0.0; P.amp = 0.0; P.omega = 0.0;
     P.c0 = bp.F - P.lambda * P.zeta;
     const double dt = step_length(a, point);

@@ -440,7 +440,7 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
   if (INERTIAL)
     v = (float)((double)S * (bp.v0_lo + (bp.v0_hi - bp.v0_lo) * (((double)wi.y + 0.5) * (1.0 / 4294967296.0))));
   int d = 0;
-  if (onD) d = ((((double)wi.z + 0.5) * (1.0 / 4294967296.0)) < bp.mu_a / (bp.mu_a + bp.mu_b)) ? 1 : 0;
+  if (onD) d = ((((double)wi.z + 0.5) * (1.0 / 4294967296.0)) < bp.mu_a / (bp.mu_a + (bp.mu_b > 0.0 ? bp.mu_b : 0.0))) ? 1 : 0;  // mu_b <= 0: +Fb absorbing, every path starts there
 
   // Standard normal of the sub-step that ends on an event, from the third word of the event's Philox call (R13):
   // radius from its top 23 bits, angle from its low 16 (the W16 assignment).

@@ -281,7 +281,8 @@ __global__ void __launch_bounds__(256, 2) bm_paths_f64(const __grid_constant__ S
   PointF64 P;
   P.A1 = bp.A1; P.A2 = bp.A2; P.D = HAS_G ? bp.D : 0.0;
   P.lambda = HAS_P ? bp.lambda : 0.0; P.zeta = HAS_P ? bp.zeta : 0.0;
-  P.Fa = bp.Fa; P.Fb = bp.Fb; P.mu_a = bp.mu_a; P.mu_b = bp.mu_b;
+  P.Fa = bp.Fa; P.Fb = bp.Fb; P.mu_a = bp.mu_a;
+  P.mu_b = bp.mu_b > 0.0 ? bp.mu_b : 0.0;  // mu_b <= 0: +Fb is absorbing (bm.h: bm_params) -- an infinite sojourn, never a negative one
   P.gamma = bp.gamma; P.amp = bp.amp; P.omega = bp.omega;
   P.c0 = bp.F - P.lambda * P.zeta;  // constant part of the drift a(x), all three stages (R6)
   const double dt = step_length(a, point);

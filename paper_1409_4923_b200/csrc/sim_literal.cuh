@@ -99,7 +99,7 @@ __global__ void __launch_bounds__(256) bm_paths_literal(const __grid_constant__ 
     // a non-positive rate of leaving -Fa switches the dichotomous source off at this point (as the oracle); a
     // non-positive rate of leaving +Fb makes that state absorbing (infinite sojourn)
     const bool onD = HAS_D && bp.mu_a > 0.0;
-    int d = onD ? ((u01_f64(wi.z) < bp.mu_a / (bp.mu_a + bp.mu_b)) ? 1 : 0) : 0;
+    int d = onD ? ((u01_f64(wi.z) < bp.mu_a / (bp.mu_a + (bp.mu_b > 0.0 ? bp.mu_b : 0.0))) ? 1 : 0) : 0;
 
     // countdowns in grid steps (integers: exact in both precisions)
     Count sP = 0, sD = 0;

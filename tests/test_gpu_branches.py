@@ -138,6 +138,30 @@ def test_sweep_points_with_zero_dichotomous_rates(B, orc):
         assert np.median(np.abs(p32[quiet, B.BM_OUT_XT] - ref[quiet, orc.OUT_XT])) < 2e-4
 
 
+def test_negative_rate_of_leaving_fb_is_the_absorbing_state_in_every_kernel(B, orc):
+    """bm.h: "mu_b <= 0 with mu_a > 0 makes +Fb absorbing".  bm_simulate does not check parameter values (device
+    pointer), so a negative mu_b reaches the kernels: it must behave as mu_b = 0 bit for bit -- an infinite sojourn, not a
+    negative waiting time -- in the fp64, fp32, paper-literal and adaptive kernels, and as the oracle."""
+    def table(mu_b):
+        return W.params_table(2, A1=1.0, A2=0.25, D=0.02, Fa=0.6, Fb=0.9, mu_a=np.array([2.0, 40.0]), mu_b=mu_b)
+    cases = [(W.SCHEME_JUMP_ADAPTED, B.BM_F64, {}), (W.SCHEME_JUMP_ADAPTED, B.BM_F32, {}),
+             (W.SCHEME_PAPER_LITERAL, B.BM_F64, {}), (W.SCHEME_PAPER_LITERAL, B.BM_F32, {}),
+             (W.SCHEME_ADAPTIVE, B.BM_F64, dict(adapt_tol=1e-5, adapt_levels=3))]
+    for scheme, prec, extra in cases:
+        def run(mu_b):
+            w = W.Workload("mub", W.OVERDAMPED, table(mu_b), 200, 800, 2e-3, 0, scheme=scheme, extra=dict(extra))
+            return w, B.run_workload(w, prec, want_paths=True)
+        w0, (s0, p0, _) = run(0.0)
+        _, (sn, pn, _) = run(np.array([-3.0, -0.5]))
+        assert np.array_equal(p0.view(np.uint64), pn.view(np.uint64)), (scheme, prec)
+        assert np.array_equal(s0.view(np.uint64), sn.view(np.uint64)), (scheme, prec)
+        assert np.all(p0[:, B.BM_OUT_JUMPS] == 0) and np.all(p0[:, B.BM_OUT_SUBSTEPS] >= 800)
+        if prec == B.BM_F64:
+            ref, _ = orc.simulate(table(np.array([-3.0, -0.5])), 200, 800, 2e-3, w0.seed, scheme=scheme, **extra)
+            assert np.abs(p0[:, B.BM_OUT_XT] - ref[:, orc.OUT_XT]).max() < 1e-9
+            assert np.array_equal(p0[:, B.BM_OUT_SUBSTEPS], ref[:, orc.OUT_SUBSTEPS])
+
+
 @pytest.mark.parametrize("prec", ["f32", "f64"])
 def test_chunked_ragged_ensemble_of_several_waves(B, prec):
     """Row f2 at a size where the grid does not fit on the device at once and the last warp is ragged: the lanes past

@@ -127,3 +127,26 @@ def test_literal_model_II_reproduces_paper_validation(orc):
     v = out[:, orc.OUT_VBAR]
     se = v.std(ddof=1) / math.sqrt(v.size)
     assert abs(v.mean() - 2 * J_model_II(Fa, Fb, tau)) < 4 * se + 0.01, (v.mean(), 2 * J_model_II(Fa, Fb, tau), se)
+
+
+def test_absorbing_dichotomous_state_closed_form_and_negative_rate(orc):
+    """include/bm.h (bm_params.mu_b): a non-positive rate of leaving +Fb makes that state absorbing.  With mu_a > 0 the
+    stationary weight of +Fb is then 1: every path starts there and never flips, so without Gaussian noise the path in
+    the harmonic potential is the ODE x' = -A1 x + Fb with x(t) = Fb/A1 + (x0 - Fb/A1) e^{-A1 t} (the weak order 2.0
+    scheme is the second-order Heun-type ODE scheme there).  A NEGATIVE mu_b must not give negative waiting times: it
+    is the same absorbing state, bit for bit -- in all three schemes."""
+    A1, Fb, x0, T, n = 1.7, 0.9, -0.4, 2.0, 400
+    def table(mu_b):
+        return W.params_table(1, A1=A1, D=0.0, Fa=0.6, Fb=Fb, mu_a=2.0, mu_b=mu_b, x0_fixed=x0 + 10.0)
+    exact = Fb / A1 + (x0 + 10.0 - Fb / A1) * math.exp(-A1 * T)
+    # (the scheme as printed keeps the constant forces out of the predictor lines: first order in dt for this ODE)
+    for scheme, tol, kw in ((W.SCHEME_JUMP_ADAPTED, 2e-5, {}), (W.SCHEME_PAPER_LITERAL, 5e-3, {}),
+                            (W.SCHEME_ADAPTIVE, 2e-5, dict(adapt_tol=1e-6, adapt_levels=3))):
+        zero, _ = orc.simulate(table(0.0), 8, n, T / n, SEED, potential=W.POT_QUAD, scheme=scheme, **kw)
+        neg, _ = orc.simulate(table(-3.0), 8, n, T / n, SEED, potential=W.POT_QUAD, scheme=scheme, **kw)
+        assert np.array_equal(zero, neg)
+        assert np.all(zero[:, orc.OUT_JUMPS] == 0)
+        assert np.abs(zero[:, orc.OUT_XT] - exact).max() < tol * abs(exact), (scheme, zero[0, orc.OUT_XT], exact)
+    # and the other way round the state is left: mu_b > 0 flips
+    both, _ = orc.simulate(table(5.0), 64, n, T / n, SEED, potential=W.POT_QUAD)
+    assert both[:, orc.OUT_JUMPS].mean() > 2
