@@ -127,12 +127,12 @@ typedef struct {
                             (1: the measured-faster form); 1; 2
                             (BM_POT_SINE2 only, else BM_ERR_UNSUPPORTED).  A path's result does not depend on it; it
                             enters the determinism contract through the reduction tree of out_stats only.  Must be 0
-                            for BM_F32 and the paper-literal scheme. */
+                            for BM_F32, the paper-literal and the adaptive scheme (else BM_ERR_UNSUPPORTED). */
   int32_t adapt_levels; /* BM_SCHEME_ADAPTIVE: how often dt may be halved, 0..20 */
   double adapt_tol;    /* BM_SCHEME_ADAPTIVE: tolerance on |chi| (in units of x), >= 0; +inf = never refine */
   int32_t event_mode;  /* bm_event_mode; must be AUTO unless BM_F32, BM_OVERDAMPED, JUMP_ADAPTED with a jump source in
                           `noise` (else BM_ERR_UNSUPPORTED) */
-  int32_t rsv;         /* 0 */
+  int32_t rsv;         /* must be 0 (else BM_ERR_INVALID_ARG) */
 } bm_config;
 
 /* per-path record written to out_paths: 6 doubles */
@@ -152,7 +152,8 @@ BM_API size_t bm_workspace_bytes(const bm_config *cfg, int32_t n_points, int64_t
  *   workspace  device scratch of >= bm_workspace_bytes(...) bytes, 16-byte aligned
  * Kernels launched on `stream`: the path kernel (a1-a10 of DESIGN.md section 2) and the grid pass of the
  * reduction (a11).  n_steps <= 2^31 - 16 for BM_F32 (32-bit cell counters), <= 2^33 for BM_F64 (the Gaussian stream is
- * indexed by a 32-bit counter word).  Parameter VALUES are not checked here (params is a device pointer; see
+ * indexed by a 32-bit counter word that advances once per four sub-steps: grid steps + events must stay below 2^34);
+ * BM_SCHEME_ADAPTIVE: n_steps * 2^adapt_levels <= 2^33 (every grid step may be refined to the last level).  Parameter VALUES are not checked here (params is a device pointer; see
  * bm_simulate_host).  Errors: BM_ERR_INVALID_ARG as listed above; BM_ERR_UNSUPPORTED for
  * PAPER_LITERAL with BM_INERTIAL, BM_INERTIAL with a potential other than SINE2, out_trace with BM_F32;
  * BM_ERR_WORKSPACE; BM_ERR_CUDA.

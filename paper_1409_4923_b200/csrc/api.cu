@@ -37,6 +37,7 @@ bool valid_cfg(const bm_config *c) {
   if (c->block_threads > 256 && !(c->prec == BM_F32 && c->model == BM_OVERDAMPED && c->scheme == BM_SCHEME_JUMP_ADAPTED)) return false;
   if (c->gauss < BM_GAUSS_AUTO || c->gauss > BM_GAUSS_W16P) return false;
   if (c->paths_per_thread < 0 || c->paths_per_thread > 2) return false;
+  if (c->rsv != 0) return false;  // bm.h: reserved, must be 0
   if (c->n_discard < 0 || c->trace_steps < 0 || c->trace_paths < 0) return false;
   if (c->event_mode < BM_EVENTS_AUTO || c->event_mode > BM_EVENTS_LANES) return false;
   return true;
@@ -122,6 +123,8 @@ bm_status pick_kernel(const bm_config *c, int32_t n_points, int64_t n_paths, Lau
   if (c->scheme == BM_SCHEME_ADAPTIVE && (c->model != BM_OVERDAMPED || c->prec != BM_F64 || chunked)) return BM_ERR_UNSUPPORTED;
   if (c->model == BM_INERTIAL && c->potential != BM_POT_SINE2) return BM_ERR_UNSUPPORTED;
   if (c->paths_per_thread == 2 && !has_two_paths(c)) return BM_ERR_UNSUPPORTED;
+  // bm.h: a knob of the BM_F64 jump-adapted kernels only; it must be 0 everywhere else
+  if (c->paths_per_thread != 0 && !(c->prec == BM_F64 && c->scheme == BM_SCHEME_JUMP_ADAPTED)) return BM_ERR_UNSUPPORTED;
   if (c->event_mode != BM_EVENTS_AUTO && !has_event_modes(c)) return BM_ERR_UNSUPPORTED;
   L->threads = block_threads_of(c, n_points, n_paths);
   L->ppt = paths_per_thread_of(c, n_points, n_paths);
@@ -247,6 +250,8 @@ static bm_status simulate_range(const bm_config *cfg, const bm_params *params, i
   // by (sub-step count)/4 in a 32-bit counter word (sub-steps = grid steps + events < 2^34)
   const bool narrow = cfg->prec == BM_F32;
   if (n_steps > (narrow ? 0x7FFFFFF0LL : (1LL << 33))) return BM_ERR_INVALID_ARG;
+  // the adaptive scheme may take 2^adapt_levels sub-steps per grid step: the same counter bounds the refined count
+  if (cfg->scheme == BM_SCHEME_ADAPTIVE && n_steps > ((1LL << 33) >> cfg->adapt_levels)) return BM_ERR_INVALID_ARG;
   if (out_trace && (cfg->trace_steps <= 0 || cfg->trace_paths <= 0)) return BM_ERR_INVALID_ARG;
   if (out_trace && cfg->prec != BM_F64) return BM_ERR_UNSUPPORTED;
   Launch L;

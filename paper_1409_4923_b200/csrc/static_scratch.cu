@@ -24,12 +24,6 @@ namespace {
 // cudaGetSymbolAddress, once per device, with that device current (every device has its own copy of the array).
 static __device__ __align__(256) unsigned char static_scratch[BM_STATIC_SCRATCH_BYTES];
 
-// Device code may name the array directly.  This kernel is never launched; it pins the array into the device image (an
-// array that no device code refers to could be dropped from it, and the look-up below would then fail).
-__global__ void static_scratch_anchor(unsigned char *out) {
-  if (out) *out = static_scratch[0];
-}
-
 constexpr int MAX_DEVICES = 64;
 
 // Device address of the array on the CURRENT device; nullptr (with *err set) if the runtime cannot give it.  The table
@@ -55,6 +49,13 @@ void *static_scratch_on_current_device(cudaError_t *err) {
 }
 
 }  // namespace
+
+// Device code may name the array directly.  This kernel is never launched; it pins the array into the device image (an
+// array that no device code refers to could be dropped from it, and the look-up above would then fail).  Not exported
+// (the library is built with hidden visibility).
+__global__ void bm_static_scratch_anchor(unsigned char *out) {
+  if (out) *out = static_scratch[0];
+}
 
 extern "C" {
 

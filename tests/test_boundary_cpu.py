@@ -111,6 +111,29 @@ def test_step_count_limits(B):
         assert L.bm_simulate(C.byref(cfg), p.ctypes.data, 1, 32, limit, 1e-3, 1, st.ctypes.data, None, None, None, 0, None) == B.BM_ERR_WORKSPACE
 
 
+def test_adaptive_step_count_limit_and_reserved_fields(B):
+    """The adaptive scheme can take 2^adapt_levels sub-steps per grid step, all indexed by the same 32-bit counter word
+    (bm.h, bm_simulate): n_steps * 2^adapt_levels <= 2^33.  paths_per_thread outside the fp64 jump-adapted kernels is
+    BM_ERR_UNSUPPORTED and a non-zero rsv BM_ERR_INVALID_ARG, as bm.h says."""
+    L = B.lib()
+    p = np.zeros((1, 16)); st = np.zeros((1, 8))
+
+    def rc(cfg, n_steps):
+        return L.bm_simulate(C.byref(cfg), p.ctypes.data, 1, 32, n_steps, 1e-3, 1, st.ctypes.data, None, None, None, 0, None)
+    for levels in (0, 7, 20):
+        cfg = B.make_config(prec=B.BM_F64, scheme=B.BM_SCHEME_ADAPTIVE, adapt_tol=1e-5, adapt_levels=levels)
+        limit = (1 << 33) >> levels
+        assert rc(cfg, limit + 1) == B.BM_ERR_INVALID_ARG
+        assert rc(cfg, limit) == B.BM_ERR_WORKSPACE            # past the argument checks
+    for kw in (dict(prec=B.BM_F32, paths_per_thread=1), dict(prec=B.BM_F64, scheme=B.BM_SCHEME_PAPER_LITERAL, paths_per_thread=1),
+               dict(prec=B.BM_F64, scheme=B.BM_SCHEME_ADAPTIVE, paths_per_thread=2)):
+        assert rc(B.make_config(**kw), 10) == B.BM_ERR_UNSUPPORTED, kw
+    assert rc(B.make_config(prec=B.BM_F64, paths_per_thread=1), 10) == B.BM_ERR_WORKSPACE
+    cfg = B.make_config(); cfg.rsv = 1
+    assert rc(cfg, 10) == B.BM_ERR_INVALID_ARG
+    assert B.bm_workspace_bytes(cfg, 1, 32) == 0
+
+
 def test_no_cpu_fallback_without_a_device(B):
     import torch
     if torch.cuda.is_available():
