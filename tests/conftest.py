@@ -23,6 +23,17 @@ def orc():
 
 
 @pytest.fixture(scope="session")
+def c1_full_oracle(orc):
+    """The oracle's per-path records of the WHOLE of C1 (65 536 paths x 1e5 steps; under a minute on 16 host cores),
+    computed once per session: the fp64 per-path test and the fp32 full-size test both compare against all of it."""
+    from paper_1409_4923_b200 import workloads as W
+    w = W.c1()
+    ref, _ = orc.simulate(w.params, w.n_paths, w.n_steps, w.dt, w.seed, model=w.model, potential=w.potential,
+                          scheme=w.scheme, n_discard=w.n_discard)
+    return ref
+
+
+@pytest.fixture(scope="session")
 def aten_philox(tmp_path_factory):
     """PyTorch's own at::philox_engine compiled into a tiny shared object: an independent library routine."""
     import ctypes as C

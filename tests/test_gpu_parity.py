@@ -24,7 +24,7 @@ def B():
     return binding
 
 
-from parity_util import assert_3se, assert_counts_close, ill_conditioned, oracle_run  # noqa: E402
+from parity_util import assert_3se, assert_counts_close, assert_few_ill_conditioned, ill_conditioned, oracle_run  # noqa: E402
 
 
 # ---- a3: Philox words -------------------------------------------------------------------------------------
@@ -115,13 +115,15 @@ def test_gauss_f32_w16_is_standard_normal(B, orc, gauss):
 
 # ---- fp64 per-path parity, overdamped ---------------------------------------------------------------------
 
-def check_fp64_overdamped(B, orc, w, ids=None, what=""):
+def check_fp64_overdamped(B, orc, w, ids=None, what="", ref=None):
     """fp64 per-path criterion |dx| <= 1e-8 (1 + |x|) with equal event and sub-step counts.  Paths beyond the bound are
     put through the A17 check (a second and third oracle run with x0 moved by +-1 ulp): only those whose
-    ORACLE result itself moves by more than 1e-9 (1 + |x|) are ill-conditioned and excluded; their number is printed.
+    ORACLE result itself moves by more than 1e-9 (1 + |x|) are ill-conditioned and excluded; their number is bounded
+    (assert_few_ill_conditioned).  ref: the oracle's records for these paths, if the caller has them already.
     Returns (stats, paths, ref, bad = ids beyond the bound that are NOT ill-conditioned, dx)."""
     stats, paths, _ = B.run_workload(w, B.BM_F64, want_paths=True)
-    ref, _ = oracle_run(orc, w, ids=ids)
+    if ref is None:
+        ref, _ = oracle_run(orc, w, ids=ids)
     got = paths if ids is None else paths[ids]
     assert np.array_equal(got[:, B.BM_OUT_JUMPS], ref[:, orc.OUT_JUMPS]), what + ": event counts differ"
     assert np.array_equal(got[:, B.BM_OUT_SUBSTEPS], ref[:, orc.OUT_SUBSTEPS]), what + ": sub-step counts differ"
@@ -132,7 +134,7 @@ def check_fp64_overdamped(B, orc, w, ids=None, what=""):
     if over.size:
         gids = over if ids is None else np.asarray(ids)[over]
         ill = ill_conditioned(orc, w, gids)
-        print(f"{what}: {over.size} paths beyond 1e-8(1+|x|), {int(ill.sum())} of them ill-conditioned (A17), excluded")
+        assert_few_ill_conditioned(int(ill.sum()), got.shape[0], what)
         bad = over[~ill]
     return stats, paths, ref, bad, dx
 
@@ -157,11 +159,11 @@ def test_c1_fp64_scaled_full_compare(B, orc):
     assert abs(stats[0, 5] - o["mean_jumps"]) < 1e-12 and abs(stats[0, 6] - o["mean_substeps"]) < 1e-9
 
 
-def test_c1_fp64_full_size_all_paths(B, orc):
+def test_c1_fp64_full_size_all_paths(B, orc, c1_full_oracle):
     """Full C1 (65536 paths x 1e5 steps) on the GPU and in the oracle, every path compared; ensemble statistics of the
     on-device reduction against the oracle's two-pass reduction within 1e-9 relative."""
     w = W.c1()
-    stats, paths, ref, bad, dx = check_fp64_overdamped(B, orc, w, what="C1 full")
+    stats, paths, ref, bad, dx = check_fp64_overdamped(B, orc, w, what="C1 full", ref=c1_full_oracle)
     assert bad.size == 0, f"C1 full: {bad.size} well-conditioned paths beyond tolerance (max {dx[bad].max():.3e})"
     o = orc.reduce(ref)
     assert stats[0, 0] == w.n_paths
@@ -337,8 +339,8 @@ def test_literal_scheme_fp64_matches_oracle_per_path(B, orc, name):
     bad = np.nonzero(dx > 1e-8 * (1 + np.abs(ref[:, orc.OUT_XT])))[0]
     if bad.size:    # piece-wise linear force: a rounding difference at a kink flips a stage force (A17 check decides)
         ill = ill_conditioned(orc, w, bad, ulps=(1, -1, 2, -2))
-        print(f"literal {name}: {bad.size} paths beyond tolerance, {int(ill.sum())} ill-conditioned, excluded")
         assert ill.all(), f"{int((~ill).sum())} well-conditioned paths beyond tolerance, max {dx[bad[~ill]].max():.3e}"
+        assert_few_ill_conditioned(int(ill.sum()), dx.size, f"literal {name}")
     good = np.setdiff1d(np.arange(dx.size), bad)
     assert np.abs(paths[good, B.BM_OUT_VBAR] - ref[good, orc.OUT_VBAR]).max() < 1e-8
     if bad.size == 0:
@@ -457,6 +459,7 @@ def test_per_point_dt_sweep_matches_oracle_and_fig3a(B, orc):
                             scheme=W.SCHEME_PAPER_LITERAL)
             ill = ill_conditioned(orc, wp, ids[over], ulps=(1, -1, 2, -2))
             assert ill.all(), f"point {pt}: {int((~ill).sum())} well-conditioned paths beyond tolerance, max {dx.max():.3e}"
+            assert_few_ill_conditioned(int(ill.sum()), n_paths, f"per-point dt, point {pt}")
         v_th = 2 * J_model_I(a, float(DPs[pt]))
         se = math.sqrt(s64[pt, 2] / n_paths)
         assert abs(s64[pt, 1] - v_th) < 4 * se + 0.01, (pt, s64[pt, 1], v_th)
