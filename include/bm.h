@@ -17,7 +17,10 @@
  *   - Every call returns a bm_status; nothing throws.  There is no CPU fallback of any kind: without a
  *     CUDA device the compute calls return BM_ERR_CUDA.
  *   - Determinism: identical arguments give bit-identical outputs, independent of stream or of earlier
- *     calls.  Path g = point*n_paths + p sees the same random words whatever the grid shape is.
+ *     calls.  Path g = point*n_paths + p sees the same random words whatever the grid shape is.  The default block
+ *     size and the register class of the fp32 kernel (which fix the reduction tree of out_stats) are functions of the
+ *     arguments only, computed for the 148 SMs of the B200 the library is built for -- on a device with another SM
+ *     count the statistics are still the same bits, the choice is just no longer the tuned one.
  */
 #ifndef BM_H
 #define BM_H
@@ -94,7 +97,9 @@ typedef struct {
   double Fa, Fb;            /* dichotomous values -Fa, +Fb (eq. 13), both > 0 */
   double mu_a, mu_b;        /* rate of leaving -Fa, rate of leaving +Fb (eq. 14).  mu_a <= 0 switches the source off at
                                this point (Gamma = 0); mu_b <= 0 with mu_a > 0 makes +Fb absorbing */
-  double gamma, amp, omega; /* inertial: friction, drive amplitude, drive angular frequency */
+  double gamma, amp, omega; /* inertial: friction, drive amplitude, drive angular frequency.  BM_F64: the drive cosine is
+                               the kernel's own, accurate for |omega * t_final| < 2^20 (1.3e4 at the end of C3); beyond
+                               that its argument reduction loses bits (not checked) */
   double x0_fixed;          /* >= 0: x0 = x0_fixed; < 0: x0 ~ U[0,L) */
   double v0_lo, v0_hi;      /* inertial: v0 ~ U[v0_lo, v0_hi] */
 } bm_params;
@@ -125,7 +130,9 @@ typedef struct {
   int64_t trace_paths; /* ... of global paths 0..trace_paths-1 (BM_F64 only) */
   int32_t paths_per_thread; /* BM_F64 jump-adapted kernels: realizations carried by one thread.  0 = library default
                             (1: the measured-faster form); 1; 2
-                            (BM_POT_SINE2 only, else BM_ERR_UNSUPPORTED).  A path's result does not depend on it; it
+                            (BM_POT_SINE2 only, else BM_ERR_UNSUPPORTED; two independent chains per thread measured
+                            slower at the BASELINE ensemble sizes and ships for ensembles below one warp per scheduler,
+                            where it is the only way to fill the FP64 pipe).  A path's result does not depend on it; it
                             enters the determinism contract through the reduction tree of out_stats only.  Must be 0
                             for BM_F32, the paper-literal and the adaptive scheme (else BM_ERR_UNSUPPORTED). */
   int32_t adapt_levels; /* BM_SCHEME_ADAPTIVE: how often dt may be halved, 0..20 */
@@ -229,7 +236,9 @@ BM_API bm_status bm_state_moments(const bm_config *cfg, int32_t n_points, int64_
  * HOST-pointer convenience entry (the end-to-end path): params, out_stats and out_paths (optional) are HOST
  * buffers.  Takes device scratch from a private stream-ordered pool (one per device, kept between calls: an
  * allocation cache with no influence on results), copies params in, runs bm_simulate on `stream`, copies the
- * results out, returns the scratch to the pool and synchronises the stream.  May be called from several host threads
+ * results out, returns the scratch to the pool and synchronises the stream.  With the parameter values in view it also
+ * resolves BM_EVENTS_AUTO to one form when all points fall on the same side of the break-even (one launch less; the
+ * results do not depend on the form).  May be called from several host threads
  * (the pool table is guarded by a mutex; calls on the same stream serialise on that stream as usual).
  * Having the values on the host, it also checks them: BM_ERR_INVALID_ARG for a non-finite entry, a negative D, lambda,
  * mu_a, mu_b or gamma, zeta <= 0 where lambda > 0, Fa <= 0 or Fb <= 0 where mu_a > 0, v0_hi < v0_lo -- for the sources
@@ -282,7 +291,9 @@ BM_API bm_status bm_box_muller_words(int32_t prec, const uint32_t *words, int32_
 
 /* Registers per thread, threads per block, resident blocks per SM, SM count and the Gaussian assignment selected
  * (bm_gauss, never AUTO; 0 for BM_F64), for the path kernel bm_simulate would launch for (cfg, n_points, n_paths)
- * (measurement aid; HOST outputs, each may be NULL). */
+ * (measurement aid; HOST outputs, each may be NULL).  Where bm_simulate launches both event forms (BM_EVENTS_AUTO with
+ * a jump source on), the figures are those of the CELLS form; set cfg->event_mode = BM_EVENTS_LANES to get the
+ * per-lane-clock form's. */
 BM_API bm_status bm_kernel_info(const bm_config *cfg, int32_t n_points, int64_t n_paths, int32_t *regs_per_thread,
                          int32_t *launch_threads, int32_t *blocks_per_sm, int32_t *sm_count, int32_t *gauss);
 

@@ -220,3 +220,13 @@ def vacf_from_trace(trace, i0, i):
     """Velocity autocovariance C(t_i - t_i0) = <v(t_i0) v(t_i)> - <v(t_i0)><v(t_i)> over the paths (unbiased, n - 1)."""
     a, b = trace[:, i0 - 1, 1], trace[:, i - 1, 1]
     return ((a - a.mean()) * (b - b.mean())).sum() / (a.size - 1)
+
+
+def hist_from_trace(trace_x, sample_steps, period, n_bins):
+    """Stationary density p(x mod L) of eq. (19), as a histogram: counts of frac(x / L) over n_bins equal
+    bins for the unfolded positions trace_x[path, step - 1] after the grid steps `sample_steps` (1-based)."""
+    x = trace_x[:, np.asarray(sample_steps) - 1]
+    u = x / period
+    u = u - np.floor(u)
+    b = np.minimum((u * n_bins).astype(np.int64), n_bins - 1)
+    return np.bincount(b.ravel(), minlength=n_bins)

@@ -207,6 +207,21 @@ bool valid_params_host(const bm_config *c, const bm_params *p, int32_t n_points)
   return true;
 }
 
+// BM_EVENTS_AUTO with the parameter values on the host: when every point of the table falls on the same side of the
+// break-even (the expression of lane_clock_point, common.cuh), the other form's launch would find no block to take --
+// name the form and save the launch.  Results do not depend on the mode (bit-identical by construction and by test).
+int resolve_event_mode_host(const bm_config *c, const bm_params *p, int32_t n_points, double dt) {
+  if (!has_event_modes(c) || c->event_mode != BM_EVENTS_AUTO) return c->event_mode;
+  bool any_lanes = false, any_cells = false;
+  for (int32_t i = 0; i < n_points; ++i) {
+    double rate = 0.0;
+    if ((c->noise & BM_NOISE_POISSON) && p[i].lambda > 0.0) rate += p[i].lambda;
+    if ((c->noise & BM_NOISE_DICH) && p[i].mu_a > 0.0) rate += 0.5 * (p[i].mu_a + (p[i].mu_b > 0.0 ? p[i].mu_b : 0.0));
+    (rate * dt > LCLK_EVENTS_PER_CELL ? any_lanes : any_cells) = true;
+  }
+  return any_lanes == any_cells ? BM_EVENTS_AUTO : (any_lanes ? BM_EVENTS_LANES : BM_EVENTS_CELLS);
+}
+
 long long blocks_per_point_of(const bm_config *c, int32_t n_points, int64_t n_paths) {
   const long long per_block = (long long)block_threads_of(c, n_points, n_paths) * paths_per_thread_of(c, n_points, n_paths);
   return (n_paths + per_block - 1) / per_block;
@@ -381,7 +396,9 @@ BM_API bm_status bm_simulate_host(const bm_config *cfg, const bm_params *params,
     if (cudaMallocFromPoolAsync(&d_ws, ws, pool, st) != cudaSuccess) break;
     if (ob && cudaMallocFromPoolAsync(&d_paths, ob, pool, st) != cudaSuccess) break;
     if (cudaMemcpyAsync(d_params, params, pb, cudaMemcpyHostToDevice, st) != cudaSuccess) break;
-    rc = bm_simulate(cfg, (const bm_params *)d_params, n_points, n_paths, n_steps, dt, seed, (bm_stats *)d_stats,
+    bm_config run = *cfg;
+    run.event_mode = resolve_event_mode_host(cfg, params, n_points, dt);
+    rc = bm_simulate(&run, (const bm_params *)d_params, n_points, n_paths, n_steps, dt, seed, (bm_stats *)d_stats,
                      (double *)d_paths, nullptr, d_ws, ws, stream);
     if (rc != BM_OK) break;
     rc = BM_ERR_CUDA;

@@ -1,6 +1,7 @@
 """Prints the polynomial coefficients of the fp64 kernels' own elementary functions (sim_f64.cuh: cos2pi_f64, log_u_f64,
 sincospi_f64): interpolants at the Chebyshev nodes of the argument range, computed with mpmath at 60 digits and rounded
-to double.  Run by hand when a range or degree changes; the output is pasted into sim_f64.cuh.  Not part of the oracle."""
+to double.  Run by hand when a range or degree changes; the output is pasted into sim_f64.cuh.  Not part of the oracle.
+tests/test_poly_tables.py runs it and checks that the tables in sim_f64.cuh are its output."""
 import mpmath as mp
 
 mp.mp.dps = 60
@@ -22,6 +23,11 @@ def show(name, c):
 
 
 sixteenth = mp.mpf(1) / 16
+# force cosine cos2pi_f64: cos(2 pi r) as a degree-12 polynomial in u = r^2 on [0, 1/16], split into the two Horner chains
+# in w = u^2 the kernel evaluates: E = (c12, c10, ..., c0), O = (c11, c9, ..., c1), highest coefficient first
+c2 = cheb_fit(lambda z: mp.cos(2 * mp.pi * mp.sqrt(z)), mp.mpf(0), sixteenth, 13)
+show("COS2PI_E", c2[12::-2])
+show("COS2PI_O", c2[11::-2])
 show("SINPI_C", cheb_fit(lambda z: mp.sin(mp.pi * mp.sqrt(z)) / mp.sqrt(z), mp.mpf(0), sixteenth, 8))   # sin(pi r) / r, z = r^2
 show("COSPI_C", cheb_fit(lambda z: mp.cos(mp.pi * mp.sqrt(z)), mp.mpf(0), sixteenth, 8))                 # cos(pi r)
 smax = (mp.sqrt(2) - 1) / (mp.sqrt(2) + 1)                     # s = f / (2 + f), f = m - 1, m in [sqrt(1/2), sqrt(2))

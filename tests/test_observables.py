@@ -13,15 +13,6 @@ from scipy import integrate
 from paper_1409_4923_b200 import workloads as W
 
 
-def hist_from_trace(trace_x, sample_steps, period, n_bins):
-    """Counts of frac(x / L) over bins for the unfolded positions after grid steps `sample_steps` (1-based)."""
-    x = trace_x[:, np.asarray(sample_steps) - 1]
-    u = x / period
-    u = u - np.floor(u)
-    b = np.minimum((u * n_bins).astype(np.int64), n_bins - 1)
-    return np.bincount(b.ravel(), minlength=n_bins)
-
-
 def boltzmann_bins(A1, A2, D, n_bins):
     f = lambda x: math.exp(-(A1 * math.sin(2 * math.pi * x) + A2 * math.sin(4 * math.pi * x)) / D)
     w = np.array([integrate.quad(f, i / n_bins, (i + 1) / n_bins)[0] for i in range(n_bins)])
@@ -34,7 +25,7 @@ def test_oracle_histogram_matches_boltzmann_density(orc):
     n_paths, n_steps = 512, 6000
     _, tr = orc.simulate(p, n_paths, n_steps, 4e-3, W.SEED, trace_paths=n_paths, trace_steps=n_steps)
     steps = np.arange(1200, n_steps + 1, 160)            # ~2.5 correlation times apart, after equilibration
-    counts = hist_from_trace(tr[:, :, 0], steps, 1.0, n_bins)
+    counts = orc.hist_from_trace(tr[:, :, 0], steps, 1.0, n_bins)
     n = counts.sum()
     assert n == n_paths * steps.size
     p_th = boltzmann_bins(A1, A2, D, n_bins)
@@ -75,7 +66,7 @@ def test_gpu_state_histogram_matches_oracle(orc, name, prec):
     got = counts.cpu().numpy()[0]
     _, tr = orc.simulate(w.params, w.n_paths, w.n_steps, w.dt, w.seed, model=w.model, potential=w.potential,
                          scheme=w.scheme, n_discard=w.n_discard, trace_paths=w.n_paths, trace_steps=w.n_steps)
-    ref = hist_from_trace(tr[:, :, 0], sample_steps, period, n_bins)
+    ref = orc.hist_from_trace(tr[:, :, 0], sample_steps, period, n_bins)
     assert got.sum() == ref.sum() == w.n_paths * len(sample_steps)
     if prec == "f64" and name != "C2":
         # same paths to 1e-12: only a position within rounding of a bin edge can change bins
