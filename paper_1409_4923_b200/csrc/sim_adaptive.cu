@@ -36,6 +36,14 @@ __global__ void __launch_bounds__(256) bm_paths_adaptive_f64(const __grid_consta
     const int K = a.adapt_levels;
     const long long TPC = 1LL << K;  // ticks per grid step
     const double tol = a.adapt_tol, tol8 = 0.125 * a.adapt_tol;
+    // Per level k: the interval length dt 2^-k and the noise amplitude sqrt(2 D H) of a sub-step that covers a whole
+    // interval -- the same expressions the time loop used to evaluate per interval and per sub-step (a library scalbn and
+    // an fp64 square root each time), so the values are the same bits; a sub-step cut short by an event takes its own root.
+    double H_of[21], amp_of[21];
+    for (int k = 0; k <= K; ++k) {
+      H_of[k] = scalbn(dt, -k);
+      amp_of[k] = sqrt(2.0 * P.D * H_of[k]);
+    }
 
     const uint4 wi = philox_call(a.keys, g, STREAM_INIT, 0);  // R4
     StateF64 s;
@@ -66,7 +74,8 @@ __global__ void __launch_bounds__(256) bm_paths_adaptive_f64(const __grid_consta
       long long tick = 0;
       while (tick < TPC) {
         const long long wd = TPC >> k;                  // interval width in ticks
-        const double H = scalbn(dt, -k);                // its length, exactly dt 2^-k
+        const double H = H_of[k];                       // its length, exactly dt 2^-k
+        const double ampH = amp_of[k];
         double rem = H, chi_max = 0.0;
         while (rem > 0.0) {
           double h = rem;
@@ -84,7 +93,7 @@ __global__ void __launch_bounds__(256) bm_paths_adaptive_f64(const __grid_consta
           }
           m++;
           const double cst = P.c0 + (onD ? (d ? P.Fb : -P.Fa) : 0.0);
-          const double dxi = HAS_G ? sqrt(2.0 * P.D * h) * gn : 0.0;
+          const double dxi = HAS_G ? ((h == H) ? ampH : amp_of_substep_f64(P.D, h)) * gn : 0.0;
           // Alg. 1; chi = predictor (line 4) - corrector (line 6)
           const double x = s.xi;
           const double F1 = minus_dV_f64<POT>(P, x) + cst;
@@ -120,7 +129,7 @@ __global__ void __launch_bounds__(256) bm_paths_adaptive_f64(const __grid_consta
         }
         tick += wd;
         if (chi_max > tol && k < K) k += 1;
-        else if (chi_max < tol8 && k > 0 && (tick % (2 * wd)) == 0) k -= 1;
+        else if (chi_max < tol8 && k > 0 && (tick & (2 * wd - 1)) == 0) k -= 1;  // wd is a power of two: aligned to 2 wd
       }
       if (tracing && n + 1 <= a.trace_steps) {
         trace[2 * n] = unfolded_f64<POT>(s);
