@@ -289,6 +289,14 @@ BM_API bm_status bm_gauss_fill(int32_t prec, int32_t gauss, uint64_t seed, uint6
  * 16-byte aligned.  Errors: BM_ERR_INVALID_ARG. */
 BM_API bm_status bm_box_muller_words(int32_t prec, const uint32_t *words, int32_t n_pairs, void *out, void *stream);
 
+/* The normal of a sub-step that ENDS ON AN EVENT in the BM_F32 kernels (reading R13; the jump adaptation of
+ * PAPER.md:301 cuts a grid step at a kick or flip, and the piece before it needs its own Gaussian increment, eq. 9): it
+ * comes from word 2 of the event's own Philox call (call k of the Poisson or dichotomous stream: bm_philox_fill with
+ * stream_id 2 or 3), radius from the word's top 23 bits, angle from its low 16.  No Gaussian-stream fill reaches that
+ * code, so this call applies it to GIVEN words: out[i] = the normal of words[i].  words, out: device, n > 0.
+ * Errors: BM_ERR_INVALID_ARG. */
+BM_API bm_status bm_event_normal_words(const uint32_t *words, int32_t n, float *out, void *stream);
+
 /* Registers per thread, threads per block, resident blocks per SM, SM count and the Gaussian assignment selected
  * (bm_gauss, never AUTO; 0 for BM_F64), for the path kernel bm_simulate would launch for (cfg, n_points, n_paths)
  * (measurement aid; HOST outputs, each may be NULL).  Where bm_simulate launches both event forms (BM_EVENTS_AUTO with

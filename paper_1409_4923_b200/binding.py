@@ -32,7 +32,7 @@ BM_STATE_SLOTS, BM_CHUNK_ALIGN = 16, 8
 BM_MOM_STRIDE = 10
 BM_STATIC_SCRATCH_BYTES = 4 * 1024 * 1024
 EXPORTS = ("bm_workspace_bytes", "bm_simulate", "bm_simulate_static", "bm_simulate_dt", "bm_state_bytes", "bm_simulate_chunk", "bm_state_histogram",
-           "bm_state_moments", "bm_simulate_host", "bm_philox_fill", "bm_gauss_fill", "bm_box_muller_words",
+           "bm_state_moments", "bm_simulate_host", "bm_philox_fill", "bm_gauss_fill", "bm_box_muller_words", "bm_event_normal_words",
            "bm_kernel_info", "bm_pipe_probe", "bm_status_string", "bm_version")
 STATS_FIELDS = ("n", "mean_v", "var_v", "mean_xT", "var_xT", "mean_jumps", "mean_substeps", "rsv")
 
@@ -88,6 +88,8 @@ def lib():
         L.bm_gauss_fill.restype = C.c_int
         L.bm_box_muller_words.argtypes = [i32, vp, i32, vp, vp]
         L.bm_box_muller_words.restype = C.c_int
+        L.bm_event_normal_words.argtypes = [vp, i32, vp, vp]
+        L.bm_event_normal_words.restype = C.c_int
         ip = C.POINTER(C.c_int32)
         L.bm_kernel_info.argtypes = [cfgp, i32, i64, ip, ip, ip, ip, ip]
         L.bm_kernel_info.restype = C.c_int
@@ -306,6 +308,17 @@ def bm_box_muller_words(prec, words, n_pairs, out, stream=None):
     rc = lib().bm_box_muller_words(prec, C.c_void_p(words.data_ptr()), n_pairs, C.c_void_p(out.data_ptr()), _stream_ptr(stream))
     if rc != BM_OK:
         raise BmError(rc, "bm_box_muller_words")
+
+
+def bm_event_normal_words(words, out, stream=None):
+    """words: CUDA int32/uint32 tensor [n] (word 2 of event Philox calls); out: CUDA float32 tensor [n] = the normal the
+    fp32 kernels give the sub-step that ends on that event (reading R13)."""
+    import torch
+    assert words.is_cuda and words.dtype in (torch.int32, torch.uint32) and words.is_contiguous()
+    assert out.is_cuda and out.dtype == torch.float32 and out.is_contiguous() and out.numel() == words.numel()
+    rc = lib().bm_event_normal_words(C.c_void_p(words.data_ptr()), words.numel(), C.c_void_p(out.data_ptr()), _stream_ptr(stream))
+    if rc != BM_OK:
+        raise BmError(rc, "bm_event_normal_words")
 
 
 def bm_pipe_probe(op, iters, blocks, threads, sink, stream=None):

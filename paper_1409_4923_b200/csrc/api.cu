@@ -440,6 +440,11 @@ BM_API bm_status bm_box_muller_words(int32_t prec, const uint32_t *words, int32_
   return launch_box_muller_words(prec, words, n_pairs, out, reinterpret_cast<cudaStream_t>(stream)) == cudaSuccess ? BM_OK : BM_ERR_CUDA;
 }
 
+BM_API bm_status bm_event_normal_words(const uint32_t *words, int32_t n, float *out, void *stream) {
+  if (!words || !out || n <= 0 || ((uintptr_t)words & 3) || ((uintptr_t)out & 3)) return BM_ERR_INVALID_ARG;
+  return launch_event_normal_words(words, n, out, reinterpret_cast<cudaStream_t>(stream)) == cudaSuccess ? BM_OK : BM_ERR_CUDA;
+}
+
 BM_API bm_status bm_kernel_info(const bm_config *cfg, int32_t n_points, int64_t n_paths, int32_t *regs_per_thread,
                          int32_t *launch_threads, int32_t *blocks_per_sm, int32_t *sm_count, int32_t *gauss) {
   if (!valid_cfg(cfg) || n_points <= 0 || n_paths <= 0) return BM_ERR_INVALID_ARG;

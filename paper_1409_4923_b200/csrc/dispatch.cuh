@@ -33,6 +33,7 @@ cudaError_t launch_philox_fill(const PhiloxKeys &K, unsigned long long path0, in
 cudaError_t launch_gauss_fill(int prec, int gauss, const PhiloxKeys &K, unsigned long long path0, int n_paths,
                               unsigned long long m0, int n_m, void *out, cudaStream_t st);
 cudaError_t launch_box_muller_words(int prec, const uint32_t *words, int n_pairs, void *out, cudaStream_t st);
+cudaError_t launch_event_normal_words(const uint32_t *words, int n, float *out, cudaStream_t st);
 cudaError_t launch_grid_reduce(const double *partials, int n_points, int blocks_per_point, bm_stats *out,
                                cudaStream_t st);
 cudaError_t launch_state_hist(const unsigned long long *state, int n_points, long long n_paths, int kind, double inv_period,

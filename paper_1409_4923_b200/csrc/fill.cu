@@ -88,6 +88,18 @@ __global__ void box_muller_words_kernel(int prec, const uint32_t *__restrict__ w
   }
 }
 
+// The normal of a sub-step that ends on an event (R13) on GIVEN words: the device code the fp32 path kernels apply to
+// word 2 of the event's Philox call (bm_event_normal_words).
+__global__ void event_normal_words_kernel(const uint32_t *__restrict__ words, int n, float *__restrict__ out) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) out[i] = event_normal_f32(words[i]);
+}
+
+cudaError_t launch_event_normal_words(const uint32_t *words, int n, float *out, cudaStream_t st) {
+  event_normal_words_kernel<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(words, n, out);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_box_muller_words(int prec, const uint32_t *words, int n_pairs, void *out, cudaStream_t st) {
   box_muller_words_kernel<<<(unsigned)((n_pairs + 127) / 128), 128, 0, st>>>(prec, words, n_pairs, out);
   return cudaGetLastError();

@@ -261,6 +261,15 @@ __device__ __forceinline__ Pair pair_w16p(uint32_t w, float cn) {
 }
 
 // Gaussian-stream call b serves NB = 4 (W32) or 8 (W16, W16P) consecutive grid cells = NB/2 Box-Muller pairs
+// Standard normal of a sub-step that ends on an event, from the third word of the event's own Philox call (R13): radius
+// from the word's top 23 bits, angle from its low 16 (the W16 assignment), cosine member of the pair.  Used by the path
+// kernels and, on given words, by bm_event_normal_words.
+__device__ __forceinline__ float event_normal_f32(uint32_t w) {
+  const float r = sqrt_approx(-2.0f * LN2_F * lg2_approx(u01_open0_f32(w)));
+  const float t = __uint_as_float((w & 0xFFFFu) | 0x3F800000u);
+  return r * cos_approx(fmaf(t, 128.0f * TWO_PI_F, -128.0f * TWO_PI_F));
+}
+
 template <int GW> struct GaussLayout {
   static constexpr int NB = GW == BM_GAUSS_W32 ? 4 : 8;
   static constexpr int NP = NB / 2;
@@ -444,11 +453,7 @@ __global__ void BM_F32_BOUNDS(MODEL, OCC) bm_paths_f32(const __grid_constant__ S
 
   // Standard normal of the sub-step that ends on an event, from the third word of the event's Philox call (R13):
   // radius from its top 23 bits, angle from its low 16 (the W16 assignment).
-  auto event_normal = [&](uint32_t w) -> float {
-    const float r = sqrt_approx(-2.0f * LN2_F * lg2_approx(u01_open0_f32(w)));
-    const float t = __uint_as_float((w & 0xFFFFu) | 0x3F800000u);
-    return r * cos_approx(fmaf(t, 128.0f * TWO_PI_F, -128.0f * TWO_PI_F));
-  };
+  auto event_normal = [](uint32_t w) -> float { return event_normal_f32(w); };
 
   const int n_discard = (int)a.n_discard;
   // next event of each stream: (cell index, offset inside that cell); NEVER = switched off at this point.  qP, qD:

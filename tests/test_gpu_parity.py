@@ -113,6 +113,40 @@ def test_gauss_f32_w16_is_standard_normal(B, orc, gauss):
                 assert abs(got[p, j + 1] - r * math.sin(ang)) < 2e-5 * (1 + r)
 
 
+@pytest.mark.parametrize("stream", [2, 3])
+def test_event_normal_of_r13_word_by_word(B, orc, stream):
+    """Reading R13: the sub-step that ends on event k of a jump stream takes its normal from word 2 of call k of THAT stream
+    (radius from the top 23 bits, angle from the low 16).  No Gaussian-stream fill reaches that code; here the words of
+    calls k = 0.. of the Poisson (2) and dichotomous (3) streams go through it: every normal against the definition, and
+    the sample against the standard normal law (moments, KS) and against the kick amplitude drawn from word 1 of the same
+    call (no correlation)."""
+    import torch
+    from scipy import stats as st
+    n_paths, n_k = 512, 256
+    raw = torch.zeros((n_paths, n_k, 4), dtype=torch.int32, device="cuda")
+    B.bm_philox_fill(W.SEED, 3, n_paths, stream, 0, n_k, raw)
+    words = raw[:, :, 2].contiguous().view(-1)
+    out = torch.zeros(words.numel(), dtype=torch.float32, device="cuda")
+    B.bm_event_normal_words(words, out)
+    torch.cuda.synchronize()
+    w = words.cpu().numpy().view(np.uint32).astype(np.int64)
+    got = out.cpu().numpy().astype(np.float64)
+    assert int(w.reshape(n_paths, n_k)[5, 7]) == orc.philox_call(W.SEED, 3 + 5, stream, 7)[2]            # the oracle's word
+    u = ((w >> 9) + 1) * 2.0 ** -23
+    r = np.sqrt(-2.0 * np.log(u))
+    exp = r * np.cos(2 * math.pi * (w & 0xFFFF) / 65536.0)
+    assert np.abs(got - exp).max() < 2e-5 * (1 + r.max()), np.abs(got - exp).max()
+    assert np.all(np.abs(got - exp) < 2e-5 * (1 + r))
+    n = got.size
+    assert abs(got.mean()) < 4 / math.sqrt(n) and abs(got.var() - 1) < 4 * math.sqrt(2 / n)
+    assert abs((got ** 3).mean()) < 4 * math.sqrt(15 / n) and abs((got ** 4).mean() - 3) < 4 * math.sqrt(96 / n)
+    assert st.kstest(got[::5], "norm").statistic < 1.63 / math.sqrt(n / 5)
+    w1 = raw[:, :, 1].contiguous().view(-1).cpu().numpy().view(np.uint32).astype(np.float64)
+    amp = -np.log((w1 + 0.5) / 4294967296.0)            # the kick amplitude / the other words of the same call
+    assert abs(np.corrcoef(got, amp)[0, 1]) < 4 / math.sqrt(n)
+    assert abs(np.corrcoef(got[:-1], got[1:])[0, 1]) < 4 / math.sqrt(n)
+
+
 # ---- fp64 per-path parity, overdamped ---------------------------------------------------------------------
 
 def check_fp64_overdamped(B, orc, w, ids=None, what="", ref=None):
